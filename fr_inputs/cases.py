@@ -1,0 +1,85 @@
+"""Assemble complete, seeded problem instances ("cases") for the configs of BASELINE.json.
+
+A case carries exactly what `fr_setup` takes (include/frb200.h) and what the oracle takes
+(oracle/fr_oracle.py `rhs`): operators, metric terms, flux-point pairs, boundary lists, parameters and
+an initial state.  It contains no right-hand-side arithmetic.
+"""
+import numpy as np
+
+from . import mesh as _mesh
+from . import refelem, state
+
+SEEDS = dict(c1=14090405, c2=14090406, c3=14090407, c4=14090408, c5=14090409)
+
+
+def build_case(m, p, system="euler", gamma=state.GAMMA, mu=0.0, prandtl=0.72, ldg_beta=0.5, ldg_tau=0.1,
+               bc_types=None, bc_params=None, by_coords=False):
+    """mesh dict -> case dict(cfg, etypes, eles, ifc, bcs).  `bc_types`: {tag: 'wall'|'farfield'}."""
+    eles, geo = [], {}
+    for t in m["etypes"]:
+        ops = refelem.operators(t, p)
+        g = _mesh.geometry(t, p, m["xv"][t])
+        geo[t] = g
+        e = dict(etype=t, order=p, nupts=ops["nupts"], nfpts=ops["nfpts"], neles=m["xv"][t].shape[0],
+                 affine=g["affine"], smats=g["smats"], rcpdjac=g["rcpdjac"], djac=g["djac"], xu=g["xu"],
+                 wts=ops["wts"], fwts=ops["fwts"])
+        for k in ("M0", "M132", "M3", "M460", "M6"):
+            e[k] = ops[k]
+        eles.append(e)
+    if by_coords:
+        ifc, bf = _mesh.connectivity_by_coords(m, p, geo)
+    else:
+        ifc, bf = _mesh.connectivity(m, p, geo)
+    bcs = []
+    for tag in sorted(bf):
+        b = dict(bf[tag])
+        b["type"] = bc_types[tag]
+        b["params"] = list(bc_params[tag])
+        bcs.append(b)
+    cfg = dict(system=system, gamma=gamma, mu=mu, prandtl=prandtl, ldg_beta=ldg_beta, ldg_tau=ldg_tau)
+    return dict(cfg=cfg, etypes=list(m["etypes"]), order=p, eles=eles, ifc=ifc, bcs=bcs, geo=geo, mesh=m)
+
+
+def ndof(case):
+    """DOF = sum over types of N_u * N_e (solution points; reading R22)."""
+    return int(sum(e["nupts"] * e["neles"] for e in case["eles"]))
+
+
+def config1(numbering="natural"):
+    """BASELINE.json configs[0]: 384 Kuhn tets on the periodic cube [0,2pi]^3, p=2, Euler, FP64,
+    freestream rho=1, v=(0.3,0,0), p=1/gamma + seeded 1 % perturbation (reading R17)."""
+    m = _mesh.box_tets(4, 2 * np.pi, numbering=numbering, seed=SEEDS["c1"])
+    case = build_case(m, 2, system="euler")
+    fs = dict(rho=1.0, v=(0.3, 0.0, 0.0), p=1.0 / state.GAMMA)
+    u0 = [state.freestream(e["xu"], **fs) for e in case["eles"]]
+    case["u0"] = state.perturb(u0, 0.01, SEEDS["c1"], **fs)
+    return case
+
+
+def config2(n=16, p=3, system="ns", mu=1e-3, numbering="natural", state_kind="vortex"):
+    """BASELINE.json configs[1]: periodic unit box, n^3 cells, lower half prisms / upper half tets
+    (reading R18 for the counts), NS mu=1e-3 Pr=0.72, LDG beta=1/2 tau=0.1, isentropic vortex."""
+    m = _mesh.box_mixed(n, 1.0, numbering=numbering, seed=SEEDS["c2"])
+    case = build_case(m, p, system=system, mu=mu if system == "ns" else 0.0)
+    if state_kind == "vortex":
+        case["u0"] = [state.isentropic_vortex(e["xu"]) for e in case["eles"]]
+    else:
+        case["u0"] = [state.smooth_periodic(e["xu"]) for e in case["eles"]]
+    return case
+
+
+def config3(p=4, ntheta=100, nz=15, nlayers=40, nr=40, numbering="morton", system="ns", amp=0.005, seed=None):
+    """BASELINE.json configs[2] (and [4] when scaled): cylinder-like O-mesh, NS at Re=3900, M=0.2
+    (PAPER.md:86-94,116), wall T_w = T_inf, far field = freestream, seeded 0.5 % perturbation."""
+    seed = SEEDS["c3"] if seed is None else seed
+    m = _mesh.cylinder_omesh(ntheta, nz, nlayers, nr, numbering=numbering, seed=seed)
+    gamma, mach = state.GAMMA, 0.2
+    fs = dict(rho=1.0, v=(1.0, 0.0, 0.0), p=1.0 / (gamma * mach * mach))
+    e_w = fs["p"] / ((gamma - 1) * fs["rho"])
+    case = build_case(m, p, system=system, mu=1.0 / 3900.0 if system == "ns" else 0.0,
+                      bc_types={0: "wall", 1: "farfield"},
+                      bc_params={0: [e_w], 1: [fs["rho"], *fs["v"], fs["p"]]})
+    u0 = [state.freestream(e["xu"], **fs) for e in case["eles"]]
+    case["u0"] = state.perturb(u0, amp, seed, **fs) if amp > 0 else u0
+    case["freestream"] = fs
+    return case

@@ -1,0 +1,124 @@
+"""Pins for the synthetic meshes, metric terms and flux-point connectivity (inputs of both sides)."""
+import numpy as np
+import pytest
+
+from fr_inputs import cases, mesh as M, refelem as R
+
+
+def _geo(m, p):
+    return {t: M.geometry(t, p, m["xv"][t]) for t in m["etypes"]}
+
+
+MESHES = {
+    "tets4": lambda: M.box_tets(4),
+    "mixed4": lambda: M.box_mixed(4),
+    "mixed4_random": lambda: M.box_mixed(4, numbering="random", seed=3),
+    "cyl": lambda: M.cylinder_omesh(ntheta=16, nz=4, nlayers=5, nr=5, seed=11),
+}
+
+
+@pytest.mark.parametrize("name", list(MESHES))
+@pytest.mark.parametrize("p", [1, 3])
+def test_pairs_cover_every_flux_point_once_and_coincide(name, p):
+    m = MESHES[name]()
+    geo = _geo(m, p)
+    ifc, bf = M.connectivity(m, p, geo)
+    seen = {ti: np.zeros((R.operators(t, p)["nfpts"], m["xv"][t].shape[0]), dtype=int) for ti, t in enumerate(m["etypes"])}
+    for s in ("l", "r"):
+        for ti in seen:
+            k = ifc[s + "_et"] == ti
+            np.add.at(seen[ti], (ifc[s + "_fpt"][k], ifc[s + "_ele"][k]), 1)
+    for b in bf.values():
+        for ti in seen:
+            k = b["et"] == ti
+            np.add.at(seen[ti], (b["fpt"][k], b["ele"][k]), 1)
+    assert all(np.all(v == 1) for v in seen.values())
+    # physical coordinates of paired points coincide (modulo the period); normals are opposite
+    n = len(ifc["l_et"])
+    xl, xr, nr, wl, wr = np.zeros((n, 3)), np.zeros((n, 3)), np.zeros((n, 3)), np.zeros(n), np.zeros(n)
+    for ti, t in enumerate(m["etypes"]):
+        g, fw = geo[t], R.operators(t, p)["fwts"]
+        k = ifc["l_et"] == ti
+        xl[k] = g["xf"][ifc["l_fpt"][k], ifc["l_ele"][k]]
+        wl[k] = fw[ifc["l_fpt"][k]]
+        k = ifc["r_et"] == ti
+        xr[k] = g["xf"][ifc["r_fpt"][k], ifc["r_ele"][k]]
+        nr[k] = g["fnorm"][ifc["r_fpt"][k], :, ifc["r_ele"][k]]
+        wr[k] = fw[ifc["r_fpt"][k]]
+    d = xl - xr
+    for a in range(3):
+        if m["period"][a]:
+            d[:, a] -= m["period"][a] * np.round(d[:, a] / m["period"][a])
+    assert np.abs(d).max() < 1e-12
+    assert np.abs(ifc["nl"].T + nr).max() < 1e-10
+    # mag_L w_L = mag_R w_R: both sides integrate the same physical face
+    assert np.abs(ifc["magl"] * wl - ifc["magr"] * wr).max() < 1e-12 * np.abs(ifc["magl"] * wl).max()
+    # L is the side with the smaller (et, ele); pairs sorted by (l_et, l_fpt, l_ele)
+    assert np.all((ifc["l_et"] < ifc["r_et"]) | ((ifc["l_et"] == ifc["r_et"]) & (ifc["l_ele"] <= ifc["r_ele"])))
+    key = (ifc["l_et"].astype(np.int64) << 50) + (ifc["l_fpt"].astype(np.int64) << 40) + ifc["l_ele"]
+    assert np.all(np.diff(key) > 0)
+
+
+@pytest.mark.parametrize("name", ["tets4", "mixed4"])
+def test_vertex_pairing_equals_coordinate_pairing(name):
+    m = MESHES[name]()
+    geo = _geo(m, 2)
+    a, _ = M.connectivity(m, 2, geo)
+    b, _ = M.connectivity_by_coords(m, 2, geo)
+    for k in a:
+        assert np.array_equal(a[k], b[k]) if a[k].dtype.kind == "i" else np.allclose(a[k], b[k], atol=1e-14)
+
+
+@pytest.mark.parametrize("name", list(MESHES))
+def test_closed_elements_and_volume(name):
+    p = 2
+    m = MESHES[name]()
+    geo = _geo(m, p)
+    vol = 0.0
+    for t in m["etypes"]:
+        o, g = R.operators(t, p), geo[t]
+        # sum over flux points of w * mag * n = integral of the outward normal over a closed surface = 0
+        closed = np.einsum("f,fe,fie->ie", o["fwts"], g["fmag"], g["fnorm"])
+        h2 = (np.einsum("f,fe->e", o["fwts"], g["fmag"]))
+        assert np.abs(closed).max() < 1e-12 * h2.max()
+        vol += (o["wts"][:, None] * g["djac"]).sum()
+        assert np.allclose(g["smats"][:, :, :, 0].transpose(2, 0, 1) @ np.linalg.inv(g["smats"][:, :, :, 0].transpose(2, 0, 1)),
+                           np.eye(3)[None], atol=1e-12)
+    if name == "tets4":
+        assert abs(vol - (2 * np.pi) ** 3) < 1e-11 * vol
+    if name.startswith("mixed"):
+        assert abs(vol - 1.0) < 1e-13
+    if name == "cyl":
+        # straight-sided O-mesh: volume = (outer polygon through the rectangle - inner 16-gon) x span pi
+        nth = 16
+        th = 2 * np.pi * np.arange(nth) / nth
+        c, s_ = np.cos(th), np.sin(th)
+        with np.errstate(divide="ignore"):
+            ro = np.minimum(np.where(c > 0, 25.0, 9.0) / np.abs(c), 9.0 / np.abs(s_))
+        outer = 0.5 * np.sum(ro * np.roll(ro, -1)) * np.sin(2 * np.pi / nth)
+        inner = 0.5 * nth * 0.25 * np.sin(2 * np.pi / nth)
+        assert abs(vol - (outer - inner) * np.pi) < 1e-10 * vol
+
+
+def test_config_counts():
+    # reading R18: 16^3 cells -> 4096 prisms + 12288 tets
+    m = M.box_mixed(16)
+    assert m["xv"]["pri"].shape[0] == 4096 and m["xv"]["tet"].shape[0] == 12288
+    c = cases.config1()
+    assert c["eles"][0]["neles"] == 384 and c["eles"][0]["nupts"] == 10 and len(c["ifc"]["l_et"]) == 4608
+    assert cases.ndof(c) == 3840
+
+
+def test_cylinder_bc_lists():
+    m = M.cylinder_omesh(ntheta=16, nz=4, nlayers=5, nr=5, seed=11)
+    p = 2
+    geo = _geo(m, p)
+    _, bf = M.connectivity(m, p, geo)
+    T = 6
+    assert len(bf[0]["et"]) == 2 * 16 * 4 * T and len(bf[1]["et"]) == 2 * 16 * 4 * T
+    assert np.all(bf[0]["et"] == 1) and np.all(bf[1]["et"] == 0)      # wall on prisms, far field on tets
+    # wall normals point towards the axis, far-field normals away from it
+    xw = geo["pri"]["xf"][bf[0]["fpt"], bf[0]["ele"]]
+    assert np.all(np.einsum("in,ni->n", bf[0]["n"][:2], xw[:, :2]) < 0)
+    xo = geo["tet"]["xf"][bf[1]["fpt"], bf[1]["ele"]]
+    assert np.all(np.einsum("in,ni->n", bf[1]["n"][:2], xo[:, :2]) > 0)

@@ -1,0 +1,27 @@
+"""Shared helpers for the tests (no method arithmetic)."""
+import numpy as np
+
+
+def field_errors(got, ref):
+    """Max-norm relative error per conserved variable, jointly over element types (reading R16):
+    err_k = max |got - ref| / max |ref| over all types, points and elements, for variable k."""
+    num, den = np.zeros(5), np.zeros(5)
+    for g, r in zip(got, ref):
+        num = np.maximum(num, np.abs(g - r).max(axis=(0, 2)))
+        den = np.maximum(den, np.abs(r).max(axis=(0, 2)))
+    return num / np.maximum(den, 1e-300), den
+
+
+def conservation_defect(case, dudt):
+    """sum_types sum_e sum_rho omega_rho |J| dudt, relative to the same sum of absolute values (T2)."""
+    tot, ab = np.zeros(5), np.zeros(5)
+    for e, d in zip(case["eles"], dudt):
+        w = e["wts"][:, None, None] * e["djac"][:, None, :]
+        tot += (w * d).sum(axis=(0, 2))
+        ab += np.abs(w * d).sum(axis=(0, 2))
+    return tot / np.maximum(ab, 1e-300)
+
+
+def oracle_rhs(case, us=None):
+    from oracle import fr_oracle
+    return fr_oracle.rhs(case["cfg"], case["eles"], case["ifc"], case["bcs"], case["u0"] if us is None else us)
