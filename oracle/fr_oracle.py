@@ -140,8 +140,9 @@ def _apply(A, B):
 
 
 # ----------------------------------------------------------------------------- right-hand side
-def rhs(cfg, eles, ifc, bcs, us):
-    """One evaluation of d u / d t, steps 1-6 of SURVEY 8(c).
+def rhs(cfg, eles, ifc, bcs, us, parts=None):
+    """One evaluation of d u / d t, steps 1-6 of SURVEY 8(c).  If `parts` is a dict it receives the
+    intermediates `ftil` (F~) and `d` (D) of step 6, for a-priori round-off bounds in the tests.
 
     cfg  : dict(system='euler'|'ns', gamma, mu, prandtl, ldg_beta, ldg_tau)
     eles : per element type dict(M0, M132, M3, M460, M6, smats [3,3,N_u,N_e], rcpdjac [N_u,N_e])
@@ -223,6 +224,8 @@ def rhs(cfg, eles, ifc, bcs, us):
             Fb = Fb - sum(fv[i] * b["n"][i] for i in range(3)) + tau * (ubL - uv)
         _scatter(d, b["et"], b["fpt"], b["ele"], b["mag"] * Fb)
 
+    if parts is not None:
+        parts.update(ftil=ftil, d=d)
     # step 6: R = M132 F~ + M3 D ; dudt = -R / |J|
     out = []
     for e, ft, dd in zip(eles, ftil, d):

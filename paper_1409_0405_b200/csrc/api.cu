@@ -1,0 +1,725 @@
+// C ABI (include/frb200.h): context set-up, device data model, RHS stage driver, Runge-Kutta graphs.
+#include <algorithm>
+#include <cmath>
+#include <cstring>
+#include <memory>
+#include <numeric>
+
+#include "kernels.cuh"
+
+namespace frb {
+
+static thread_local std::string g_error;
+
+struct CtxBase {
+  fr_prec prec;
+  std::string err;
+  long long launches = 0;
+  virtual ~CtxBase() {}
+  virtual void state_layout(int et, int64_t *ld, int64_t *nbytes) const = 0;
+  virtual void rhs(const void *const *u, void *const *dudt) = 0;
+  virtual void set_state(const double *const *u) = 0;
+  virtual void get_state(double *const *u) = 0;
+  virtual void rk_step(double dt, long long nsteps) = 0;
+  virtual void sync() = 0;
+  virtual void profile(int reps, double ms[4], fr_kernel_stat *out, int cap, int *n) = 0;
+  virtual void rk_step_host(double dt, void *const *u_host) = 0;
+};
+
+template <typename T>
+struct DevBuf {
+  T *p = nullptr;
+  size_t n = 0;
+  void alloc(size_t count, bool zero = true) {
+    n = count;
+    if (count == 0) return;
+    cudaError_t e = cudaMalloc(&p, count * sizeof(T));
+    if (e != cudaSuccess) throw Error{FR_ENOMEM, std::string("cudaMalloc: ") + cudaGetErrorString(e)};
+    if (zero) FR_CUDA_TRY(cudaMemset(p, 0, count * sizeof(T)));
+  }
+  void upload(const std::vector<T> &h) {
+    alloc(h.size(), false);
+    if (n) FR_CUDA_TRY(cudaMemcpy(p, h.data(), n * sizeof(T), cudaMemcpyHostToDevice));
+  }
+  ~DevBuf() {
+    if (p) cudaFree(p);
+  }
+  DevBuf() = default;
+  DevBuf(const DevBuf &) = delete;
+  DevBuf &operator=(const DevBuf &) = delete;
+};
+
+enum { CAT_GEMM = 0, CAT_PW = 1, CAT_IFACE = 2 };
+
+// Per-kernel CUDA-event timeline of one RHS evaluation (measurement aid; never active on the normal path).
+struct Timeline {
+  std::vector<cudaEvent_t> ev;
+  std::vector<int> cat;
+  std::vector<std::string> name;
+  std::vector<double> bytes, flops;
+  cudaStream_t s;
+  void mark(int c, const std::string &nm = "", double b = 0, double f = 0) {
+    cudaEvent_t e;
+    cudaEventCreate(&e);
+    cudaEventRecord(e, s);
+    ev.push_back(e);
+    cat.push_back(c);
+    name.push_back(nm);
+    bytes.push_back(b);
+    flops.push_back(f);
+  }
+};
+
+template <typename T>
+struct EleData {
+  EleView<T> view;
+  DevBuf<T> smats, rcpdjac;
+  GemmPlan<T> pM0, pM132, pM3, pM460, pM6;
+  DevBuf<T> X, Y, ACC;   // solution register, stage input, RK4 accumulator
+  DevBuf<T> grad;        // [3][nupts][5][ld]: G~ -> G -> F~
+  DevBuf<T> R;           // [nupts][5][ld]
+  ~EleData() {
+    gemm_plan_free(pM0);
+    gemm_plan_free(pM132);
+    gemm_plan_free(pM3);
+    gemm_plan_free(pM460);
+    gemm_plan_free(pM6);
+  }
+};
+
+template <typename T>
+struct BndData {
+  BndView<T> view;
+  DevBuf<BndRec> recs;
+  DevBuf<T> nrm, mag;
+};
+
+template <typename T>
+struct Ctx : CtxBase {
+  fr_system system;
+  fr_stepper stepper;
+  fr_mode mode;
+  PhysParams<T> ph;
+  cudaStream_t stream = nullptr;
+  bool own_stream = false;
+  int nt = 0;
+  std::vector<std::unique_ptr<EleData<T>>> el;
+  const char *tname[FR_MAXTYPES] = {"t0", "t1", "t2", "t3"};
+  TypeTab tt;
+  DevBuf<T> uf, cf, gf;
+  IfaceView<T> iv;
+  DevBuf<PairRec> pairs;
+  DevBuf<T> nl, magl, magr;
+  std::vector<std::unique_ptr<BndData<T>>> bnd;
+  DevBuf<StageCoef> coef;
+  StageCoef *coef_host = nullptr;   // pinned
+  double coef_dt = std::nan("");
+  cudaGraphExec_t graph = nullptr;
+  int graph_kernels = 0;
+
+  ~Ctx() override {
+    if (graph) cudaGraphExecDestroy(graph);
+    if (coef_host) cudaFreeHost(coef_host);
+    if (own_stream && stream) cudaStreamDestroy(stream);
+  }
+
+  // ------------------------------------------------------------------ set-up
+  void setup(const fr_config *c) {
+    prec = c->prec;
+    system = c->system;
+    stepper = c->stepper;
+    mode = c->mode;
+    stream = (cudaStream_t)c->cuda_stream;
+    if (!stream) {
+      // the legacy default stream cannot be captured into a graph: use an own *blocking* stream, which keeps the
+      // implicit ordering with work the caller enqueues on the default stream
+      FR_CUDA_TRY(cudaStreamCreate(&stream));
+      own_stream = true;
+    }
+    FR_REQUIRE(c->gamma > 1.0, "gamma must be > 1");
+    const bool ns = system == FR_NAVIER_STOKES;
+    FR_REQUIRE(!ns || (c->mu >= 0.0 && c->prandtl > 0.0), "mu must be >= 0 and prandtl > 0");
+    ph.gamma = (T)c->gamma;
+    ph.mu = (T)(ns ? c->mu : 0.0);
+    ph.prandtl = (T)(ns ? c->prandtl : 1.0);
+    ph.beta = (T)(ns ? c->ldg_beta : 0.0);
+    ph.tau = (T)(ns ? c->ldg_tau : 0.0);
+    ph.ns = ns ? 1 : 0;
+    nt = c->netypes;
+    FR_REQUIRE(nt >= 1 && nt <= FR_MAXTYPES && c->eles, "netypes must be in [1,4] and eles non-NULL");
+    FR_REQUIRE(c->ifaces, "ifaces must be non-NULL");
+
+    long long utot = 0, gtot = 0;
+    for (int t = 0; t < nt; ++t) {
+      const fr_eles_desc &d = c->eles[t];
+      FR_REQUIRE(d.etype == FR_TET || d.etype == FR_PRI, "only tetrahedra and prisms are supported by fr_setup");
+      FR_REQUIRE(d.order >= 1 && d.nupts > 0 && d.nfpts > 0 && d.nfpts < 65536 && d.neles > 0 &&
+                     d.neles < (1ll << 31) - 64,
+                 "bad element counts");
+      const int p = d.order;
+      const int nu = d.etype == FR_TET ? (p + 1) * (p + 2) * (p + 3) / 6 : (p + 1) * (p + 1) * (p + 2) / 2;
+      const int nf = d.etype == FR_TET ? 2 * (p + 1) * (p + 2) : (p + 1) * (p + 2) + 3 * (p + 1) * (p + 1);
+      FR_REQUIRE(nu == d.nupts && nf == d.nfpts, "nupts / nfpts do not match the element type and order (Table 2)");
+      FR_REQUIRE(d.M0 && d.M132 && d.M3 && d.smats && d.rcpdjac, "operator / metric pointers must be non-NULL");
+      FR_REQUIRE(!ns || (d.M460 && d.M6), "M460 and M6 are required for Navier-Stokes");
+      auto e = std::make_unique<EleData<T>>();
+      tname[t] = d.etype == FR_TET ? "tet" : "pri";
+      EleView<T> &v = e->view;
+      v.nupts = nu;
+      v.nfpts = nf;
+      v.affine = d.affine ? 1 : 0;
+      v.neles = d.neles;
+      v.ld = (d.neles + 31) / 32 * 32;
+      const long long ld = v.ld, ne = d.neles;
+      // metric terms, padded with the identity so padding lanes stay finite
+      const long long npt = v.affine ? 1 : nu;
+      std::vector<T> sm((size_t)9 * npt * ld, T(0)), rj((size_t)npt * ld, T(1));
+      for (int ai = 0; ai < 9; ++ai)
+        for (long long r = 0; r < npt; ++r) {
+          const double *src = d.smats + ((size_t)ai * npt + r) * ne;
+          T *dst = sm.data() + ((size_t)ai * npt + r) * ld;
+          for (long long k = 0; k < ne; ++k) dst[k] = (T)src[k];
+          if (ai % 4 == 0)
+            for (long long k = ne; k < ld; ++k) dst[k] = T(1);
+        }
+      for (long long r = 0; r < npt; ++r)
+        for (long long k = 0; k < ne; ++k) {
+          const double x = d.rcpdjac[(size_t)r * ne + k];
+          FR_REQUIRE(x > 0.0 && std::isfinite(x), "rcpdjac must be positive and finite");
+          rj[(size_t)r * ld + k] = (T)x;
+        }
+      e->smats.upload(sm);
+      e->rcpdjac.upload(rj);
+      v.smats = e->smats.p;
+      v.rcpdjac = e->rcpdjac.p;
+      gemm_plan_build(e->pM0, nf, nu, d.M0);
+      gemm_plan_build(e->pM132, nu, 3 * nu, d.M132);
+      gemm_plan_build(e->pM3, nu, nf, d.M3);
+      if (ns) {
+        gemm_plan_build(e->pM460, 3 * nu, nu, d.M460);
+        gemm_plan_build(e->pM6, 3 * nu, nf, d.M6);
+      }
+      const size_t nstate = (size_t)nu * 5 * ld;
+      e->X.alloc(nstate);
+      e->Y.alloc(nstate);
+      if (stepper == FR_RK4) e->ACC.alloc(nstate);
+      e->grad.alloc(3 * nstate);
+      e->R.alloc(nstate);
+      tt.ubase[t] = utot;
+      tt.gbase[t] = gtot;
+      tt.ld[t] = ld;
+      tt.gcomp[t] = (long long)nf * 5 * ld;
+      utot += (long long)nf * 5 * ld;
+      gtot += 3ll * nf * 5 * ld;
+      el.push_back(std::move(e));
+    }
+    for (int t = nt; t < FR_MAXTYPES; ++t) tt.ubase[t] = tt.gbase[t] = tt.ld[t] = tt.gcomp[t] = 0;
+    uf.alloc(utot);
+    if (ns) {
+      cf.alloc(utot);
+      gf.alloc(gtot);
+    }
+    build_views(c);
+    coef.alloc(8);
+    FR_CUDA_TRY(cudaMallocHost(&coef_host, 8 * sizeof(StageCoef)));
+    FR_CUDA_TRY(cudaDeviceSynchronize());
+  }
+
+  void build_views(const fr_config *c) {
+    const fr_iface_desc &f = *c->ifaces;
+    FR_REQUIRE(f.npairs >= 0, "npairs must be >= 0");
+    FR_REQUIRE(f.npairs == 0 || (f.l_et && f.l_fpt && f.l_ele && f.r_et && f.r_fpt && f.r_ele && f.nl && f.magl && f.magr),
+               "interface arrays must be non-NULL");
+    // every (type, element, flux point) exactly once across pairs and boundaries
+    std::vector<std::vector<uint8_t>> seen(nt);
+    for (int t = 0; t < nt; ++t) seen[t].assign(((size_t)el[t]->view.nfpts * el[t]->view.neles + 7) / 8, 0);
+    auto visit = [&](int t, long long e, int s) {
+      FR_REQUIRE(t >= 0 && t < nt, "flux-point reference: element type out of range");
+      FR_REQUIRE(e >= 0 && e < el[t]->view.neles && s >= 0 && s < el[t]->view.nfpts,
+                 "flux-point reference: element or flux point out of range");
+      const size_t bit = (size_t)s * el[t]->view.neles + e;
+      FR_REQUIRE(!(seen[t][bit >> 3] & (1u << (bit & 7))), "a flux point is referenced more than once");
+      seen[t][bit >> 3] |= (uint8_t)(1u << (bit & 7));
+    };
+    const long long np = f.npairs;
+    for (long long k = 0; k < np; ++k) {
+      visit(f.l_et[k], f.l_ele[k], f.l_fpt[k]);
+      visit(f.r_et[k], f.r_ele[k], f.r_fpt[k]);
+    }
+    FR_REQUIRE(c->nbcs >= 0 && (c->nbcs == 0 || c->bcs), "bcs must be non-NULL when nbcs > 0");
+    for (int b = 0; b < c->nbcs; ++b) {
+      const fr_bc_desc &d = c->bcs[b];
+      FR_REQUIRE(d.type == FR_BC_NOSLIP_ISOTHERMAL_WALL || d.type == FR_BC_CHAR_RIEMANN_INV, "unknown boundary type");
+      FR_REQUIRE(d.nfpts >= 0 && (d.nfpts == 0 || (d.et && d.fpt && d.ele && d.n && d.mag)), "boundary arrays must be non-NULL");
+      for (long long k = 0; k < d.nfpts; ++k) visit(d.et[k], d.ele[k], d.fpt[k]);
+    }
+    for (int t = 0; t < nt; ++t) {
+      const size_t nbits = (size_t)el[t]->view.nfpts * el[t]->view.neles;
+      size_t cnt = 0;
+      for (uint8_t b : seen[t]) cnt += __builtin_popcount(b);
+      FR_REQUIRE(cnt == nbits, "unpaired flux points: every flux point must appear in a pair or a boundary list");
+    }
+    // pairs sorted by (type_L, sigma_L, e_L) so that the L side is read and written fully coalesced
+    std::vector<long long> order(np);
+    std::iota(order.begin(), order.end(), 0ll);
+    auto key_less = [&](long long a, long long b) {
+      if (f.l_et[a] != f.l_et[b]) return f.l_et[a] < f.l_et[b];
+      if (f.l_fpt[a] != f.l_fpt[b]) return f.l_fpt[a] < f.l_fpt[b];
+      return f.l_ele[a] < f.l_ele[b];
+    };
+    if (!std::is_sorted(order.begin(), order.end(), key_less)) std::sort(order.begin(), order.end(), key_less);
+    std::vector<PairRec> pr(np);
+    std::vector<T> hn(3 * (size_t)np), hl(np), hr(np);
+    for (long long i = 0; i < np; ++i) {
+      const long long k = order[i];
+      pr[i] = PairRec{(int)f.l_ele[k], (f.l_et[k] << 16) | f.l_fpt[k], (int)f.r_ele[k], (f.r_et[k] << 16) | f.r_fpt[k]};
+      double nn = 0;
+      for (int d = 0; d < 3; ++d) {
+        hn[(size_t)d * np + i] = (T)f.nl[(size_t)d * np + k];
+        nn += f.nl[(size_t)d * np + k] * f.nl[(size_t)d * np + k];
+      }
+      FR_REQUIRE(std::fabs(nn - 1.0) < 1e-6, "interface normals must be unit vectors");
+      FR_REQUIRE(f.magl[k] > 0 && f.magr[k] > 0, "interface magnitudes must be positive");
+      hl[i] = (T)f.magl[k];
+      hr[i] = (T)f.magr[k];
+    }
+    pairs.upload(pr);
+    nl.upload(hn);
+    magl.upload(hl);
+    magr.upload(hr);
+    iv.npairs = np;
+    iv.pairs = pairs.p;
+    iv.nl = nl.p;
+    iv.magl = magl.p;
+    iv.magr = magr.p;
+    for (int b = 0; b < c->nbcs; ++b) {
+      const fr_bc_desc &d = c->bcs[b];
+      auto bd = std::make_unique<BndData<T>>();
+      const long long n = d.nfpts;
+      std::vector<BndRec> rec(n);
+      std::vector<T> bn(3 * (size_t)n), bm(n);
+      for (long long k = 0; k < n; ++k) {
+        rec[k] = BndRec{(int)d.ele[k], (d.et[k] << 16) | d.fpt[k]};
+        for (int q = 0; q < 3; ++q) bn[(size_t)q * n + k] = (T)d.n[(size_t)q * n + k];
+        bm[k] = (T)d.mag[k];
+      }
+      bd->recs.upload(rec);
+      bd->nrm.upload(bn);
+      bd->mag.upload(bm);
+      bd->view.n = n;
+      bd->view.type = (int)d.type;
+      bd->view.recs = bd->recs.p;
+      bd->view.nrm = bd->nrm.p;
+      bd->view.mag = bd->mag.p;
+      for (int q = 0; q < 8; ++q) bd->view.par[q] = (T)d.params[q];
+      bnd.push_back(std::move(bd));
+    }
+  }
+
+  // ------------------------------------------------------------------ one RHS evaluation (S1..S9/S10)
+  // u[t]: stage input; sa[t]: what the last kernel of type t writes.  Returns kernels launched.
+  int run_rhs(const T *const *u, const StageArgs<T> *sa, Timeline *tl) {
+    int nk = 0;
+    cudaStream_t s = stream;
+    const bool ns = ph.ns;
+    const double w = sizeof(T);
+    auto mark = [&](int c, int t, const char *step, double words, double fl) {
+      if (!tl) return;
+      std::string nm = t >= 0 ? std::string(tname[t]) + ":" + step : std::string(step);
+      tl->mark(c, nm, words * w, fl);
+    };
+    if (tl) tl->mark(-1);
+    double nbnd = 0;
+    for (auto &b : bnd) nbnd += (double)b->view.n;
+    const double npr = (double)iv.npairs;
+    for (int t = 0; t < nt; ++t) {   // S1: U_f = M0 U
+      EleData<T> &e = *el[t];
+      const double n = (double)e.view.neles, nu = e.view.nupts, nf = e.view.nfpts;
+      nk += gemm_run(e.pM0, 5 * e.view.ld, T(1), u[t], 5 * e.view.ld, 0, T(0), uf.p + tt.ubase[t], 5 * e.view.ld, 0, 1, s);
+      mark(CAT_GEMM, t, "S1_M0", (nu + nf) * 5 * n, 2 * nf * nu * 5 * n);
+    }
+    if (ns) {
+      nk += launch_con_u(iv, tt, uf.p, cf.p, ph.beta, s);   // S2
+      for (auto &b : bnd) nk += launch_bc_con_u(b->view, tt, uf.p, cf.p, ph.gamma, s);
+      mark(CAT_IFACE, -1, "S2_con_u", npr * (20 + 16 / w) + nbnd * (10 + 3 + 8 / w), npr * 15 + nbnd * 60);
+      for (int t = 0; t < nt; ++t) {
+        EleData<T> &e = *el[t];
+        const long long n5 = 5 * e.view.ld;
+        const double n = (double)e.view.neles, nu = e.view.nupts, nf = e.view.nfpts;
+        const double nmet = e.view.affine ? 1 : nu;
+        // S3: G~ = M460 U + M6 C
+        nk += gemm_run(e.pM460, n5, T(1), u[t], n5, 0, T(0), e.grad.p, n5, 0, 1, s);
+        mark(CAT_GEMM, t, "S3a_M460", (nu + 3 * nu) * 5 * n, 2 * 3 * nu * nu * 5 * n);
+        nk += gemm_run(e.pM6, n5, T(1), cf.p + tt.ubase[t], n5, 0, T(1), e.grad.p, n5, 0, 1, s);
+        mark(CAT_GEMM, t, "S3b_M6", (nf + 6 * nu) * 5 * n, 2 * 3 * nu * nf * 5 * n);
+        nk += launch_gradcoru(e.view, e.grad.p, s);   // S4
+        mark(CAT_PW, t, "S4_gradcoru", (30 * nu + 10 * nmet) * n, 15 * 6 * nu * n);
+        // S5: G_f,i = M0 G_i, i = 0..2 (batched)
+        nk += gemm_run(e.pM0, n5, T(1), e.grad.p, n5, (long long)e.view.nupts * n5, T(0), gf.p + tt.gbase[t], n5,
+                       tt.gcomp[t], 3, s);
+        mark(CAT_GEMM, t, "S5_M0grad", (nu + nf) * 15 * n, 2 * nf * nu * 15 * n);
+      }
+    }
+    nk += launch_comm_flux(iv, tt, uf.p, gf.p, ph, s);   // S7 (D overwrites U_f)
+    for (auto &b : bnd) nk += launch_bc_comm_flux(b->view, tt, uf.p, gf.p, ph, s);
+    {
+      const double sides = ns ? ((ph.beta == T(0.5) || ph.beta == T(-0.5)) ? 1 : 2) : 0;
+      mark(CAT_IFACE, -1, "S7_comm_flux", npr * (20 + 15 * sides + 5 + 16 / w) + nbnd * (10 + (ns ? 15 : 0) + 4 + 8 / w),
+           npr * (ns ? 420 : 160) + nbnd * (ns ? 420 : 200));
+    }
+    for (int t = 0; t < nt; ++t) {
+      EleData<T> &e = *el[t];
+      const long long n5 = 5 * e.view.ld;
+      const double n = (double)e.view.neles, nu = e.view.nupts, nf = e.view.nfpts;
+      const double nmet = e.view.affine ? 1 : nu;
+      nk += launch_tdisf(e.view, u[t], e.grad.p, ph, s);   // S6
+      mark(CAT_PW, t, "S6_tdisf", ((ns ? 35 : 20) * nu + 9 * nmet) * n, (ns ? 210 : 110) * nu * n);
+      // S8: R = M132 F~ + M3 D
+      nk += gemm_run(e.pM132, n5, T(1), e.grad.p, n5, 0, T(0), e.R.p, n5, 0, 1, s);
+      mark(CAT_GEMM, t, "S8a_M132", (3 * nu + nu) * 5 * n, 2 * nu * 3 * nu * 5 * n);
+      nk += gemm_run(e.pM3, n5, T(1), uf.p + tt.ubase[t], n5, 0, T(1), e.R.p, n5, 0, 1, s);
+      mark(CAT_GEMM, t, "S8b_M3", (nf + 2 * nu) * 5 * n, 2 * nu * nf * 5 * n);
+      nk += launch_negdivconf(e.view, e.R.p, sa[t], s);   // S9 / S10
+      const double extra = sa[t].coef ? (sa[t].out2 ? 20 : 10) : 5;
+      mark(CAT_PW, t, sa[t].coef ? "S9_S10_negdiv_rk" : "S9_negdivconf", ((5 + extra) * nu + nmet) * n, 5 * nu * n * (sa[t].coef ? 5 : 1));
+    }
+    return nk;
+  }
+
+  void state_layout(int et, int64_t *ld, int64_t *nbytes) const override {
+    FR_REQUIRE(et >= 0 && et < nt, "element type index out of range");
+    if (ld) *ld = el[et]->view.ld;
+    if (nbytes) *nbytes = (int64_t)el[et]->view.nupts * 5 * el[et]->view.ld * (int64_t)sizeof(T);
+  }
+
+  void rhs(const void *const *u, void *const *dudt) override {
+    FR_REQUIRE(u && dudt, "u_dev and dudt_dev must be non-NULL");
+    std::vector<const T *> up(nt);
+    std::vector<StageArgs<T>> sa(nt);
+    for (int t = 0; t < nt; ++t) {
+      FR_REQUIRE(u[t] && dudt[t] && u[t] != dudt[t], "state pointers must be non-NULL and must not alias");
+      FR_REQUIRE(((uintptr_t)u[t] % 16) == 0 && ((uintptr_t)dudt[t] % 16) == 0, "state pointers must be 16-byte aligned");
+      up[t] = (const T *)u[t];
+      sa[t] = StageArgs<T>{nullptr, nullptr, nullptr, (T *)dudt[t], nullptr};
+    }
+    launches += run_rhs(up.data(), sa.data(), nullptr);
+  }
+
+  void set_state(const double *const *u) override {
+    FR_REQUIRE(u, "u_host must be non-NULL");
+    for (int t = 0; t < nt; ++t) {
+      FR_REQUIRE(u[t], "u_host[t] must be non-NULL");
+      const EleView<T> &v = el[t]->view;
+      std::vector<T> h((size_t)v.nupts * 5 * v.ld, T(0));
+      for (long long r = 0; r < (long long)v.nupts * 5; ++r)
+        for (long long k = 0; k < v.neles; ++k) h[(size_t)r * v.ld + k] = (T)u[t][(size_t)r * v.neles + k];
+      FR_CUDA_TRY(cudaStreamSynchronize(stream));
+      FR_CUDA_TRY(cudaMemcpy(el[t]->X.p, h.data(), h.size() * sizeof(T), cudaMemcpyHostToDevice));
+    }
+  }
+
+  void get_state(double *const *u) override {
+    FR_REQUIRE(u, "u_host must be non-NULL");
+    FR_CUDA_TRY(cudaStreamSynchronize(stream));
+    for (int t = 0; t < nt; ++t) {
+      FR_REQUIRE(u[t], "u_host[t] must be non-NULL");
+      const EleView<T> &v = el[t]->view;
+      std::vector<T> h((size_t)v.nupts * 5 * v.ld);
+      FR_CUDA_TRY(cudaMemcpy(h.data(), el[t]->X.p, h.size() * sizeof(T), cudaMemcpyDeviceToHost));
+      for (long long r = 0; r < (long long)v.nupts * 5; ++r)
+        for (long long k = 0; k < v.neles; ++k) u[t][(size_t)r * v.neles + k] = (double)h[(size_t)r * v.ld + k];
+    }
+  }
+
+  // ------------------------------------------------------------------ Runge-Kutta (S10 fused into S9)
+  int nstages() const { return stepper == FR_RK4 ? 4 : 5; }
+
+  void fill_coefs(double dt) {
+    if (stepper == FR_RK4) {
+      const StageCoef c[4] = {{dt / 6, dt / 2}, {dt / 3, dt / 2}, {dt / 3, dt}, {dt / 6, 0.0}};
+      for (int i = 0; i < 4; ++i) coef_host[i] = c[i];
+    } else {
+      // RK4(3)5[2R+]C (reading R12): X += dt b_i K ; Y = X_old + dt a_i K
+      static const double a[5] = {970286171893.0 / 4311952581923.0, 6584761158862.0 / 12103376702013.0,
+                                  2251764453980.0 / 15575788980749.0, 26877169314380.0 / 34165994151039.0, 0.0};
+      static const double b[5] = {1153189308089.0 / 22510343858157.0, 1772645290293.0 / 4653164025191.0,
+                                  -1672844663538.0 / 4480602732383.0, 2114624349019.0 / 3568978502595.0,
+                                  5198255086312.0 / 14908931495163.0};
+      for (int i = 0; i < 5; ++i) coef_host[i] = StageCoef{dt * b[i], dt * a[i]};
+    }
+  }
+
+  int enqueue_step() {
+    int nk = 0;
+    const int S = nstages();
+    std::vector<const T *> up(nt);
+    std::vector<StageArgs<T>> sa(nt);
+    for (int i = 0; i < S; ++i) {
+      for (int t = 0; t < nt; ++t) {
+        EleData<T> &e = *el[t];
+        up[t] = i == 0 ? e.X.p : e.Y.p;
+        const StageCoef *c = coef.p + i;
+        if (stepper == FR_RK4) {
+          if (i == 0) sa[t] = StageArgs<T>{c, e.X.p, e.X.p, e.ACC.p, e.Y.p};
+          else if (i < 3) sa[t] = StageArgs<T>{c, e.ACC.p, e.X.p, e.ACC.p, e.Y.p};
+          else sa[t] = StageArgs<T>{c, e.ACC.p, nullptr, e.X.p, nullptr};
+        } else {
+          sa[t] = StageArgs<T>{c, e.X.p, e.X.p, e.X.p, i < S - 1 ? e.Y.p : nullptr};
+        }
+      }
+      nk += run_rhs(up.data(), sa.data(), nullptr);
+    }
+    return nk;
+  }
+
+  void rk_step(double dt, long long nsteps) override {
+    FR_REQUIRE(std::isfinite(dt), "dt must be finite");
+    if (nsteps <= 0) return;
+    if (!(dt == coef_dt)) {
+      FR_CUDA_TRY(cudaStreamSynchronize(stream));   // pinned staging buffer may still be in use
+      fill_coefs(dt);
+      FR_CUDA_TRY(cudaMemcpyAsync(coef.p, coef_host, 8 * sizeof(StageCoef), cudaMemcpyHostToDevice, stream));
+      coef_dt = dt;
+    }
+    if (!graph) {
+      // warm the function attributes outside capture, then capture one step
+      cudaGraph_t g = nullptr;
+      FR_CUDA_TRY(cudaStreamBeginCapture(stream, cudaStreamCaptureModeThreadLocal));
+      int nk = 0;
+      try {
+        nk = enqueue_step();
+      } catch (...) {
+        cudaStreamEndCapture(stream, &g);
+        if (g) cudaGraphDestroy(g);
+        throw;
+      }
+      FR_CUDA_TRY(cudaStreamEndCapture(stream, &g));
+      cudaError_t e = cudaGraphInstantiate(&graph, g, 0);
+      cudaGraphDestroy(g);
+      FR_CUDA_TRY(e);
+      graph_kernels = nk;
+    }
+    for (long long i = 0; i < nsteps; ++i) {
+      FR_CUDA_TRY(cudaGraphLaunch(graph, stream));
+      launches += graph_kernels;
+    }
+  }
+
+  void sync() override {
+    FR_CUDA_TRY(cudaStreamSynchronize(stream));
+    FR_CUDA_TRY(cudaGetLastError());
+  }
+
+  // Events between all kernels of `reps` RHS evaluations of the internal state; per-category and per-kernel means.
+  void profile(int reps, double ms[4], fr_kernel_stat *out, int cap, int *nout) override {
+    FR_REQUIRE(reps > 0, "reps must be positive");
+    std::vector<const T *> up(nt);
+    std::vector<StageArgs<T>> sa(nt);
+    for (int t = 0; t < nt; ++t) {
+      up[t] = el[t]->X.p;
+      sa[t] = StageArgs<T>{nullptr, nullptr, nullptr, el[t]->Y.p, nullptr};
+    }
+    launches += run_rhs(up.data(), sa.data(), nullptr);   // warm-up
+    double acc[4] = {0, 0, 0, 0};
+    std::vector<fr_kernel_stat> ks;
+    for (int r = 0; r < reps; ++r) {
+      Timeline tl;
+      tl.s = stream;
+      launches += run_rhs(up.data(), sa.data(), &tl);
+      FR_CUDA_TRY(cudaStreamSynchronize(stream));
+      if (ks.empty()) {
+        ks.resize(tl.ev.size() - 1);
+        for (size_t i = 1; i < tl.ev.size(); ++i) {
+          fr_kernel_stat &k = ks[i - 1];
+          memset(&k, 0, sizeof(k));
+          strncpy(k.name, tl.name[i].c_str(), sizeof(k.name) - 1);
+          k.alg_bytes = tl.bytes[i];
+          k.flops = tl.flops[i];
+          k.category = tl.cat[i];
+        }
+      }
+      for (size_t i = 1; i < tl.ev.size(); ++i) {
+        float m = 0;
+        cudaEventElapsedTime(&m, tl.ev[i - 1], tl.ev[i]);
+        acc[tl.cat[i]] += m;
+        acc[3] += m;
+        ks[i - 1].ms += m / reps;
+      }
+      for (auto e : tl.ev) cudaEventDestroy(e);
+    }
+    if (ms)
+      for (int i = 0; i < 4; ++i) ms[i] = acc[i] / reps;
+    if (nout) *nout = (int)ks.size();
+    if (out)
+      for (int i = 0; i < (int)ks.size() && i < cap; ++i) out[i] = ks[i];
+  }
+
+  // H2D of the state (device layout, context precision), one step, D2H -- the end-to-end user call.
+  void rk_step_host(double dt, void *const *u_host) override {
+    FR_REQUIRE(u_host, "u_host must be non-NULL");
+    for (int t = 0; t < nt; ++t) {
+      FR_REQUIRE(u_host[t], "u_host[t] must be non-NULL");
+      const size_t nb = (size_t)el[t]->view.nupts * 5 * el[t]->view.ld * sizeof(T);
+      FR_CUDA_TRY(cudaMemcpyAsync(el[t]->X.p, u_host[t], nb, cudaMemcpyHostToDevice, stream));
+    }
+    rk_step(dt, 1);
+    for (int t = 0; t < nt; ++t) {
+      const size_t nb = (size_t)el[t]->view.nupts * 5 * el[t]->view.ld * sizeof(T);
+      FR_CUDA_TRY(cudaMemcpyAsync(u_host[t], el[t]->X.p, nb, cudaMemcpyDeviceToHost, stream));
+    }
+    FR_CUDA_TRY(cudaStreamSynchronize(stream));
+  }
+};
+
+}  // namespace frb
+
+// ---------------------------------------------------------------------------- C ABI
+struct fr_ctx {
+  frb::CtxBase *impl;
+};
+struct fr_gemm_plan {
+  fr_prec prec;
+  frb::GemmPlan<double> pd;
+  frb::GemmPlan<float> pf;
+};
+
+namespace {
+template <typename F>
+fr_status guard(std::string *err, F &&f) {
+  try {
+    f();
+    return FR_OK;
+  } catch (const frb::Error &e) {
+    if (err) *err = e.msg;
+    frb::g_error = e.msg;
+    return e.st;
+  } catch (const std::bad_alloc &) {
+    if (err) *err = "host allocation failed";
+    frb::g_error = "host allocation failed";
+    return FR_ENOMEM;
+  } catch (...) {
+    if (err) *err = "unknown error";
+    frb::g_error = "unknown error";
+    return FR_ESTATE;
+  }
+}
+void require_device() {
+  int n = 0;
+  cudaError_t e = cudaGetDeviceCount(&n);
+  if (e != cudaSuccess || n <= 0)
+    throw frb::Error{FR_ECUDA, std::string("no usable CUDA device: ") + (e != cudaSuccess ? cudaGetErrorString(e) : "count = 0")};
+}
+}  // namespace
+
+extern "C" {
+
+fr_status fr_setup(const fr_config *cfg, fr_ctx **out) {
+  if (out) *out = nullptr;
+  return guard(nullptr, [&] {
+    FR_REQUIRE(cfg && out, "cfg and out must be non-NULL");
+    FR_REQUIRE(cfg->prec == FR_F32 || cfg->prec == FR_F64, "prec must be FR_F32 or FR_F64");
+    FR_REQUIRE(cfg->system == FR_EULER || cfg->system == FR_NAVIER_STOKES, "unknown system");
+    FR_REQUIRE(cfg->stepper == FR_RK4 || cfg->stepper == FR_RK45_2R, "unknown stepper");
+    FR_REQUIRE(cfg->mode == FR_MODE_FUSED || cfg->mode == FR_MODE_UNFUSED, "unknown mode");
+    require_device();
+    std::unique_ptr<frb::CtxBase> impl;
+    if (cfg->prec == FR_F64) {
+      auto c = std::make_unique<frb::Ctx<double>>();
+      c->setup(cfg);
+      impl = std::move(c);
+    } else {
+      auto c = std::make_unique<frb::Ctx<float>>();
+      c->setup(cfg);
+      impl = std::move(c);
+    }
+    *out = new fr_ctx{impl.release()};
+  });
+}
+
+#define FR_CTX_CALL(ctx, body)                            \
+  if (!(ctx) || !(ctx)->impl) return FR_EINVAL;           \
+  return guard(&(ctx)->impl->err, [&] { body; })
+
+fr_status fr_state_layout(const fr_ctx *ctx, int32_t et, int64_t *ld, int64_t *nbytes) {
+  FR_CTX_CALL(ctx, ctx->impl->state_layout(et, ld, nbytes));
+}
+fr_status fr_rhs(fr_ctx *ctx, const void *const *u_dev, void *const *dudt_dev) { FR_CTX_CALL(ctx, ctx->impl->rhs(u_dev, dudt_dev)); }
+fr_status fr_set_state(fr_ctx *ctx, const double *const *u_host) { FR_CTX_CALL(ctx, ctx->impl->set_state(u_host)); }
+fr_status fr_get_state(fr_ctx *ctx, double *const *u_host) { FR_CTX_CALL(ctx, ctx->impl->get_state(u_host)); }
+fr_status fr_rk_step(fr_ctx *ctx, double dt) { FR_CTX_CALL(ctx, ctx->impl->rk_step(dt, 1)); }
+fr_status fr_rk_run(fr_ctx *ctx, double dt, int64_t nsteps) { FR_CTX_CALL(ctx, ctx->impl->rk_step(dt, nsteps)); }
+fr_status fr_sync(fr_ctx *ctx) { FR_CTX_CALL(ctx, ctx->impl->sync()); }
+fr_status fr_profile_rhs(fr_ctx *ctx, int32_t reps, double ms[4]) {
+  FR_CTX_CALL(ctx, {
+    FR_REQUIRE(ms, "ms must be non-NULL");
+    ctx->impl->profile(reps, ms, nullptr, 0, nullptr);
+  });
+}
+fr_status fr_profile_kernels(fr_ctx *ctx, int32_t reps, fr_kernel_stat *out, int32_t cap, int32_t *n) {
+  FR_CTX_CALL(ctx, {
+    FR_REQUIRE(n && (out || cap == 0), "n must be non-NULL (and out non-NULL when cap > 0)");
+    int nn = 0;
+    ctx->impl->profile(reps, nullptr, out, cap, &nn);
+    *n = nn;
+  });
+}
+fr_status fr_rk_step_host(fr_ctx *ctx, double dt, void *const *u_host) { FR_CTX_CALL(ctx, ctx->impl->rk_step_host(dt, u_host)); }
+int64_t fr_launch_count(const fr_ctx *ctx) { return ctx && ctx->impl ? ctx->impl->launches : 0; }
+const char *fr_last_error(const fr_ctx *ctx) { return ctx && ctx->impl ? ctx->impl->err.c_str() : "invalid context"; }
+const char *fr_global_error(void) { return frb::g_error.c_str(); }
+void fr_destroy(fr_ctx *ctx) {
+  if (!ctx) return;
+  delete ctx->impl;
+  delete ctx;
+}
+
+fr_status fr_gemm_plan_create(int32_t M, int32_t K, const double *A_host, fr_prec prec, fr_gemm_plan **out) {
+  if (out) *out = nullptr;
+  return guard(nullptr, [&] {
+    FR_REQUIRE(out, "out must be non-NULL");
+    FR_REQUIRE(prec == FR_F32 || prec == FR_F64, "prec must be FR_F32 or FR_F64");
+    require_device();
+    auto p = std::make_unique<fr_gemm_plan>();
+    p->prec = prec;
+    if (prec == FR_F64) frb::gemm_plan_build(p->pd, M, K, A_host);
+    else frb::gemm_plan_build(p->pf, M, K, A_host);
+    *out = p.release();
+  });
+}
+fr_status fr_gemm_plan_run(fr_gemm_plan *plan, int64_t N, double c1, const void *B_dev, int64_t ldb, double c2, void *C_dev,
+                           int64_t ldc, void *cuda_stream) {
+  return guard(nullptr, [&] {
+    FR_REQUIRE(plan && B_dev && C_dev, "plan, B and C must be non-NULL");
+    FR_REQUIRE(N >= 0, "N must be >= 0");
+    cudaStream_t s = (cudaStream_t)cuda_stream;
+    if (plan->prec == FR_F64)
+      frb::gemm_run(plan->pd, N, c1, (const double *)B_dev, ldb, 0, c2, (double *)C_dev, ldc, 0, 1, s);
+    else
+      frb::gemm_run(plan->pf, N, (float)c1, (const float *)B_dev, ldb, 0, (float)c2, (float *)C_dev, ldc, 0, 1, s);
+  });
+}
+void fr_gemm_plan_destroy(fr_gemm_plan *plan) {
+  if (!plan) return;
+  frb::gemm_plan_free(plan->pd);
+  frb::gemm_plan_free(plan->pf);
+  delete plan;
+}
+fr_status fr_gemm(int32_t M, int32_t K, int64_t N, double c1, const double *A_host, const void *B_dev, int64_t ldb, double c2,
+                  void *C_dev, int64_t ldc, fr_prec prec, void *cuda_stream) {
+  fr_gemm_plan *p = nullptr;
+  fr_status st = fr_gemm_plan_create(M, K, A_host, prec, &p);
+  if (st != FR_OK) return st;
+  st = fr_gemm_plan_run(p, N, c1, B_dev, ldb, c2, C_dev, ldc, cuda_stream);
+  if (st == FR_OK) {
+    // the operator buffer is freed below: wait for the product that reads it
+    cudaError_t e = cudaStreamSynchronize((cudaStream_t)cuda_stream);
+    if (e != cudaSuccess) {
+      frb::g_error = std::string("fr_gemm: ") + cudaGetErrorString(e);
+      st = FR_ECUDA;
+    }
+  }
+  fr_gemm_plan_destroy(p);
+  return st;
+}
+
+}  // extern "C"

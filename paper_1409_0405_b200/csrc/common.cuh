@@ -1,0 +1,84 @@
+// Shared declarations of the frb200 library (host + device).  sm_100a only.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <stdio.h>
+
+#include <string>
+#include <vector>
+
+#include "../../include/frb200.h"
+
+#define FR_NVAR 5
+#define FR_MAXTYPES 4
+
+namespace frb {
+
+struct Error {
+  fr_status st;
+  std::string msg;
+};
+
+#define FR_CUDA_TRY(expr)                                                                       \
+  do {                                                                                          \
+    cudaError_t _e = (expr);                                                                    \
+    if (_e != cudaSuccess) {                                                                    \
+      throw frb::Error{FR_ECUDA, std::string(#expr) + ": " + cudaGetErrorString(_e)};           \
+    }                                                                                           \
+  } while (0)
+
+#define FR_REQUIRE(cond, msg_)                                                                  \
+  do {                                                                                          \
+    if (!(cond)) throw frb::Error{FR_EINVAL, std::string(msg_)};                                \
+  } while (0)
+
+// Per-type addressing table of the flat flux-point arrays, passed by value to the interface kernels.
+// U_f / C / D of type t: [nfpts][5][ld] at ubase[t];  G_f: [3][nfpts][5][ld] at gbase[t].
+struct TypeTab {
+  long long ubase[FR_MAXTYPES];
+  long long gbase[FR_MAXTYPES];
+  long long ld[FR_MAXTYPES];
+  long long gcomp[FR_MAXTYPES];   // nfpts*5*ld: stride between gradient components in G_f
+};
+
+// One side of a flux-point pair: element index and (type << 16 | sigma).
+struct PairRec {
+  int le, lts, re, rts;
+};
+struct BndRec {
+  int e, ts;
+};
+
+template <typename T>
+struct PhysParams {
+  T gamma, mu, prandtl, beta, tau;
+  int ns;
+};
+
+// Stage-update coefficients live in device memory so a captured graph needs no re-capture when dt changes.
+struct StageCoef {
+  double c1, c2;
+};
+
+template <typename T>
+struct GemmPlan {
+  int M = 0, K = 0;
+  int TY = 0, MT = 0, nrb = 0;   // thread rows, rows per thread, row blocks (M <= nrb*TY*MT)
+  int resident = 0;              // whole operator slab kept in shared memory
+  int ctas_per_sm = 1;
+  size_t smem = 0;
+  T *At = nullptr;               // device, [nrb][K][TY*MT], zero padded, transposed operator
+};
+
+template <typename T>
+void gemm_plan_build(GemmPlan<T> &p, int M, int K, const double *A_host);
+template <typename T>
+void gemm_plan_free(GemmPlan<T> &p);
+// C[b] <- c1 * A * B[b] + c2 * C[b], b < nbatch; returns the number of kernels launched
+template <typename T>
+int gemm_run(const GemmPlan<T> &p, long long N, T c1, const T *B, long long ldb, long long bstrideB, T c2, T *C,
+             long long ldc, long long bstrideC, int nbatch, cudaStream_t s);
+
+int device_sm_count();
+
+}  // namespace frb

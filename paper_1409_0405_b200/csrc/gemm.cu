@@ -1,0 +1,340 @@
+// Operator product C <- c1*A*B + c2*C (eq. 1): A = small constant operator (M x K),
+// B (K x N) and C (M x N) wide row-major state matrices -- the block-by-panel (GEBP) case of PAPER.md:39.
+//
+// B200 design (not the paper's: it defers to cuBLAS): every column of B is independent, so a
+// persistent CTA owns column panels (the decomposition the paper's OpenMP backend found best).
+//   * the operator slab (transposed, zero padded, [K][TY*MT]) stays resident in shared memory for the whole
+//     kernel when it fits, so L2->SM traffic is the B panel only;
+//   * B panels stream global->shared through a 4-stage cp.async ring that runs across panel boundaries
+//     (16-byte, fully coalesced row segments; K and N tails zero-filled by the copy itself);
+//   * each thread keeps an MT x CT register tile (CT = one 16-byte vector of columns), A is read as warp-wide
+//     broadcast vectors, B as conflict-free vectors; FP64 uses DFMA, FP32 FFMA (no TF32: the 2e-5 parity bound
+//     and reading R15 exclude it; tcgen05 has no FP64 kind);
+//   * C is written once with 16-byte coalesced stores; c2 != 0 reads it once.
+#include <algorithm>
+
+#include "common.cuh"
+
+namespace frb {
+
+namespace {
+
+constexpr int KC = 16;      // K rows per pipeline stage
+constexpr int NSTAGE = 4;   // cp.async ring depth
+
+template <typename T>
+struct VecT;
+template <>
+struct VecT<double> {
+  using type = double2;
+  static constexpr int CT = 2;
+};
+template <>
+struct VecT<float> {
+  using type = float4;
+  static constexpr int CT = 4;
+};
+
+template <typename T>
+struct GemmArgs {
+  int M, K, nchunks, nrb, nbatch;
+  long long N, ntn;            // columns, column tiles per batch
+  const T *At;                 // [nrb][Kpad][MTILE]
+  const T *B;
+  T *C;
+  long long ldb, ldc, bsB, bsC;
+  T c1, c2;
+};
+
+__device__ __forceinline__ void cp_async16(void *smem, const void *gmem, int src_bytes) {
+  unsigned s = (unsigned)__cvta_generic_to_shared(smem);
+  asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;\n" ::"r"(s), "l"(gmem), "r"(src_bytes));
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;\n" ::); }
+template <int N>
+__device__ __forceinline__ void cp_async_wait() {
+  asm volatile("cp.async.wait_group %0;\n" ::"n"(N));
+}
+
+template <typename T, int MT, int TY, bool RESIDENT>
+__global__ void __launch_bounds__(32 * TY) k_gemm(const __grid_constant__ GemmArgs<T> a) {
+  using V = typename VecT<T>::type;
+  constexpr int CT = VecT<T>::CT;
+  constexpr int NT = 32 * CT;
+  constexpr int MTILE = TY * MT;
+  constexpr int NTHREADS = 32 * TY;
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  T *Bs = reinterpret_cast<T *>(smem_raw);                         // [NSTAGE][KC][NT]
+  T *As = Bs + NSTAGE * KC * NT;                                   // resident: [Kpad][MTILE]; else [NSTAGE][KC][MTILE]
+
+  const int tx = threadIdx.x, ty = threadIdx.y;
+  const int tid = ty * 32 + tx;
+  const int rb = blockIdx.x % a.nrb;
+  const long long lane = blockIdx.x / a.nrb;
+  const long long stride = gridDim.x / a.nrb;
+  const long long ntiles = a.ntn * a.nbatch;
+  const long long mytiles = lane < ntiles ? (ntiles - lane + stride - 1) / stride : 0;
+  const long long total = mytiles * a.nchunks;
+  const int Kpad = a.nchunks * KC;
+  const T *At = a.At + (long long)rb * Kpad * MTILE;
+
+  if (RESIDENT) {
+    const int npieces = Kpad * MTILE * (int)sizeof(T) / 16;
+    for (int p = tid; p < npieces; p += NTHREADS)
+      cp_async16(reinterpret_cast<char *>(As) + 16 * p, reinterpret_cast<const char *>(At) + 16 * p, 16);
+  }
+
+  auto issue = [&](long long q) {
+    const long long tile = lane + (q / a.nchunks) * stride;
+    const int c = (int)(q % a.nchunks);
+    const int st = (int)(q % NSTAGE);
+    const long long batch = tile / a.ntn;
+    const long long col0 = (tile % a.ntn) * NT;
+    const T *Bb = a.B + batch * a.bsB;
+    T *bs = Bs + st * KC * NT;
+#pragma unroll
+    for (int p = tid; p < KC * 32; p += NTHREADS) {
+      const int row = p >> 5, pc = p & 31;
+      const int k = c * KC + row;
+      const long long col = col0 + pc * CT;
+      long long rem = (a.N - col) * (long long)sizeof(T);
+      int nb = (k < a.K) ? (rem >= 16 ? 16 : (rem > 0 ? (int)rem : 0)) : 0;
+      const T *src = nb > 0 ? Bb + (long long)k * a.ldb + col : a.B;
+      cp_async16(bs + row * NT + pc * CT, src, nb);
+    }
+    if (!RESIDENT) {
+      T *as = As + st * KC * MTILE;
+      constexpr int PPR = MTILE * (int)sizeof(T) / 16;             // 16-byte pieces per row
+      for (int p = tid; p < KC * PPR; p += NTHREADS) {
+        const int row = p / PPR, pc = p % PPR;
+        cp_async16(reinterpret_cast<char *>(as + row * MTILE) + 16 * pc,
+                   reinterpret_cast<const char *>(At + (long long)(c * KC + row) * MTILE) + 16 * pc, 16);
+      }
+    }
+  };
+
+  for (int q = 0; q < NSTAGE - 1; ++q) {
+    if (q < total) issue(q);
+    cp_async_commit();
+  }
+
+  T acc[MT][CT];
+#pragma unroll
+  for (int i = 0; i < MT; ++i)
+#pragma unroll
+    for (int j = 0; j < CT; ++j) acc[i][j] = T(0);
+
+  for (long long q = 0; q < total; ++q) {
+    cp_async_wait<NSTAGE - 2>();
+    __syncthreads();
+    if (q + NSTAGE - 1 < total) issue(q + NSTAGE - 1);
+    cp_async_commit();
+
+    const int c = (int)(q % a.nchunks);
+    const int st = (int)(q % NSTAGE);
+    const T *bs = Bs + st * KC * NT + tx * CT;
+    const T *as = (RESIDENT ? As + c * KC * MTILE : As + st * KC * MTILE) + ty * MT;
+    const int kend = min(KC, a.K - c * KC);
+#pragma unroll 4
+    for (int kk = 0; kk < kend; ++kk) {
+      T bv[CT];
+      *reinterpret_cast<V *>(bv) = *reinterpret_cast<const V *>(bs + kk * NT);
+      T av[MT];
+      // warp-wide broadcast reads of the operator column; vector width limited by the alignment of ty*MT
+      constexpr int AV = (MT % CT == 0) ? CT : 2;
+      static_assert(MT % 2 == 0, "MT must be even");
+#pragma unroll
+      for (int i = 0; i < MT; i += AV) {
+        if (AV == CT) {
+          *reinterpret_cast<V *>(av + i) = *reinterpret_cast<const V *>(as + kk * MTILE + i);
+        } else {
+          *reinterpret_cast<float2 *>(av + i) = *reinterpret_cast<const float2 *>(as + kk * MTILE + i);
+        }
+      }
+#pragma unroll
+      for (int i = 0; i < MT; ++i)
+#pragma unroll
+        for (int j = 0; j < CT; ++j) acc[i][j] = fma(av[i], bv[j], acc[i][j]);
+    }
+
+    if (c == a.nchunks - 1) {
+      const long long tile = lane + (q / a.nchunks) * stride;
+      const long long batch = tile / a.ntn;
+      const long long col = (tile % a.ntn) * NT + tx * CT;
+      T *Cb = a.C + batch * a.bsC;
+      const bool full = col + CT <= a.N;
+#pragma unroll
+      for (int i = 0; i < MT; ++i) {
+        const int m = rb * MTILE + ty * MT + i;
+        if (m < a.M) {
+          T *cp = Cb + (long long)m * a.ldc + col;
+          if (full) {
+            T out[CT];
+            if (a.c2 != T(0)) {
+              T old[CT];
+              *reinterpret_cast<V *>(old) = *reinterpret_cast<const V *>(cp);
+#pragma unroll
+              for (int j = 0; j < CT; ++j) out[j] = fma(a.c1, acc[i][j], a.c2 * old[j]);
+            } else {
+#pragma unroll
+              for (int j = 0; j < CT; ++j) out[j] = a.c1 * acc[i][j];
+            }
+            *reinterpret_cast<V *>(cp) = *reinterpret_cast<V *>(out);
+          } else {
+#pragma unroll
+            for (int j = 0; j < CT; ++j)
+              if (col + j < a.N) cp[j] = (a.c2 != T(0)) ? fma(a.c1, acc[i][j], a.c2 * cp[j]) : a.c1 * acc[i][j];
+          }
+        }
+#pragma unroll
+        for (int j = 0; j < CT; ++j) acc[i][j] = T(0);
+      }
+    }
+  }
+  cp_async_wait<0>();
+}
+
+// Grid: persistent CTAs, (resident CTAs per SM from the occupancy calculator) x (SM count), a multiple of the
+// number of row blocks, never more than there are panels.
+template <typename K, typename T>
+void launch_kernel(K k, const GemmPlan<T> &p, const GemmArgs<T> &a, int nthreads, cudaStream_t s) {
+  FR_CUDA_TRY(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p.smem));
+  int occ = 1;
+  FR_CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k, nthreads, p.smem));
+  occ = std::max(1, std::min(occ, 4));
+  const long long ntiles = a.ntn * a.nbatch;
+  long long lanes = std::max(1, device_sm_count() * occ / p.nrb);
+  lanes = std::min(lanes, ntiles);
+  k<<<(unsigned)(lanes * p.nrb), dim3(32, nthreads / 32), p.smem, s>>>(a);
+  FR_CUDA_TRY(cudaGetLastError());
+}
+
+template <typename T, int MT, int TY>
+void launch_variant(const GemmPlan<T> &p, const GemmArgs<T> &a, int, cudaStream_t s) {
+  if (p.resident) launch_kernel(k_gemm<T, MT, TY, true>, p, a, 32 * TY, s);
+  else launch_kernel(k_gemm<T, MT, TY, false>, p, a, 32 * TY, s);
+}
+
+template <typename T, int TY>
+void launch_ty(const GemmPlan<T> &p, const GemmArgs<T> &a, int grid, cudaStream_t s) {
+  switch (p.MT) {
+    case 2: launch_variant<T, 2, TY>(p, a, grid, s); break;
+    case 4: launch_variant<T, 4, TY>(p, a, grid, s); break;
+    case 6: launch_variant<T, 6, TY>(p, a, grid, s); break;
+    case 8: launch_variant<T, 8, TY>(p, a, grid, s); break;
+    case 10: launch_variant<T, 10, TY>(p, a, grid, s); break;
+    case 12: launch_variant<T, 12, TY>(p, a, grid, s); break;
+    case 14: launch_variant<T, 14, TY>(p, a, grid, s); break;
+    case 16: launch_variant<T, 16, TY>(p, a, grid, s); break;
+    default: throw Error{FR_EINVAL, "gemm: bad MT"};
+  }
+}
+
+}  // namespace
+
+int device_sm_count() {
+  static int n = 0;
+  if (n == 0) {
+    int dev = 0;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev);
+    if (n <= 0) n = 148;
+  }
+  return n;
+}
+
+template <typename T>
+void gemm_plan_build(GemmPlan<T> &p, int M, int K, const double *A_host) {
+  FR_REQUIRE(M > 0 && K > 0 && A_host, "gemm: M, K must be positive and A non-NULL");
+  constexpr int CT = VecT<T>::CT;
+  p.M = M;
+  p.K = K;
+  double best = 1e300;
+  const int tys[3] = {4, 6, 8};
+  for (int t = 0; t < 3; ++t)
+    for (int mt = 2; mt <= 16; mt += 2) {
+      const int tile = tys[t] * mt;
+      const int nrb = (M + tile - 1) / tile;
+      double score = (double)nrb * tile * (1.0 + 0.15 * (nrb - 1)) - 1e-3 * tys[t];
+      if (score < best) {
+        best = score;
+        p.TY = tys[t];
+        p.MT = mt;
+        p.nrb = nrb;
+      }
+    }
+  const int MTILE = p.TY * p.MT;
+  const int nchunks = (K + KC - 1) / KC;
+  const int Kpad = nchunks * KC;
+  const size_t bs_bytes = (size_t)NSTAGE * KC * 32 * CT * sizeof(T);
+  const size_t slab = (size_t)Kpad * MTILE * sizeof(T);
+  p.resident = slab <= 96 * 1024;
+  p.smem = bs_bytes + (p.resident ? slab : (size_t)NSTAGE * KC * MTILE * sizeof(T));
+  p.ctas_per_sm = (int)std::max<size_t>(1, std::min<size_t>(3, (200 * 1024) / p.smem));
+  // register file: 32*TY threads at <= 128 registers
+  p.ctas_per_sm = std::min(p.ctas_per_sm, std::max(1, 512 / (32 * p.TY)));
+  std::vector<T> At((size_t)p.nrb * Kpad * MTILE, T(0));
+  for (int m = 0; m < M; ++m) {
+    const int rb = m / MTILE, mm = m % MTILE;
+    for (int k = 0; k < K; ++k) {
+      const double v = A_host[(size_t)m * K + k];
+      FR_REQUIRE(v == v && v - v == 0.0, "gemm: operator contains non-finite entries");
+      At[((size_t)rb * Kpad + k) * MTILE + mm] = (T)v;
+    }
+  }
+  FR_CUDA_TRY(cudaMalloc(&p.At, At.size() * sizeof(T)));
+  FR_CUDA_TRY(cudaMemcpy(p.At, At.data(), At.size() * sizeof(T), cudaMemcpyHostToDevice));
+}
+
+template <typename T>
+void gemm_plan_free(GemmPlan<T> &p) {
+  if (p.At) cudaFree(p.At);
+  p.At = nullptr;
+}
+
+template <typename T>
+int gemm_run(const GemmPlan<T> &p, long long N, T c1, const T *B, long long ldb, long long bstrideB, T c2, T *C,
+             long long ldc, long long bstrideC, int nbatch, cudaStream_t s) {
+  constexpr int CT = VecT<T>::CT;
+  if (N <= 0 || nbatch <= 0) return 0;
+  FR_REQUIRE(ldb >= N && ldc >= N, "gemm: leading dimensions must be >= N");
+  FR_REQUIRE((ldb * sizeof(T)) % 16 == 0 && (ldc * sizeof(T)) % 16 == 0 && ((uintptr_t)B % 16) == 0 &&
+                 ((uintptr_t)C % 16) == 0 && (bstrideB * sizeof(T)) % 16 == 0 && (bstrideC * sizeof(T)) % 16 == 0,
+             "gemm: B and C rows must be 16-byte aligned");
+  GemmArgs<T> a;
+  a.M = p.M;
+  a.K = p.K;
+  a.nchunks = (p.K + KC - 1) / KC;
+  a.nrb = p.nrb;
+  a.nbatch = nbatch;
+  a.N = N;
+  a.ntn = (N + 32 * CT - 1) / (32 * CT);
+  a.At = p.At;
+  a.B = B;
+  a.C = C;
+  a.ldb = ldb;
+  a.ldc = ldc;
+  a.bsB = bstrideB;
+  a.bsC = bstrideC;
+  a.c1 = c1;
+  a.c2 = c2;
+  const int grid = 0;
+  switch (p.TY) {
+    case 4: launch_ty<T, 4>(p, a, grid, s); break;
+    case 6: launch_ty<T, 6>(p, a, grid, s); break;
+    case 8: launch_ty<T, 8>(p, a, grid, s); break;
+    default: throw Error{FR_EINVAL, "gemm: bad TY"};
+  }
+  return 1;
+}
+
+template void gemm_plan_build<double>(GemmPlan<double> &, int, int, const double *);
+template void gemm_plan_build<float>(GemmPlan<float> &, int, int, const double *);
+template void gemm_plan_free<double>(GemmPlan<double> &);
+template void gemm_plan_free<float>(GemmPlan<float> &);
+template int gemm_run<double>(const GemmPlan<double> &, long long, double, const double *, long long, long long, double,
+                              double *, long long, long long, int, cudaStream_t);
+template int gemm_run<float>(const GemmPlan<float> &, long long, float, const float *, long long, long long, float,
+                             float *, long long, long long, int, cudaStream_t);
+
+}  // namespace frb

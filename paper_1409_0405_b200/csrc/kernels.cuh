@@ -1,0 +1,60 @@
+// Device-side views and kernel launchers shared by the stage driver (api.cu).
+#pragma once
+#include "common.cuh"
+
+namespace frb {
+
+// One element type on the device (all arrays in precision T, element index fastest, leading dimension ld).
+template <typename T>
+struct EleView {
+  int nupts, nfpts, affine;
+  long long neles, ld;
+  const T *smats;     // [3][3][nupts][ld]  or [3][3][ld] if affine
+  const T *rcpdjac;   // [nupts][ld]        or [ld] if affine
+};
+
+template <typename T>
+struct IfaceView {
+  long long npairs;
+  const PairRec *pairs;
+  const T *nl;        // [3][npairs]
+  const T *magl, *magr;
+};
+
+template <typename T>
+struct BndView {
+  long long n;
+  int type;
+  const BndRec *recs;
+  const T *nrm;       // [3][n]
+  const T *mag;
+  T par[8];
+};
+
+// Fused Runge-Kutta stage update (S10): out1 = in1 + c1*K, out2 = in2 + c2*K with K = -R/|J|.
+// coef == nullptr: plain S9, out1 = K.
+template <typename T>
+struct StageArgs {
+  const StageCoef *coef;
+  const T *in1, *in2;
+  T *out1, *out2;
+};
+
+template <typename T>
+int launch_tdisf(const EleView<T> &ev, const T *u, T *gf, const PhysParams<T> &ph, cudaStream_t s);
+template <typename T>
+int launch_gradcoru(const EleView<T> &ev, T *g, cudaStream_t s);
+template <typename T>
+int launch_negdivconf(const EleView<T> &ev, const T *r, const StageArgs<T> &sa, cudaStream_t s);
+template <typename T>
+int launch_con_u(const IfaceView<T> &iv, const TypeTab &tt, const T *uf, T *cf, T beta, cudaStream_t s);
+template <typename T>
+int launch_comm_flux(const IfaceView<T> &iv, const TypeTab &tt, T *uf, const T *gf, const PhysParams<T> &ph,
+                     cudaStream_t s);
+template <typename T>
+int launch_bc_con_u(const BndView<T> &bv, const TypeTab &tt, const T *uf, T *cf, T gamma, cudaStream_t s);
+template <typename T>
+int launch_bc_comm_flux(const BndView<T> &bv, const TypeTab &tt, T *uf, const T *gf, const PhysParams<T> &ph,
+                        cudaStream_t s);
+
+}  // namespace frb

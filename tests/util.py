@@ -25,3 +25,23 @@ def conservation_defect(case, dudt):
 def oracle_rhs(case, us=None):
     from oracle import fr_oracle
     return fr_oracle.rhs(case["cfg"], case["eles"], case["ifc"], case["bcs"], case["u0"] if us is None else us)
+
+
+EPS32 = 2.0 ** -24
+
+
+def oracle_rhs_with_amplification(case, us=None):
+    """Oracle RHS plus the a-priori round-off amplification of its last step per variable (reading R23):
+    amp_k = max (|M132| |F~| + |M3| |D|) / |J|  divided by  max |dudt_k|.  A computation that stores F~ and D in a
+    precision with unit round-off eps cannot be closer to the exact result than ~ eps * amp_k."""
+    from oracle import fr_oracle
+    parts = {}
+    ref = fr_oracle.rhs(case["cfg"], case["eles"], case["ifc"], case["bcs"], case["u0"] if us is None else us, parts)
+    A, den = np.zeros(5), np.zeros(5)
+    for e, ft, d, r in zip(case["eles"], parts["ftil"], parts["d"], ref):
+        nu = e["nupts"]
+        a = (np.abs(e["M132"]) @ np.abs(ft.reshape(3 * nu, -1)) + np.abs(e["M3"]) @ np.abs(d.reshape(d.shape[0], -1)))
+        a = a.reshape(r.shape) * e["rcpdjac"][:, None, :]
+        A = np.maximum(A, a.max(axis=(0, 2)))
+        den = np.maximum(den, np.abs(r).max(axis=(0, 2)))
+    return ref, A / np.maximum(den, 1e-300)
