@@ -1,0 +1,296 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the flux-reconstruction hot path on B200 (contract: see DESIGN.md "Measurement").
+
+Workload (BASELINE.json configs[2], "RK45 stages timed"): the synthetic cylinder-like O-mesh of 120 000 prisms +
+360 000 tetrahedra at p = 4 (21.6 M solution points), compressible Navier-Stokes at Re = 3900, M = 0.2, Rusanov +
+LDG, RK45[2R+].  One "step" = one RK45[2R+] time step = 5 evaluations of the whole right-hand side (S1..S10 of
+SURVEY 8(a)) through the C ABI (`fr_rk_step`).  metric = GDOF-RHS/s = solution points x RHS evaluations / s / 1e9.
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl frb200|reference] [--small]
+
+`--impl reference` times the CPU oracle (oracle/fr_oracle.py, FP64 numpy, as it stands) on the host cores on a
+bounded sample of the same workload.  Under torchrun each rank runs an independent replica (DESIGN.md "Multi-GPU":
+replicas only, no collective on the data path).
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+import numpy as np  # noqa: E402
+
+METRIC = "GDOF-RHS/s"
+FULL = dict(p=4, ntheta=100, nz=15, nlayers=40, nr=40)      # BASELINE.json configs[2]
+SMALL = dict(p=4, ntheta=24, nz=4, nlayers=10, nr=10)       # --small: quick functional check only
+SAMPLE = dict(p=4, ntheta=40, nz=6, nlayers=40, nr=40)      # bounded sample for the CPU oracle (16 % of FULL)
+DT = 2e-6
+
+
+def _peaks():
+    """Roofline denominators: MEASURED_PEAKS.json (driver-written) else the profiling guide's fallback."""
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    try:
+        with open(path) as f:
+            d = json.load(f)
+        return float(d["hbm_gbs"]), "MEASURED_PEAKS.json hbm_gbs"
+    except Exception:
+        return 6550.0, "fallback (B200_PROFILING.md measured copy rate)"
+
+
+class ClockSampler(threading.Thread):
+    """Samples SM clock and throttle reasons with nvidia-smi while the timed region runs."""
+
+    def __init__(self, index=0, period=0.2):
+        super().__init__(daemon=True)
+        self.index, self.period = index, period
+        self.samples, self.reasons, self.maxmhz = [], set(), None
+        self._stop_evt = threading.Event()
+
+    def _query(self):
+        q = "clocks.sm,clocks.max.sm,clocks_event_reasons.active"
+        try:
+            out = subprocess.run(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + q, "--format=csv,noheader,nounits"],
+                                 capture_output=True, text=True, timeout=5).stdout.strip()
+            a = [x.strip() for x in out.split(",")]
+            self.samples.append(float(a[0]))
+            self.maxmhz = float(a[1])
+            bits = int(a[2], 16)
+            names = {0x1: "gpu_idle", 0x2: "applications_clocks_setting", 0x4: "sw_power_cap", 0x8: "hw_slowdown",
+                     0x10: "sync_boost", 0x20: "sw_thermal_slowdown", 0x40: "hw_thermal_slowdown",
+                     0x80: "hw_power_brake_slowdown", 0x100: "display_clock_setting"}
+            for b, n in names.items():
+                if bits & b and n != "gpu_idle":
+                    self.reasons.add(n)
+        except Exception:
+            pass
+
+    def run(self):
+        while not self._stop_evt.is_set():
+            self._query()
+            self._stop_evt.wait(self.period)
+
+    def stop(self):
+        self._stop_evt.set()
+        self.join(timeout=10)
+        s = sorted(self.samples)
+        return dict(sm_mhz=(s[len(s) // 2] if s else None), sm_max_mhz=self.maxmhz, reasons=sorted(self.reasons),
+                    samples=len(s))
+
+
+def _case(kind):
+    from fr_inputs import cases
+    return cases.config3(**kind)
+
+
+def _workload_name(kind, case):
+    ne = {e["etype"]: e["neles"] for e in case["eles"]}
+    return "config3 cylinder O-mesh p=%d NS RK45[2R+]: %d pri + %d tet" % (kind["p"], ne.get("pri", 0), ne.get("tet", 0))
+
+
+# ------------------------------------------------------------------------------------------------ CPU oracle arm
+def oracle_rate(case, nrhs, budget_s=40.0):
+    """GDOF-RHS/s of the oracle as it stands on this host: `nrhs` RHS evaluations (at least one)."""
+    from fr_inputs import cases
+    from oracle import fr_oracle as O
+    n = cases.ndof(case)
+    t0 = time.perf_counter()
+    done = 0
+    us = case["u0"]
+    for _ in range(max(1, nrhs)):
+        O.rhs(case["cfg"], case["eles"], case["ifc"], case["bcs"], us)
+        done += 1
+        if time.perf_counter() - t0 > budget_s:
+            break
+    dt = time.perf_counter() - t0
+    return n * done / dt / 1e9, done, dt
+
+
+def _blas_threads():
+    try:
+        from threadpoolctl import threadpool_info
+        return max([i.get("num_threads", 1) for i in threadpool_info()] + [1])
+    except Exception:
+        return os.cpu_count() or 1
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    kind = SMALL if args.small else SAMPLE
+    case = _case(kind)
+    from fr_inputs import cases
+    for _ in range(args.warmup and 1):
+        oracle_rate(case, 1)
+    # one "step" of this arm = one RHS evaluation of the bounded sample (an RK45 step is 5 of them)
+    rate, done, dt = oracle_rate(case, args.steps, budget_s=150.0)
+    cores = _blas_threads()
+    sample = "%s (%d DOF, %.0f %% of the full workload), %d RHS evaluations" % (
+        _workload_name(kind, case), cases.ndof(case), 100.0 * cases.ndof(case) / 21.6e6, done)
+    line = dict(impl="reference", metric=METRIC, value=rate, unit="GDOF-RHS/s", n_gpus=args.gpus, steps=done,
+                warmup=args.warmup, ms_per_step=1e3 * dt / done, higher_is_better=True, scaling="weak", vs_baseline=None,
+                dtype="f64", data="synthetic",
+                config=dict(workload=_workload_name(FULL if not args.small else SMALL, case), sample=sample),
+                cpu_baseline=dict(value=rate, unit="GDOF-RHS/s", cores=cores, kind="oracle", sample=sample),
+                e2e=dict(value=rate, unit="GDOF-RHS/s", h2d_bytes_per_step=0, d2h_bytes_per_step=0), gpu_launches=0)
+    print(json.dumps(line))
+
+
+# ------------------------------------------------------------------------------------------------ CUDA arm
+def _time_steps(ctx, stream, dt, steps, torch):
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(stream)
+    ctx.rk_run(dt, steps)
+    e1.record(stream)
+    e1.synchronize()
+    return e0.elapsed_time(e1) * 1e-3
+
+
+def _measure(case, prec, args, torch, dist, rank, world, with_e2e=True, sampler=None):
+    from fr_inputs import cases
+    from paper_1409_0405_b200 import Context
+    stream = torch.cuda.Stream()
+    ctx = Context(case, prec=prec, stepper="rk45", stream=stream.cuda_stream)
+    ndof = cases.ndof(case)
+    ctx.set_state(case["u0"])
+    ctx.rk_run(DT, args.warmup)
+    ctx.sync()
+    n0 = ctx.launch_count()
+    if world > 1:
+        dist.barrier()
+    torch.cuda.synchronize()
+    if sampler is not None:
+        sampler.start()
+    sec = _time_steps(ctx, stream, DT, args.steps, torch)
+    torch.cuda.synchronize()
+    clocks = sampler.stop() if sampler is not None else None
+    launches = ctx.launch_count() - n0
+    if world > 1:
+        t = torch.tensor([sec], dtype=torch.float64, device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        sec = float(t.item())
+    nstage = 5
+    res = dict(seconds=sec, value=world * ndof * nstage * args.steps / sec / 1e9, launches=launches, clocks=clocks,
+               ndof=ndof)
+    # state must still be finite after the timed steps (a blown-up run would be timing NaN arithmetic)
+    chk = ctx.get_state()
+    res["finite"] = bool(all(np.isfinite(a).all() for a in chk))
+    # per-kernel CUDA-event breakdown of one RHS (same context, same data, right after the timed region)
+    ks = ctx.profile_kernels(reps=3)
+    res["kernels"] = ks
+    if with_e2e:
+        # end to end through the C ABI with HOST buffers: H2D of the state, one RK45 step, D2H of the new state
+        tdt = torch.float64 if prec == "f64" else torch.float32
+        hbuf = []
+        for u, ld in zip(chk, ctx.ld):
+            h = torch.zeros((u.shape[0], 5, ld), dtype=tdt).pin_memory()
+            h[:, :, :u.shape[2]] = torch.from_numpy(np.ascontiguousarray(u)).to(tdt)
+            hbuf.append(h)
+        ptrs = [h.data_ptr() for h in hbuf]
+        ne2e = max(2, min(args.steps, 5))
+        ctx.rk_step_host(DT, ptrs)
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        for _ in range(ne2e):
+            ctx.rk_step_host(DT, ptrs)
+        torch.cuda.synchronize()
+        t1 = time.perf_counter() - t0
+        if world > 1:
+            t = torch.tensor([t1], dtype=torch.float64, device="cuda")
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            t1 = float(t.item())
+        nb = int(sum(h.numel() * h.element_size() for h in hbuf))
+        res["e2e"] = dict(value=world * ndof * nstage * ne2e / t1 / 1e9, unit="GDOF-RHS/s", h2d_bytes_per_step=nb,
+                          d2h_bytes_per_step=nb, steps=ne2e)
+    ctx.close()
+    return res
+
+
+def _roofline(kernels, peak, peak_src):
+    """Dominant kernel of one RHS by CUDA-event time; achieved = algorithmic bytes per launch / mean duration."""
+    tot = sum(k["ms"] for k in kernels)
+    top = max(kernels, key=lambda k: k["ms"])
+    ach = top["alg_bytes"] / (top["ms"] * 1e-3) / 1e9
+    whole = sum(k["alg_bytes"] for k in kernels) / (tot * 1e-3) / 1e9
+    return dict(bound="hbm", kernel=top["name"], achieved=ach, peak=peak, unit="GB/s", frac=ach / peak, traffic=None,
+                peak_source=peak_src, share_of_rhs=top["ms"] / tot, ms_per_launch=top["ms"],
+                alg_bytes_per_launch=top["alg_bytes"], tflops=top["flops"] / (top["ms"] * 1e-3) / 1e12,
+                whole_rhs=dict(alg_gbs=whole, frac=whole / peak, ms=tot,
+                               tflops=sum(k["flops"] for k in kernels) / (tot * 1e-3) / 1e12))
+
+
+def run_frb200(args):
+    import torch
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (there is no CPU fallback; use --impl reference for the oracle)")
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    kind = SMALL if args.small else FULL
+    case = _case(kind)
+    peak, peak_src = _peaks()
+    sampler = ClockSampler(index=local) if rank == 0 else None
+    r64 = _measure(case, "f64", args, torch, dist, rank, world, sampler=sampler)
+    r32 = _measure(case, "f32", args, torch, dist, rank, world, with_e2e=False)
+    if rank == 0:
+        cpu = None
+        if world == 1 and not args.no_cpu_baseline:
+            scase = case if args.small else _case(SAMPLE)
+            from fr_inputs import cases
+            v, done, dt = oracle_rate(scase, 2, budget_s=20.0)
+            cpu = dict(value=v, unit="GDOF-RHS/s", cores=_blas_threads(), kind="oracle",
+                       sample="%s (%d DOF), %d RHS evaluations in %.1f s" % (
+                           _workload_name(SMALL if args.small else SAMPLE, scase), cases.ndof(scase), done, dt))
+        ms = 1e3 * r64["seconds"] / args.steps
+        line = dict(metric=METRIC, value=r64["value"], unit="GDOF-RHS/s", n_gpus=world, steps=args.steps,
+                    warmup=args.warmup, ms_per_step=ms, higher_is_better=True, scaling="weak", vs_baseline=None,
+                    dtype="f64", data="synthetic",
+                    config=dict(workload=_workload_name(kind, case), dof=r64["ndof"], rhs_per_step=5, dt=DT,
+                                parallelism="replicas only" if world > 1 else "single GPU",
+                                l2="state 0.86 GB (FP64) per register, working set >> 126 MB L2: no flush needed"),
+                    clocks=r64["clocks"], e2e=r64["e2e"], gpu_launches=r64["launches"],
+                    roofline=_roofline(r64["kernels"], peak, peak_src), cpu_baseline=cpu, finite=r64["finite"],
+                    fp32=dict(value=r32["value"], unit="GDOF-RHS/s", ms_per_step=1e3 * r32["seconds"] / args.steps,
+                              dtype="f32", gpu_launches=r32["launches"], finite=r32["finite"],
+                              roofline=_roofline(r32["kernels"], peak, peak_src)))
+        if args.kernels:
+            line["kernels_f64"] = r64["kernels"]
+            line["kernels_f32"] = r32["kernels"]
+        print(json.dumps(line))
+    if world > 1:
+        dist.barrier()
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="frb200", choices=["frb200", "reference"])
+    ap.add_argument("--small", action="store_true", help="small mesh (functional check, not a bench number)")
+    ap.add_argument("--kernels", action="store_true", help="add the per-kernel breakdown to the JSON line")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "frb200" else args.warmup
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_frb200(args)
+
+
+if __name__ == "__main__":
+    main()
