@@ -61,6 +61,9 @@ struct StageCoef {
 };
 
 template <typename T>
+struct PanelOp;   // panel.cuh: operator packed for the resident-operator panel kernels
+
+template <typename T>
 struct GemmPlan {
   int M = 0, K = 0;
   int TY = 0, MT = 0, nrb = 0;   // thread rows, rows per thread, row blocks (M <= nrb*TY*MT)
@@ -68,6 +71,7 @@ struct GemmPlan {
   int ctas_per_sm = 1;
   size_t smem = 0;
   T *At = nullptr;               // device, [nrb][K][TY*MT], zero padded, transposed operator
+  PanelOp<T> *pop = nullptr;     // non-null: the panel kernel serves this operator (At is then unused)
 };
 
 template <typename T>

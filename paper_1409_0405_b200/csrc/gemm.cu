@@ -14,8 +14,15 @@
 #include <algorithm>
 
 #include "common.cuh"
+#include "panel.cuh"
 
 namespace frb {
+
+template <typename T>
+bool panel_gemm_build(PanelOp<T> &op, int M, int K, const double *A);
+template <typename T>
+void panel_gemm_run(const PanelOp<T> &op, long long N, T c1, const T *B, long long ldb, long long bsB, T c2, T *C,
+                    long long ldc, long long bsC, int nbatch, cudaStream_t s);
 
 namespace {
 
@@ -249,6 +256,22 @@ void gemm_plan_build(GemmPlan<T> &p, int M, int K, const double *A_host) {
   constexpr int CT = VecT<T>::CT;
   p.M = M;
   p.K = K;
+  {
+    // preferred path: operator resident in shared memory, all rows in one CTA (panel.cuh)
+    auto *pop = new PanelOp<T>();
+    bool ok = false;
+    try {
+      ok = panel_gemm_build(*pop, M, K, A_host);
+    } catch (...) {
+      delete pop;
+      throw;
+    }
+    if (ok) {
+      p.pop = pop;
+      return;
+    }
+    delete pop;
+  }
   double best = 1e300;
   const int tys[3] = {4, 6, 8};
   for (int t = 0; t < 3; ++t)
@@ -290,6 +313,11 @@ template <typename T>
 void gemm_plan_free(GemmPlan<T> &p) {
   if (p.At) cudaFree(p.At);
   p.At = nullptr;
+  if (p.pop) {
+    panel_op_free(*p.pop);
+    delete p.pop;
+    p.pop = nullptr;
+  }
 }
 
 template <typename T>
@@ -301,6 +329,10 @@ int gemm_run(const GemmPlan<T> &p, long long N, T c1, const T *B, long long ldb,
   FR_REQUIRE((ldb * sizeof(T)) % 16 == 0 && (ldc * sizeof(T)) % 16 == 0 && ((uintptr_t)B % 16) == 0 &&
                  ((uintptr_t)C % 16) == 0 && (bstrideB * sizeof(T)) % 16 == 0 && (bstrideC * sizeof(T)) % 16 == 0,
              "gemm: B and C rows must be 16-byte aligned");
+  if (p.pop) {
+    panel_gemm_run(*p.pop, N, c1, B, ldb, bstrideB, c2, C, ldc, bstrideC, nbatch, s);
+    return 1;
+  }
   GemmArgs<T> a;
   a.M = p.M;
   a.K = p.K;

@@ -1,0 +1,626 @@
+// Panel kernels: the operator products C <- c1*A*B + c2*C (eq. 1) and their fusions with the adjacent
+// point-wise work, for one element type.  "A is a constant operator matrix, and B and C are row-major state matrices"
+// (PAPER.md:39): every column of B is independent, so one CTA owns a *panel* of NE consecutive elements (all 5
+// conserved variables = 5*NE columns) and ALL rows of A -- the column slicing the paper's OpenMP backend found best
+// -- while B streams through shared memory in K-chunks and the accumulators stay in registers.
+//
+// B200 design:
+//   * the operator is packed once at fr_setup into 8-row groups with a compact list of the k indices that are non-zero
+//     in the group (dense operators: all k; prism operators are 15-45 % dense and skip the rest) and stays resident in
+//     shared memory for the life of the persistent CTA;
+//   * FP64 multiplies on the FP64 tensor pipe, mma.sync.m8n8k4.f64 (DMMA: measured 37.1 TFLOP/s on B200 against 33.7
+//     for a DFMA chain, with 1/8 of the issue slots and a fraction of the shared-memory operand traffic);
+//     FP32 multiplies with FFMA on register tiles of 8 rows x 5 variables x (1|2) elements (no TF32: the 2e-5 parity
+//     bound excludes it, and tcgen05 has no FP32/FP64 kind);
+//   * B chunks arrive through a multi-stage cp.async ring that runs across panel boundaries; rows are padded so that the
+//     DMMA fragment loads are bank-conflict free;
+//   * producers (how a B chunk comes to be) and epilogues (what happens to the accumulators) are policies, which is how the
+//     point-wise flux, gradient transform, -1/|J| scaling and Runge-Kutta stage update are fused into the products.
+#pragma once
+#include <algorithm>
+#include <cmath>
+#include <cstring>
+#include <numeric>
+
+#include "common.cuh"
+
+namespace frb {
+
+constexpr int PV = FR_NVAR;          // variable segments per panel
+constexpr int PANEL_MAXW = 16;       // warps per CTA (upper bound; 8 when the accumulators need > 128 registers)
+constexpr int PANEL_MAXCHUNKS = 64;
+
+// One K-chunk of the stacked right-hand operand: rows [row0, row0+nrows) of source `src`.
+struct ChunkDesc {
+  int src, row0, nrows, kind;
+};
+
+// Device image of a packed operator + its launch geometry (all pointers device).
+template <typename T>
+struct PanelOp {
+  int M = 0, K = 0;
+  int WR = 0, WC = 0, NIT = 0, CX = 0;   // warp grid, row groups per row-warp, column blocks (FP64) / elements per lane (FP32)
+  int NE = 0;                            // elements per panel
+  int KC = 0, nchunks = 0, NS = 0;       // rows per chunk (max), chunks, slots = WR*NIT
+  int nblk = 0;                          // packed blocks (FP64: 8x4 tiles; FP32: 8x1 columns)
+  int sparse = 0;
+  double macs_per_col = 0;               // executed multiply-adds per column (dense: M*K)
+  T *vals = nullptr;                     // FP64 [nblk][32]; FP32 [nblk][8]
+  uint32_t *idx = nullptr;               // byte offset of the B row in the stage: FP64 [nblk][4], FP32 [nblk]
+  int *off = nullptr;                    // [nchunks*NS + 1]
+  int *rowmap = nullptr;                 // [NS*8] actual row of (slot, r) or -1
+  ChunkDesc *chunks = nullptr;           // [nchunks]
+  size_t smem_op = 0;                    // bytes of the operator image in shared memory
+  bool ok() const { return vals != nullptr; }
+};
+
+template <typename T>
+void panel_op_free(PanelOp<T> &p) {
+  if (p.vals) cudaFree(p.vals);
+  if (p.idx) cudaFree(p.idx);
+  if (p.off) cudaFree(p.off);
+  if (p.rowmap) cudaFree(p.rowmap);
+  if (p.chunks) cudaFree(p.chunks);
+  p = PanelOp<T>();
+}
+
+// How the K dimension of the operator is fed: a list of sources stacked along K, each cut into chunks of at most KC rows.
+struct KSource {
+  int rows;      // rows of this source (columns of A it multiplies)
+  int kind;      // producer-specific tag (0 = plain rows of a matrix)
+  int unit;      // chunk granularity: chunk rows are a multiple of `unit` (e.g. 3 for (alpha, nu) triples)
+};
+
+struct PanelGeom {
+  int WR, WC, NIT, CX, NE;
+  double eff;
+};
+
+// Accumulator budget: a CTA of up to 16 warps (128 registers per thread) if NIT*CX <= small, else up to 8 warps.
+// FP64: NIT*CX*10 doubles per thread; FP32: NIT*CX*40 floats.
+template <typename T>
+constexpr int panel_maxw(int nit, int cx) {
+  return sizeof(T) == 8 ? (nit * cx <= 4 ? 16 : 8) : (nit * cx <= 2 ? 16 : 8);
+}
+
+// Choose the warp grid for G row groups.  The FP64 tensor pipe takes one DMMA per warp every ~32 cycles, so two warps per
+// scheduler saturate it only if they do nothing else: prefer 12-16 warps per SM.
+template <typename T>
+inline PanelGeom choose_geom(int G, int min_ne, int max_ne, int triple) {
+  PanelGeom best{0, 0, 0, 0, 0, -1.0};
+  const bool f64 = sizeof(T) == 8;
+  const int gu = triple ? 3 : 1;            // groups come in units of `gu` that must stay on one row-warp
+  const int GU = (G + gu - 1) / gu;
+  for (int WR = 1; WR <= PANEL_MAXW; ++WR) {
+    const int nit = ((GU + WR - 1) / WR) * gu;
+    for (int WC = 1; WR * WC <= PANEL_MAXW; WC *= 2) {
+      for (int CX = 2; CX >= 1; --CX) {
+        if (f64 ? nit * CX > 8 : nit * CX > 4) continue;
+        const int W = WR * WC;
+        if (W > panel_maxw<T>(nit, CX)) continue;
+        const int NE = (f64 ? 8 : 32) * CX * WC;
+        if (NE < min_ne || NE > max_ne) continue;
+        double eff = (double)G / (WR * nit);
+        // prefer many warps, then wider panels, then fewer accumulators
+        double score = eff * (0.4 + 0.6 * std::min(W, 14) / 14.0) * (1.0 + 0.02 * std::log2((double)NE)) * (1.0 - 0.005 * nit * CX);
+        if (score > best.eff) best = PanelGeom{WR, WC, nit, CX, NE, score};
+      }
+    }
+  }
+  return best;
+}
+
+// Greedy clustering of rows into groups of 8 with similar column support (sparse operators only).
+inline std::vector<int> cluster_rows(const std::vector<std::vector<uint8_t>> &sup, int M, int K) {
+  std::vector<int> order;
+  std::vector<char> used(M, 0);
+  std::vector<int> cnt(M, 0);
+  for (int m = 0; m < M; ++m)
+    for (int k = 0; k < K; ++k) cnt[m] += sup[m][k];
+  int remaining = M;
+  while (remaining > 0) {
+    // seed: the unused row with the largest support
+    int seed = -1;
+    for (int m = 0; m < M; ++m)
+      if (!used[m] && (seed < 0 || cnt[m] > cnt[seed])) seed = m;
+    std::vector<uint8_t> u = sup[seed];
+    used[seed] = 1;
+    order.push_back(seed);
+    --remaining;
+    for (int j = 1; j < 8 && remaining > 0; ++j) {
+      int bi = -1;
+      int bgrow = 1 << 30, bshare = -1;
+      for (int m = 0; m < M; ++m) {
+        if (used[m]) continue;
+        int grow = 0, share = 0;
+        for (int k = 0; k < K; ++k) {
+          grow += sup[m][k] & ~u[k] & 1;
+          share += sup[m][k] & u[k];
+        }
+        if (grow < bgrow || (grow == bgrow && share > bshare)) {
+          bgrow = grow;
+          bshare = share;
+          bi = m;
+        }
+      }
+      used[bi] = 1;
+      order.push_back(bi);
+      --remaining;
+      for (int k = 0; k < K; ++k) u[k] |= sup[bi][k];
+    }
+    while (order.size() % 8) order.push_back(-1);
+  }
+  return order;
+}
+
+struct PackOptions {
+  int min_ne = 16, max_ne = 64;
+  int triple = 0;          // rows come as (alpha, rho) with alpha-major blocks of M/3: keep the three alpha of a rho in one thread
+  int kc = 0;              // rows per chunk (0 = default)
+  int allow_sparse = 1;
+};
+
+// Pack A (M x K, host FP64, row-major) for the panel kernels.  `srcs` stacks the K dimension.  Returns false if the
+// operator does not fit the resident-in-shared-memory design (caller falls back to the streaming kernel).
+template <typename T>
+bool panel_op_build_kc(PanelOp<T> &p, int M, int K, const double *A, const std::vector<KSource> &srcs, const PackOptions &opt,
+                       size_t smem_budget, size_t smem_total, int kc_try, int *kc_fit);
+
+// Chunk height: as tall as the B ring allows (few, large cp.async stages keep enough bytes in flight to cover HBM latency
+// with one persistent CTA per SM); first try whole sources, then the height that makes three stages fit `smem_total`.
+template <typename T>
+bool panel_op_build(PanelOp<T> &p, int M, int K, const double *A, const std::vector<KSource> &srcs, const PackOptions &opt,
+                    size_t smem_budget, size_t smem_total = 200 * 1024) {
+  int kc = opt.kc > 0 ? opt.kc : 252;
+  for (int attempt = 0; attempt < 6 && kc >= 4; ++attempt) {
+    int fit = 0;
+    if (panel_op_build_kc(p, M, K, A, srcs, opt, smem_budget, smem_total, kc, &fit)) return true;
+    if (fit <= 0) return false;
+    kc = std::min(fit, kc - 4);
+  }
+  return false;
+}
+
+template <typename T>
+bool panel_op_build_kc(PanelOp<T> &p, int M, int K, const double *A, const std::vector<KSource> &srcs, const PackOptions &opt,
+                       size_t smem_budget, size_t smem_total, int kc_try, int *kc_fit) {
+  const bool f64 = sizeof(T) == 8;
+  int ktot = 0;
+  for (auto &s : srcs) ktot += s.rows;
+  FR_REQUIRE(ktot == K, "panel_op_build: sources do not add up to K");
+  double amax = 0;
+  for (size_t i = 0; i < (size_t)M * K; ++i) {
+    FR_REQUIRE(A[i] == A[i] && A[i] - A[i] == 0.0, "operator contains non-finite entries");
+    amax = std::max(amax, std::fabs(A[i]));
+  }
+  // structural zeros: entries below 2^-46 of the largest entry are dropped (reading R24)
+  const double thr = amax * 1.4210854715202004e-14;
+  std::vector<std::vector<uint8_t>> sup(M, std::vector<uint8_t>(K, 0));
+  size_t nnz = 0;
+  for (int m = 0; m < M; ++m)
+    for (int k = 0; k < K; ++k)
+      if (std::fabs(A[(size_t)m * K + k]) > thr) {
+        sup[m][k] = 1;
+        ++nnz;
+      }
+  const double density = (double)nnz / ((double)M * K);
+  const bool sparse = opt.allow_sparse && density < 0.6;
+  // ---- rows -> groups of 8
+  std::vector<int> order;   // virtual row -> actual row or -1
+  if (opt.triple) {
+    FR_REQUIRE(M % 3 == 0, "triple packing needs M divisible by 3");
+    const int nu = M / 3;
+    std::vector<int> rho_order;
+    if (sparse) {
+      std::vector<std::vector<uint8_t>> s3(nu, std::vector<uint8_t>(K, 0));
+      for (int r = 0; r < nu; ++r)
+        for (int a = 0; a < 3; ++a)
+          for (int k = 0; k < K; ++k) s3[r][k] |= sup[a * nu + r][k];
+      rho_order = cluster_rows(s3, nu, K);
+    } else {
+      for (int r = 0; r < nu; ++r) rho_order.push_back(r);
+      while (rho_order.size() % 8) rho_order.push_back(-1);
+    }
+    // group 3g+a holds rows (a, rho_order[8g .. 8g+7])
+    for (size_t g = 0; g < rho_order.size() / 8; ++g)
+      for (int a = 0; a < 3; ++a)
+        for (int r = 0; r < 8; ++r) {
+          const int rho = rho_order[8 * g + r];
+          order.push_back(rho < 0 ? -1 : a * nu + rho);
+        }
+  } else if (sparse) {
+    order = cluster_rows(sup, M, K);
+  } else {
+    for (int m = 0; m < M; ++m) order.push_back(m);
+    while (order.size() % 8) order.push_back(-1);
+  }
+  const int G = (int)order.size() / 8;
+  // ---- chunks
+  const int KC = kc_try;
+  std::vector<ChunkDesc> chunks;
+  std::vector<int> chunk_k0;   // first column of A of each chunk
+  {
+    int k0 = 0, si = 0;
+    for (auto &s : srcs) {
+      // equal chunks of at most KC rows, a multiple of lcm(unit, 4) so that dense k-lists need no padding
+      const int unit = std::max(1, s.unit);
+      const int q = unit % 4 == 0 ? unit : (unit % 2 == 0 ? 2 * unit : 4 * unit);
+      const int nch = std::max(1, (s.rows + KC - 1) / KC);
+      int step = ((s.rows + nch - 1) / nch + q - 1) / q * q;
+      if (step > KC) step = std::max(q, KC / q * q);
+      for (int r = 0; r < s.rows; r += step) {
+        chunks.push_back(ChunkDesc{si, r, std::min(step, s.rows - r), s.kind});
+        chunk_k0.push_back(k0 + r);
+      }
+      k0 += s.rows;
+      ++si;
+    }
+  }
+  const int nchunks = (int)chunks.size();
+  if (nchunks > PANEL_MAXCHUNKS) return false;
+  int kcmax = 0;
+  for (auto &c : chunks) kcmax = std::max(kcmax, c.nrows);
+  if (kcmax > 255) return false;
+  // ---- cost of each group (number of listed k) and its assignment to row-warps
+  std::vector<std::vector<std::vector<int>>> lists(G, std::vector<std::vector<int>>(nchunks));
+  std::vector<long long> gcost(G, 0);
+  for (int g = 0; g < G; ++g)
+    for (int c = 0; c < nchunks; ++c) {
+      for (int kk = 0; kk < chunks[c].nrows; ++kk) {
+        bool any = !sparse;
+        for (int r = 0; r < 8 && !any; ++r) {
+          const int m = order[8 * g + r];
+          if (m >= 0 && sup[m][chunk_k0[c] + kk]) any = true;
+        }
+        if (any) lists[g][c].push_back(kk);
+      }
+      const int n = (int)lists[g][c].size();
+      gcost[g] += f64 ? (n + 3) / 4 * 4 : n;
+    }
+  PanelGeom geo = choose_geom<T>(G, opt.min_ne, opt.max_ne, opt.triple);
+  if (geo.eff < 0) return false;
+  const int WR = geo.WR, NIT = geo.NIT, NS = WR * NIT;
+  // LPT assignment of group units (1 or 3 groups) to row-warps, at most NIT groups per row-warp
+  const int gu = opt.triple ? 3 : 1;
+  const int GU = G / gu;
+  std::vector<int> uorder(GU);
+  std::iota(uorder.begin(), uorder.end(), 0);
+  auto ucost = [&](int u) {
+    long long c = 0;
+    for (int j = 0; j < gu; ++j) c += gcost[u * gu + j];
+    return c;
+  };
+  std::stable_sort(uorder.begin(), uorder.end(), [&](int a, int b) { return ucost(a) > ucost(b); });
+  std::vector<long long> wload(WR, 0);
+  std::vector<int> wcount(WR, 0);
+  std::vector<int> slot_group(NS, -1);
+  for (int u : uorder) {
+    int bw = -1;
+    for (int w = 0; w < WR; ++w)
+      if (wcount[w] + gu <= NIT && (bw < 0 || wload[w] < wload[bw])) bw = w;
+    FR_REQUIRE(bw >= 0, "panel_op_build: slot assignment failed");
+    for (int j = 0; j < gu; ++j) slot_group[bw * NIT + wcount[bw] + j] = u * gu + j;
+    wcount[bw] += gu;
+    wload[bw] += ucost(u);
+  }
+  // ---- pack
+  std::vector<T> vals;
+  std::vector<uint32_t> idx;
+  std::vector<int> off(nchunks * NS + 1, 0);
+  std::vector<int> rowmap(NS * 8, -1);
+  for (int s = 0; s < NS; ++s)
+    if (slot_group[s] >= 0)
+      for (int r = 0; r < 8; ++r) rowmap[s * 8 + r] = order[8 * slot_group[s] + r];
+  long long macs = 0;
+  int nblk = 0;
+  for (int c = 0; c < nchunks; ++c)
+    for (int s = 0; s < NS; ++s) {
+      off[c * NS + s] = nblk;
+      const int g = slot_group[s];
+      if (g < 0) continue;
+      const std::vector<int> &L = lists[g][c];
+      const int n = (int)L.size();
+      if (f64) {
+        for (int b = 0; b < (n + 3) / 4; ++b) {
+          for (int j = 0; j < 4; ++j) {
+            const int kk = 4 * b + j < n ? L[4 * b + j] : 0;
+            idx.push_back((uint32_t)kk * (uint32_t)(PV * geo.NE + 4) * (uint32_t)sizeof(T));
+          }
+          for (int lane = 0; lane < 32; ++lane) {
+            const int r = lane >> 2, j = lane & 3;
+            const int m = order[8 * g + r];
+            double v = 0;
+            if (m >= 0 && 4 * b + j < n) v = A[(size_t)m * K + chunk_k0[c] + L[4 * b + j]];
+            if (sparse && std::fabs(v) <= thr) v = 0;
+            vals.push_back((T)v);
+          }
+          ++nblk;
+          macs += 32;
+        }
+      } else {
+        for (int b = 0; b < n; ++b) {
+          idx.push_back((uint32_t)L[b] * (uint32_t)(PV * geo.NE + 4) * (uint32_t)sizeof(T));
+          for (int r = 0; r < 8; ++r) {
+            const int m = order[8 * g + r];
+            double v = m >= 0 ? A[(size_t)m * K + chunk_k0[c] + L[b]] : 0.0;
+            if (sparse && std::fabs(v) <= thr) v = 0;
+            vals.push_back((T)v);
+          }
+          ++nblk;
+          macs += 8;
+        }
+      }
+    }
+  off[nchunks * NS] = nblk;
+  // the multiply loop prefetches two blocks ahead: two all-zero blocks close the arrays (not counted in nblk)
+  for (int d = 0; d < 2; ++d) {
+    for (int j = 0; j < (f64 ? 4 : 1); ++j) idx.push_back(0u);
+    for (int j = 0; j < (f64 ? 32 : 8); ++j) vals.push_back(T(0));
+  }
+  const size_t smem_op = ((vals.size() * sizeof(T) + 15) / 16 * 16) + ((idx.size() * 4 + 15) / 16 * 16) +
+                         ((off.size() * 4 + 15) / 16 * 16) + ((rowmap.size() * 4 + 15) / 16 * 16) +
+                         ((chunks.size() * sizeof(ChunkDesc) + 15) / 16 * 16);
+  if (smem_op > smem_budget) return false;
+  if (smem_op + (size_t)3 * kcmax * (PV * geo.NE + 4) * sizeof(T) + 16 > smem_total) {
+    if (smem_total > smem_op + 4096) *kc_fit = (int)((smem_total - smem_op - 1024) / ((size_t)3 * (PV * geo.NE + 4) * sizeof(T)));
+    return false;
+  }
+  panel_op_free(p);
+  p.M = M;
+  p.K = K;
+  p.WR = WR;
+  p.WC = geo.WC;
+  p.NIT = NIT;
+  p.CX = geo.CX;
+  p.NE = geo.NE;
+  p.KC = kcmax;
+  p.nchunks = nchunks;
+  p.NS = NS;
+  p.nblk = nblk;
+  p.sparse = sparse ? 1 : 0;
+  p.macs_per_col = (double)macs;
+  p.smem_op = smem_op;
+  auto up = [](auto *&dst, const auto &h) {
+    using E = typename std::remove_reference<decltype(h[0])>::type;
+    const size_t nb = std::max<size_t>(h.size(), 1) * sizeof(E);
+    FR_CUDA_TRY(cudaMalloc((void **)&dst, nb));
+    if (!h.empty()) FR_CUDA_TRY(cudaMemcpy((void *)dst, h.data(), h.size() * sizeof(E), cudaMemcpyHostToDevice));
+  };
+  up(p.vals, vals);
+  up(p.idx, idx);
+  up(p.off, off);
+  up(p.rowmap, rowmap);
+  up(p.chunks, chunks);
+  return true;
+}
+
+// ------------------------------------------------------------------------------------------------ device side
+#ifdef __CUDACC__
+
+__device__ __forceinline__ void pcp_async16(void *smem, const void *gmem, int src_bytes) {
+  unsigned s = (unsigned)__cvta_generic_to_shared(smem);
+  asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;\n" ::"r"(s), "l"(gmem), "r"(src_bytes));
+}
+__device__ __forceinline__ void pcp_commit() { asm volatile("cp.async.commit_group;\n" ::); }
+template <int N>
+__device__ __forceinline__ void pcp_wait() {
+  asm volatile("cp.async.wait_group %0;\n" ::"n"(N));
+}
+
+__device__ __forceinline__ void dmma884(double &c0, double &c1, double a, double b) {
+  asm("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};\n"
+               : "+d"(c0), "+d"(c1)
+               : "d"(a), "d"(b));
+}
+
+// Shared-memory view of the packed operator.
+template <typename T>
+struct OpSmem {
+  const T *vals;
+  const uint32_t *idx;
+  const int *off;
+  const int *rowmap;
+  const ChunkDesc *chunks;
+};
+
+template <typename T>
+__device__ __forceinline__ char *op_smem_carve(char *base, const PanelOp<T> &op, OpSmem<T> &v) {
+  auto al = [](size_t n) { return (n + 15) / 16 * 16; };
+  const size_t nv = (size_t)(op.nblk + 2) * (sizeof(T) == 8 ? 32 : 8) * sizeof(T);
+  v.vals = reinterpret_cast<const T *>(base);
+  base += al(nv);
+  v.idx = reinterpret_cast<const uint32_t *>(base);
+  base += al((size_t)(op.nblk + 2) * (sizeof(T) == 8 ? 16 : 4));
+  v.off = reinterpret_cast<const int *>(base);
+  base += al(((size_t)op.nchunks * op.NS + 1) * 4);
+  v.rowmap = reinterpret_cast<const int *>(base);
+  base += al((size_t)op.NS * 8 * 4);
+  v.chunks = reinterpret_cast<const ChunkDesc *>(base);
+  base += al((size_t)op.nchunks * sizeof(ChunkDesc));
+  return base;
+}
+
+// Copy the operator image global -> shared with cp.async (all threads), one commit group.
+template <typename T>
+__device__ __forceinline__ void op_smem_load(char *base, const PanelOp<T> &op, int tid, int nthreads) {
+  auto al = [](size_t n) { return (n + 15) / 16 * 16; };
+  auto copy = [&](char *dst, const void *src, size_t nbytes) {
+    const int np = (int)(al(nbytes) / 16);
+    for (int p = tid; p < np; p += nthreads) {
+      const int rem = (int)nbytes - 16 * p;
+      pcp_async16(dst + 16 * p, reinterpret_cast<const char *>(src) + 16 * p, rem >= 16 ? 16 : rem);
+    }
+    return dst + al(nbytes);
+  };
+  char *b = base;
+  b = copy(b, op.vals, (size_t)(op.nblk + 2) * (sizeof(T) == 8 ? 32 : 8) * sizeof(T));
+  b = copy(b, op.idx, (size_t)(op.nblk + 2) * (sizeof(T) == 8 ? 16 : 4));
+  b = copy(b, op.off, ((size_t)op.nchunks * op.NS + 1) * 4);
+  b = copy(b, op.rowmap, (size_t)op.NS * 8 * 4);
+  b = copy(b, op.chunks, (size_t)op.nchunks * sizeof(ChunkDesc));
+}
+
+// ---- accumulators and the multiply-accumulate core.  Panel columns in shared memory: c = v*NE + e, row pitch LDB.
+template <typename T, int NIT, int CX>
+struct Acc;
+
+// FP64: per slot, CX column blocks of 8 elements x 5 variables, one m8n8k4 C fragment (2 doubles) each.
+template <int NIT, int CX>
+struct Acc<double, NIT, CX> {
+  double c[NIT][CX][PV][2];
+  __device__ __forceinline__ void zero() {
+#pragma unroll
+    for (int i = 0; i < NIT; ++i)
+#pragma unroll
+      for (int b = 0; b < CX; ++b)
+#pragma unroll
+        for (int v = 0; v < PV; ++v) c[i][b][v][0] = c[i][b][v][1] = 0.0;
+  }
+  // elements of the panel this warp-column owns: [wc*8*CX, (wc+1)*8*CX)
+  __device__ __forceinline__ void mac_chunk(const OpSmem<double> &A, int chunk, int NS, int slot0, const double *Bst, int LDB,
+                                            int NE, int wc, int lane) {
+    // 32-bit byte-offset arithmetic inside the shared window.  The warp's blocks of this chunk are contiguous across
+    // its NIT slots, so one software pipeline runs through all of them: operator value and row offset are fetched two
+    // blocks ahead, the B fragments one block ahead of the DMMAs that consume them.
+    const char *bcol = reinterpret_cast<const char *>(Bst + wc * 8 * CX + (lane >> 2));
+    const char *av = reinterpret_cast<const char *>(A.vals) + lane * 8;
+    const char *ai = reinterpret_cast<const char *>(A.idx) + (lane & 3) * 4;
+    const uint32_t vs = (uint32_t)NE * 8u;
+    const int *offp = A.off + chunk * NS + slot0;
+    int b = offp[0];
+    double a0 = *reinterpret_cast<const double *>(av + (uint32_t)b * 256u);
+    double a1 = *reinterpret_cast<const double *>(av + (uint32_t)b * 256u + 256u);
+    uint32_t ro1 = *reinterpret_cast<const uint32_t *>(ai + (uint32_t)b * 16u + 16u);
+    double bf0[PV][CX];
+    {
+      const char *bp = bcol + *reinterpret_cast<const uint32_t *>(ai + (uint32_t)b * 16u);
+#pragma unroll
+      for (int v = 0; v < PV; ++v) {
+#pragma unroll
+        for (int cb = 0; cb < CX; ++cb) bf0[v][cb] = *reinterpret_cast<const double *>(bp + cb * 64);
+        bp += vs;
+      }
+    }
+#pragma unroll
+    for (int i = 0; i < NIT; ++i) {
+      const int bend = offp[i + 1];
+#pragma unroll 2
+      for (; b < bend; ++b) {
+        double bf1[PV][CX];
+        const char *bp = bcol + ro1;
+#pragma unroll
+        for (int v = 0; v < PV; ++v) {
+#pragma unroll
+          for (int cb = 0; cb < CX; ++cb) bf1[v][cb] = *reinterpret_cast<const double *>(bp + cb * 64);
+          bp += vs;
+        }
+        const double a2 = *reinterpret_cast<const double *>(av + (uint32_t)b * 256u + 512u);
+        const uint32_t ro2 = *reinterpret_cast<const uint32_t *>(ai + (uint32_t)b * 16u + 32u);
+#pragma unroll
+        for (int v = 0; v < PV; ++v)
+#pragma unroll
+          for (int cb = 0; cb < CX; ++cb) dmma884(c[i][cb][v][0], c[i][cb][v][1], a0, bf0[v][cb]);
+        a0 = a1;
+        a1 = a2;
+        ro1 = ro2;
+#pragma unroll
+        for (int v = 0; v < PV; ++v)
+#pragma unroll
+          for (int cb = 0; cb < CX; ++cb) bf0[v][cb] = bf1[v][cb];
+      }
+    }
+  }
+  // f(i, r, v, e, value&): slot i, row-in-group r, variable v, element-in-panel e (two consecutive e per call site)
+  template <typename F>
+  __device__ __forceinline__ void foreach2(int wc, int lane, F &&f) {
+#pragma unroll
+    for (int i = 0; i < NIT; ++i)
+#pragma unroll
+      for (int cb = 0; cb < CX; ++cb)
+#pragma unroll
+        for (int v = 0; v < PV; ++v) f(i, 0, v, wc * 8 * CX + cb * 8 + 2 * (lane & 3), c[i][cb][v]);
+  }
+  // g(i, rr, r): thread-local row index rr of slot i is row r of the 8-row group
+  template <typename G>
+  __device__ __forceinline__ void foreach_row(int lane, G &&g) {
+#pragma unroll
+    for (int i = 0; i < NIT; ++i) g(i, 0, lane >> 2);
+  }
+  static constexpr int EW = 2;   // consecutive elements per foreach2 call
+  static constexpr int ROWS = 1; // rows per thread per slot
+  static constexpr int NSLOT = NIT;
+};
+
+// FP32: per slot, 8 rows x 5 variables x CX elements per lane.
+template <int NIT, int CX>
+struct Acc<float, NIT, CX> {
+  float c[NIT][8][PV][CX];
+  __device__ __forceinline__ void zero() {
+#pragma unroll
+    for (int i = 0; i < NIT; ++i)
+#pragma unroll
+      for (int r = 0; r < 8; ++r)
+#pragma unroll
+        for (int v = 0; v < PV; ++v)
+#pragma unroll
+          for (int j = 0; j < CX; ++j) c[i][r][v][j] = 0.f;
+  }
+  __device__ __forceinline__ void mac_chunk(const OpSmem<float> &A, int chunk, int NS, int slot0, const float *Bst, int LDB,
+                                            int NE, int wc, int lane) {
+    const char *bcol = reinterpret_cast<const char *>(Bst + wc * 32 * CX + lane * CX);
+    const char *avp = reinterpret_cast<const char *>(A.vals);
+    const uint32_t vs = (uint32_t)NE * 4u;
+#pragma unroll
+    for (int i = 0; i < NIT; ++i) {
+      const int b0 = A.off[chunk * NS + slot0 + i], b1 = A.off[chunk * NS + slot0 + i + 1];
+#pragma unroll 2
+      for (int b = b0; b < b1; ++b) {
+        const float4 a0 = *reinterpret_cast<const float4 *>(avp + (uint32_t)b * 32u);
+        const float4 a1 = *reinterpret_cast<const float4 *>(avp + (uint32_t)b * 32u + 16u);
+        const float av[8] = {a0.x, a0.y, a0.z, a0.w, a1.x, a1.y, a1.z, a1.w};
+        const char *bp = bcol + A.idx[b];
+        float bv[PV][CX];
+#pragma unroll
+        for (int v = 0; v < PV; ++v) {
+          if (CX == 2) {
+            const float2 t = *reinterpret_cast<const float2 *>(bp);
+            bv[v][0] = t.x;
+            bv[v][CX - 1] = t.y;
+          } else {
+            bv[v][0] = *reinterpret_cast<const float *>(bp);
+          }
+          bp += vs;
+        }
+#pragma unroll
+        for (int r = 0; r < 8; ++r)
+#pragma unroll
+          for (int v = 0; v < PV; ++v)
+#pragma unroll
+            for (int j = 0; j < CX; ++j) c[i][r][v][j] = fmaf(av[r], bv[v][j], c[i][r][v][j]);
+      }
+    }
+  }
+  template <typename F>
+  __device__ __forceinline__ void foreach2(int wc, int lane, F &&f) {
+#pragma unroll
+    for (int i = 0; i < NIT; ++i)
+#pragma unroll
+      for (int r = 0; r < 8; ++r)
+#pragma unroll
+        for (int v = 0; v < PV; ++v) f(i, r, v, wc * 32 * CX + lane * CX, c[i][r][v]);
+  }
+  template <typename G>
+  __device__ __forceinline__ void foreach_row(int lane, G &&g) {
+#pragma unroll
+    for (int i = 0; i < NIT; ++i)
+#pragma unroll
+      for (int r = 0; r < 8; ++r) g(i, r, r);
+  }
+  static constexpr int EW = CX;
+  static constexpr int ROWS = 8;
+  static constexpr int NSLOT = NIT;
+};
+
+#endif  // __CUDACC__
+
+}  // namespace frb

@@ -1,0 +1,191 @@
+// The persistent panel main loop shared by the plain operator product and its fused variants (see panel.cuh).
+#pragma once
+#include "panel.cuh"
+
+namespace frb {
+
+constexpr int PANEL_NSTAGE = 3;
+
+// Where a panel's columns live in a global matrix: column(v, e) = p*pstride + v*vstride + e, valid iff
+// p*pstride + v*vlim + e < lim.  State matrices [rows][5][ld]: pstride = NE, vstride = ld, vlim = 0, lim = ld.
+// Plain matrices [rows][N] (fr_gemm): pstride = 5*NE, vstride = vlim = NE, lim = N.
+struct ColMap {
+  long long pstride, vstride, vlim, lim;
+};
+
+template <typename T>
+struct MatRef {
+  const T *p;
+  long long ld, bstride;   // row stride, batch stride (elements)
+};
+
+// ---- producer: B chunks are plain rows of up to two stacked global matrices
+template <typename T>
+struct PlainProducer {
+  MatRef<T> src[2];
+  ColMap cm;
+  static constexpr bool kTransform = false;
+  __device__ __forceinline__ size_t stage_elems(int KC, int LDB) const { return (size_t)KC * LDB; }
+  __device__ __forceinline__ void issue(const ChunkDesc &cd, long long batch, long long pl, T *stage, int LDB, int NE, int tid,
+                                        int nthreads) const {
+    // Each thread owns one fixed 16-byte column piece (variable v, elements e..e+CTV) and walks down the rows, so the
+    // per-piece cost is two pointer bumps and the copy; the (v, e, first row) split of the thread index is done once per
+    // call with shifts (pieces per variable segment is a power of two).
+    constexpr int CTV = 16 / (int)sizeof(T);
+    const int lg = 31 - __clz(NE / CTV);
+    const int ppr = PV << lg;                         // pieces per row
+    const bool wide = nthreads >= ppr;                // the usual case: one sweep of the CTA covers >= 1 whole row
+    const int rpi = wide ? nthreads / ppr : 1;        // rows per sweep
+    const int sub = wide ? tid / ppr : 0;
+    if (sub >= rpi) return;
+    const T *mp = cd.src ? src[1].p : src[0].p;
+    const long long mld = cd.src ? src[1].ld : src[0].ld, mbs = cd.src ? src[1].bstride : src[0].bstride;
+    for (int col = tid - sub * ppr; col < ppr; col += wide ? ppr : nthreads) {
+      const int v = col >> lg, e = (col - (v << lg)) * CTV;
+      long long nv = cm.lim - pl * cm.pstride - v * cm.vlim - e;
+      nv = nv < 0 ? 0 : (nv > CTV ? CTV : nv);
+      const int nbytes = (int)nv * (int)sizeof(T);
+      const T *g = mp;
+      long long gstep = 0;
+      if (nv > 0) {
+        g = mp + batch * mbs + (long long)(cd.row0 + sub) * mld + pl * cm.pstride + v * cm.vstride + e;
+        gstep = (long long)rpi * mld;
+      }
+      T *sp = stage + sub * LDB + v * NE + e;
+      const int sstep = rpi * LDB;
+      for (int r = sub; r < cd.nrows; r += rpi) {
+        pcp_async16(sp, g, nbytes);
+        g += gstep;
+        sp += sstep;
+      }
+    }
+  }
+  __device__ __forceinline__ void transform(const ChunkDesc &, long long, long long, T *, int, int, int, int) const {}
+  __device__ __forceinline__ const T *bstage(const T *stage) const { return stage; }
+};
+
+// ---- epilogue: C <- c1*acc + c2*C
+template <typename T>
+struct PlainEpilogue {
+  T *C;
+  long long ldc, bstride;
+  ColMap cm;
+  T c1, c2;
+  template <typename ACC>
+  __device__ __forceinline__ void operator()(ACC &acc, const int *rowmap, int slot0, long long batch, long long pl, int wc,
+                                             int lane) const {
+    T *Cb = C + batch * bstride + pl * cm.pstride;
+    const long long vb = pl * cm.pstride;
+    constexpr int EW = ACC::EW;
+    const bool interior = vb + (PV - 1) * cm.vlim + (cm.pstride > cm.vstride ? cm.vstride : cm.pstride) <= cm.lim;
+    int mrow[ACC::NSLOT][ACC::ROWS];
+    acc.foreach_row(lane, [&](int i, int rr, int r) { mrow[i][rr] = rowmap[(slot0 + i) * 8 + r]; });
+    acc.foreach2(wc, lane, [&](int i, int rr, int v, int e, T *val) {
+      const int m = mrow[i][rr];
+      if (m < 0) return;
+      T *cp = Cb + (long long)m * ldc + v * cm.vstride + e;
+      const long long room = interior ? EW : cm.lim - (vb + v * cm.vlim + e);
+      if (room >= EW) {
+        T out[EW];
+        if (c2 != T(0)) {
+#pragma unroll
+          for (int j = 0; j < EW; ++j) out[j] = fma(c1, val[j], c2 * cp[j]);
+        } else {
+#pragma unroll
+          for (int j = 0; j < EW; ++j) out[j] = c1 * val[j];
+        }
+        if (EW == 2 && sizeof(T) == 8) *reinterpret_cast<double2 *>(cp) = *reinterpret_cast<double2 *>(out);
+        else if (EW == 2) *reinterpret_cast<float2 *>(cp) = *reinterpret_cast<float2 *>(out);
+        else cp[0] = out[0];
+      } else {
+#pragma unroll
+        for (int j = 0; j < EW; ++j)
+          if (j < room) cp[j] = (c2 != T(0)) ? fma(c1, val[j], c2 * cp[j]) : c1 * val[j];
+      }
+    });
+  }
+};
+
+// ---- the persistent main loop.  Grid = any number of CTAs; CTA b owns panels b, b+grid, ...
+template <typename T, int NIT, int CX, class Prod, class Epi>
+__device__ __forceinline__ void panel_mainloop(const PanelOp<T> &op, const Prod &prod, const Epi &epi, long long npanels_per_batch,
+                                               int nbatch, char *smem) {
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const int nthreads = blockDim.x;
+  const int WC = op.WC, NS = op.NS, NE = op.NE;
+  const int wr = warp / WC, wc = warp - wr * WC;
+  const int LDB = PV * NE + 4;
+  OpSmem<T> A;
+  char *ringp = op_smem_carve(smem, op, A);
+  op_smem_load(smem, op, tid, nthreads);
+  pcp_commit();
+  T *ring = reinterpret_cast<T *>(ringp);
+  const size_t stage_elems = prod.stage_elems(op.KC, LDB);
+  const long long ntot = npanels_per_batch * nbatch;
+  const long long first = blockIdx.x, stride = gridDim.x;
+  const long long mine = first < ntot ? (ntot - first + stride - 1) / stride : 0;
+  const int nchunks = op.nchunks;
+  const long long total = mine * nchunks;
+  // two cursors over (panel, chunk): `iq` for the loads being issued, `cq` for the chunk being multiplied
+  long long ipanel = first, cpanel = first;
+  int ic = 0, cc = 0, istage = 0, cstage = 0;
+  long long ibatch = ipanel / npanels_per_batch, ipl = ipanel - ibatch * npanels_per_batch;
+  long long cbatch = ibatch, cpl = ipl;
+  auto issue = [&]() {
+    const ChunkDesc cd = op.chunks[ic];              // global copy (the shared image may still be in flight)
+    prod.issue(cd, ibatch, ipl, ring + istage * stage_elems, LDB, NE, tid, nthreads);
+    if (++istage == PANEL_NSTAGE) istage = 0;
+    if (++ic == nchunks) {
+      ic = 0;
+      ipanel += stride;
+      ipl += stride;
+      while (ipl >= npanels_per_batch) {
+        ipl -= npanels_per_batch;
+        ++ibatch;
+      }
+    }
+  };
+  for (int q = 0; q < PANEL_NSTAGE - 1; ++q) {
+    if (q < total) issue();
+    pcp_commit();
+  }
+  Acc<T, NIT, CX> acc;
+  acc.zero();
+  for (long long q = 0; q < total; ++q) {
+    pcp_wait<PANEL_NSTAGE - 2>();
+    __syncthreads();
+    if (q + PANEL_NSTAGE - 1 < total) issue();
+    pcp_commit();
+    T *stage = ring + cstage * stage_elems;
+    if (Prod::kTransform) {
+      prod.transform(A.chunks[cc], cbatch, cpl, stage, LDB, NE, tid, nthreads);
+      __syncthreads();
+    }
+    acc.mac_chunk(A, cc, NS, wr * NIT, prod.bstage(stage), LDB, NE, wc, lane);
+    if (++cstage == PANEL_NSTAGE) cstage = 0;
+    if (++cc == nchunks) {
+      epi(acc, A.rowmap, wr * NIT, cbatch, cpl, wc, lane);
+      acc.zero();
+      cc = 0;
+      cpanel += stride;
+      cpl += stride;
+      while (cpl >= npanels_per_batch) {
+        cpl -= npanels_per_batch;
+        ++cbatch;
+      }
+    }
+  }
+  pcp_wait<0>();
+}
+
+// Dispatch over the compile-time accumulator shapes.  FP64: NIT*CX <= 8; FP32: NIT*CX <= 4.
+#define FR_PANEL_SHAPES_F64(X) \
+  X(1, 1) X(2, 1) X(3, 1) X(4, 1) X(5, 1) X(6, 1) X(7, 1) X(8, 1) X(1, 2) X(2, 2) X(3, 2) X(4, 2)
+#define FR_PANEL_SHAPES_F32(X) X(1, 1) X(2, 1) X(3, 1) X(4, 1) X(1, 2) X(2, 2)
+
+template <typename T>
+inline size_t panel_smem_bytes(const PanelOp<T> &op, size_t stage_elems) {
+  return op.smem_op + PANEL_NSTAGE * stage_elems * sizeof(T) + 16;
+}
+
+}  // namespace frb
