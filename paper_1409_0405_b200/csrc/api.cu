@@ -75,6 +75,7 @@ struct EleData {
   EleView<T> view;
   DevBuf<T> smats, rcpdjac;
   GemmPlan<T> pM0, pM132, pM3, pM460, pM6;
+  PanelOp<T> pDiv, pGrad;   // fused operators [M132 | M3] and [M460 | M6] (FR_MODE_FUSED)
   DevBuf<T> X, Y, ACC;   // solution register, stage input, RK4 accumulator
   DevBuf<T> grad;        // [3][nupts][5][ld]: G~ -> G -> F~
   DevBuf<T> R;           // [nupts][5][ld]
@@ -84,6 +85,8 @@ struct EleData {
     gemm_plan_free(pM3);
     gemm_plan_free(pM460);
     gemm_plan_free(pM6);
+    panel_op_free(pDiv);
+    panel_op_free(pGrad);
   }
 };
 
@@ -169,7 +172,7 @@ struct Ctx : CtxBase {
       v.nfpts = nf;
       v.affine = d.affine ? 1 : 0;
       v.neles = d.neles;
-      v.ld = (d.neles + 31) / 32 * 32;
+      v.ld = (d.neles + 63) / 64 * 64;   // whole panels of up to 64 elements (panel.cuh); 512-byte rows
       const long long ld = v.ld, ne = d.neles;
       // metric terms, padded with the identity so padding lanes stay finite
       const long long npt = v.affine ? 1 : nu;
@@ -198,6 +201,10 @@ struct Ctx : CtxBase {
       if (ns) {
         gemm_plan_build(e->pM460, 3 * nu, nu, d.M460);
         gemm_plan_build(e->pM6, 3 * nu, nf, d.M6);
+      }
+      if (mode == FR_MODE_FUSED) {
+        fused_div_build(e->pDiv, nu, nf, d.M132, d.M3, v.affine ? 0 : 1);
+        if (ns) fused_grad_build(e->pGrad, nu, nf, d.M460, d.M6);
       }
       const size_t nstate = (size_t)nu * 5 * ld;
       e->X.alloc(nstate);
@@ -347,13 +354,20 @@ struct Ctx : CtxBase {
         const long long n5 = 5 * e.view.ld;
         const double n = (double)e.view.neles, nu = e.view.nupts, nf = e.view.nfpts;
         const double nmet = e.view.affine ? 1 : nu;
-        // S3: G~ = M460 U + M6 C
-        nk += gemm_run(e.pM460, n5, T(1), u[t], n5, 0, T(0), e.grad.p, n5, 0, 1, s);
-        mark(CAT_GEMM, t, "S3a_M460", (nu + 3 * nu) * 5 * n, 2 * 3 * nu * nu * 5 * n);
-        nk += gemm_run(e.pM6, n5, T(1), cf.p + tt.ubase[t], n5, 0, T(1), e.grad.p, n5, 0, 1, s);
-        mark(CAT_GEMM, t, "S3b_M6", (nf + 6 * nu) * 5 * n, 2 * 3 * nu * nf * 5 * n);
-        nk += launch_gradcoru(e.view, e.grad.p, s);   // S4
-        mark(CAT_PW, t, "S4_gradcoru", (30 * nu + 10 * nmet) * n, 15 * 6 * nu * n);
+        if (e.pGrad.ok()) {
+          // S3 + S4 fused: G = (1/|J|) S^T ([M460 | M6] [U; C])
+          nk += launch_fused_grad(e.pGrad, e.view, u[t], cf.p + tt.ubase[t], e.grad.p, s);
+          mark(CAT_GEMM, t, "S3_S4_fused_grad", (5 * nu + 5 * nf + 15 * nu + 10 * nmet) * n,
+               2 * 3 * nu * (nu + nf) * 5 * n + 15 * 6 * nu * n);
+        } else {
+          // S3: G~ = M460 U + M6 C
+          nk += gemm_run(e.pM460, n5, T(1), u[t], n5, 0, T(0), e.grad.p, n5, 0, 1, s);
+          mark(CAT_GEMM, t, "S3a_M460", (nu + 3 * nu) * 5 * n, 2 * 3 * nu * nu * 5 * n);
+          nk += gemm_run(e.pM6, n5, T(1), cf.p + tt.ubase[t], n5, 0, T(1), e.grad.p, n5, 0, 1, s);
+          mark(CAT_GEMM, t, "S3b_M6", (nf + 6 * nu) * 5 * n, 2 * 3 * nu * nf * 5 * n);
+          nk += launch_gradcoru(e.view, e.grad.p, s);   // S4
+          mark(CAT_PW, t, "S4_gradcoru", (30 * nu + 10 * nmet) * n, 15 * 6 * nu * n);
+        }
         // S5: G_f,i = M0 G_i, i = 0..2 (batched)
         nk += gemm_run(e.pM0, n5, T(1), e.grad.p, n5, (long long)e.view.nupts * n5, T(0), gf.p + tt.gbase[t], n5,
                        tt.gcomp[t], 3, s);
@@ -372,6 +386,15 @@ struct Ctx : CtxBase {
       const long long n5 = 5 * e.view.ld;
       const double n = (double)e.view.neles, nu = e.view.nupts, nf = e.view.nfpts;
       const double nmet = e.view.affine ? 1 : nu;
+      if (e.pDiv.ok()) {
+        // S6 + S8 + S9 (+S10) fused: out = -(1/|J|) [M132 | M3] [F~(U, G); D], stage update in the epilogue
+        nk += launch_fused_div(e.pDiv, e.view, u[t], e.grad.p, uf.p + tt.ubase[t], ph, sa[t], s);
+        const double rk = sa[t].coef ? (sa[t].out2 ? 15 : 10) : 5;
+        mark(CAT_GEMM, t, sa[t].coef ? "S6_S8_S9_S10_fused_div_rk" : "S6_S8_S9_fused_div",
+             ((ns ? 20 : 5) * nu + 5 * nf + rk * nu + 10 * nmet) * n,
+             2 * nu * (3 * nu + nf) * 5 * n + (ns ? 210 : 110) * nu * n + 5 * nu * n);
+        continue;
+      }
       nk += launch_tdisf(e.view, u[t], e.grad.p, ph, s);   // S6
       mark(CAT_PW, t, "S6_tdisf", ((ns ? 35 : 20) * nu + 9 * nmet) * n, (ns ? 210 : 110) * nu * n);
       // S8: R = M132 F~ + M3 D

@@ -42,6 +42,8 @@ struct PanelOp {
   int WR = 0, WC = 0, NIT = 0, CX = 0;   // warp grid, row groups per row-warp, column blocks (FP64) / elements per lane (FP32)
   int NE = 0;                            // elements per panel
   int KC = 0, nchunks = 0, NS = 0;       // rows per chunk (max), chunks, slots = WR*NIT
+  int stage_elems = 0;                   // elements of one ring stage
+  int curved = 0;                        // flux chunks: metric terms per point (1) or per element (0)
   int nblk = 0;                          // packed blocks (FP64: 8x4 tiles; FP32: 8x1 columns)
   int sparse = 0;
   double macs_per_col = 0;               // executed multiply-adds per column (dense: M*K)
@@ -65,22 +67,34 @@ void panel_op_free(PanelOp<T> &p) {
 }
 
 // How the K dimension of the operator is fed: a list of sources stacked along K, each cut into chunks of at most KC rows.
+// kind 0: `rows` plain rows of a global matrix <-> `rows` columns of A.
+// kind 1: transformed flux at `rows` solution points <-> 3*rows columns of A (alpha-major: column alpha*rows + nu); a chunk
+//         of n points occupies stage rows [0,3n) (alpha-major within the chunk: row alpha*n + j) for G -> F~, rows [3n,4n)
+//         for U, followed by the metric terms (flux_stage_elems).
 struct KSource {
-  int rows;      // rows of this source (columns of A it multiplies)
-  int kind;      // producer-specific tag (0 = plain rows of a matrix)
-  int unit;      // chunk granularity: chunk rows are a multiple of `unit` (e.g. 3 for (alpha, nu) triples)
+  int rows;
+  int kind;
+  int unit;      // unused (kept for aggregate initialisation)
 };
+constexpr int KIND_PLAIN = 0, KIND_FLUX = 1;
+
+// shared-memory elements of one stage holding a flux chunk of n points
+inline __host__ __device__ size_t flux_stage_elems(int n, int NE, int LDB, int curved) {
+  return (size_t)4 * n * LDB + (size_t)9 * (curved ? n : 1) * NE;
+}
 
 struct PanelGeom {
   int WR, WC, NIT, CX, NE;
   double eff;
 };
 
-// Accumulator budget: a CTA of up to 16 warps (128 registers per thread) if NIT*CX <= small, else up to 8 warps.
+// Warps per CTA a given accumulator shape allows: registers per thread ~ accumulators + 70 must fit the 64K register file.
 // FP64: NIT*CX*10 doubles per thread; FP32: NIT*CX*40 floats.
 template <typename T>
 constexpr int panel_maxw(int nit, int cx) {
-  return sizeof(T) == 8 ? (nit * cx <= 4 ? 16 : 8) : (nit * cx <= 2 ? 16 : 8);
+  const int acc_regs = sizeof(T) == 8 ? nit * cx * 20 : nit * cx * 40;
+  const int w = 2048 / (acc_regs + 70);
+  return w > 16 ? 16 : (w < 1 ? 1 : w);
 }
 
 // Choose the warp grid for G row groups.  The FP64 tensor pipe takes one DMMA per warp every ~32 cycles, so two warps per
@@ -158,6 +172,7 @@ struct PackOptions {
   int triple = 0;          // rows come as (alpha, rho) with alpha-major blocks of M/3: keep the three alpha of a rho in one thread
   int kc = 0;              // rows per chunk (0 = default)
   int allow_sparse = 1;
+  int curved = 0;          // flux sources: per-point metric terms
 };
 
 // Pack A (M x K, host FP64, row-major) for the panel kernels.  `srcs` stacks the K dimension.  Returns false if the
@@ -186,7 +201,7 @@ bool panel_op_build_kc(PanelOp<T> &p, int M, int K, const double *A, const std::
                        size_t smem_budget, size_t smem_total, int kc_try, int *kc_fit) {
   const bool f64 = sizeof(T) == 8;
   int ktot = 0;
-  for (auto &s : srcs) ktot += s.rows;
+  for (auto &s : srcs) ktot += s.kind == KIND_FLUX ? 3 * s.rows : s.rows;
   FR_REQUIRE(ktot == K, "panel_op_build: sources do not add up to K");
   double amax = 0;
   for (size_t i = 0; i < (size_t)M * K; ++i) {
@@ -238,39 +253,56 @@ bool panel_op_build_kc(PanelOp<T> &p, int M, int K, const double *A, const std::
   // ---- chunks
   const int KC = kc_try;
   std::vector<ChunkDesc> chunks;
-  std::vector<int> chunk_k0;   // first column of A of each chunk
+  std::vector<std::vector<int>> chunk_cols;   // column of A behind each MAC row of the chunk's stage
   {
     int k0 = 0, si = 0;
     for (auto &s : srcs) {
-      // equal chunks of at most KC rows, a multiple of lcm(unit, 4) so that dense k-lists need no padding
-      const int unit = std::max(1, s.unit);
-      const int q = unit % 4 == 0 ? unit : (unit % 2 == 0 ? 2 * unit : 4 * unit);
-      const int nch = std::max(1, (s.rows + KC - 1) / KC);
-      int step = ((s.rows + nch - 1) / nch + q - 1) / q * q;
-      if (step > KC) step = std::max(q, KC / q * q);
-      for (int r = 0; r < s.rows; r += step) {
-        chunks.push_back(ChunkDesc{si, r, std::min(step, s.rows - r), s.kind});
-        chunk_k0.push_back(k0 + r);
+      if (s.kind == KIND_PLAIN) {
+        // equal chunks of at most KC rows, a multiple of 4 so that dense k-lists need no padding
+        const int nch = std::max(1, (s.rows + KC - 1) / KC);
+        int step = ((s.rows + nch - 1) / nch + 3) / 4 * 4;
+        if (step > KC) step = std::max(4, KC / 4 * 4);
+        for (int r = 0; r < s.rows; r += step) {
+          const int n = std::min(step, s.rows - r);
+          chunks.push_back(ChunkDesc{si, r, n, s.kind});
+          std::vector<int> cols(n);
+          for (int j = 0; j < n; ++j) cols[j] = k0 + r + j;
+          chunk_cols.push_back(cols);
+        }
+        k0 += s.rows;
+      } else {
+        const int nlim = std::max(1, KC / 3);
+        const int nch = std::max(1, (s.rows + nlim - 1) / nlim);
+        int step = (s.rows + nch - 1) / nch;
+        if ((step + 3) / 4 * 4 <= nlim) step = (step + 3) / 4 * 4;
+        for (int r = 0; r < s.rows; r += step) {
+          const int n = std::min(step, s.rows - r);
+          chunks.push_back(ChunkDesc{si, r, n, s.kind});
+          std::vector<int> cols(3 * n);
+          for (int a = 0; a < 3; ++a)
+            for (int j = 0; j < n; ++j) cols[a * n + j] = k0 + a * s.rows + r + j;
+          chunk_cols.push_back(cols);
+        }
+        k0 += 3 * s.rows;
       }
-      k0 += s.rows;
       ++si;
     }
   }
   const int nchunks = (int)chunks.size();
   if (nchunks > PANEL_MAXCHUNKS) return false;
   int kcmax = 0;
-  for (auto &c : chunks) kcmax = std::max(kcmax, c.nrows);
-  if (kcmax > 255) return false;
+  for (auto &c : chunk_cols) kcmax = std::max(kcmax, (int)c.size());
+  if (kcmax > 8000) return false;
   // ---- cost of each group (number of listed k) and its assignment to row-warps
   std::vector<std::vector<std::vector<int>>> lists(G, std::vector<std::vector<int>>(nchunks));
   std::vector<long long> gcost(G, 0);
   for (int g = 0; g < G; ++g)
     for (int c = 0; c < nchunks; ++c) {
-      for (int kk = 0; kk < chunks[c].nrows; ++kk) {
+      for (int kk = 0; kk < (int)chunk_cols[c].size(); ++kk) {
         bool any = !sparse;
         for (int r = 0; r < 8 && !any; ++r) {
           const int m = order[8 * g + r];
-          if (m >= 0 && sup[m][chunk_k0[c] + kk]) any = true;
+          if (m >= 0 && sup[m][chunk_cols[c][kk]]) any = true;
         }
         if (any) lists[g][c].push_back(kk);
       }
@@ -330,7 +362,7 @@ bool panel_op_build_kc(PanelOp<T> &p, int M, int K, const double *A, const std::
             const int r = lane >> 2, j = lane & 3;
             const int m = order[8 * g + r];
             double v = 0;
-            if (m >= 0 && 4 * b + j < n) v = A[(size_t)m * K + chunk_k0[c] + L[4 * b + j]];
+            if (m >= 0 && 4 * b + j < n) v = A[(size_t)m * K + chunk_cols[c][L[4 * b + j]]];
             if (sparse && std::fabs(v) <= thr) v = 0;
             vals.push_back((T)v);
           }
@@ -342,7 +374,7 @@ bool panel_op_build_kc(PanelOp<T> &p, int M, int K, const double *A, const std::
           idx.push_back((uint32_t)L[b] * (uint32_t)(PV * geo.NE + 4) * (uint32_t)sizeof(T));
           for (int r = 0; r < 8; ++r) {
             const int m = order[8 * g + r];
-            double v = m >= 0 ? A[(size_t)m * K + chunk_k0[c] + L[b]] : 0.0;
+            double v = m >= 0 ? A[(size_t)m * K + chunk_cols[c][L[b]]] : 0.0;
             if (sparse && std::fabs(v) <= thr) v = 0;
             vals.push_back((T)v);
           }
@@ -361,8 +393,16 @@ bool panel_op_build_kc(PanelOp<T> &p, int M, int K, const double *A, const std::
                          ((off.size() * 4 + 15) / 16 * 16) + ((rowmap.size() * 4 + 15) / 16 * 16) +
                          ((chunks.size() * sizeof(ChunkDesc) + 15) / 16 * 16);
   if (smem_op > smem_budget) return false;
-  if (smem_op + (size_t)3 * kcmax * (PV * geo.NE + 4) * sizeof(T) + 16 > smem_total) {
-    if (smem_total > smem_op + 4096) *kc_fit = (int)((smem_total - smem_op - 1024) / ((size_t)3 * (PV * geo.NE + 4) * sizeof(T)));
+  size_t stage_elems = 0;
+  const int LDBh = PV * geo.NE + 4;
+  for (auto &c : chunks)
+    stage_elems = std::max(stage_elems, c.kind == KIND_FLUX ? flux_stage_elems(c.nrows, geo.NE, LDBh, opt.curved) : (size_t)c.nrows * LDBh);
+  if (smem_op + 3 * stage_elems * sizeof(T) + 16 > smem_total) {
+    // MAC rows per chunk that would fit: scale the tallest chunk down proportionally (flux chunks carry 4/3 rows + metrics)
+    if (smem_total > smem_op + 4096) {
+      const double room = (double)(smem_total - smem_op - 1024) / (3.0 * sizeof(T));
+      *kc_fit = (int)(kcmax * room / (double)stage_elems);
+    }
     return false;
   }
   panel_op_free(p);
@@ -374,6 +414,8 @@ bool panel_op_build_kc(PanelOp<T> &p, int M, int K, const double *A, const std::
   p.CX = geo.CX;
   p.NE = geo.NE;
   p.KC = kcmax;
+  p.stage_elems = (int)stage_elems;
+  p.curved = opt.curved;
   p.nchunks = nchunks;
   p.NS = NS;
   p.nblk = nblk;
@@ -530,15 +572,22 @@ struct Acc<double, NIT, CX> {
       }
     }
   }
-  // f(i, r, v, e, value&): slot i, row-in-group r, variable v, element-in-panel e (two consecutive e per call site)
+  // f(i, rr, e, tile[PV][EW]): slot i, thread-local row rr, first element e of EW consecutive ones, all 5 variables
   template <typename F>
-  __device__ __forceinline__ void foreach2(int wc, int lane, F &&f) {
+  __device__ __forceinline__ void foreach_tile(int wc, int lane, F &&f) {
 #pragma unroll
     for (int i = 0; i < NIT; ++i)
 #pragma unroll
-      for (int cb = 0; cb < CX; ++cb)
+      for (int cb = 0; cb < CX; ++cb) f(i, 0, wc * 8 * CX + cb * 8 + 2 * (lane & 3), c[i][cb]);
+  }
+  // f(t, rr, e, tile_a0, tile_a1, tile_a2): slots 3t, 3t+1, 3t+2 hold the three alpha of the same rows
+  template <typename F>
+  __device__ __forceinline__ void foreach_triple(int wc, int lane, F &&f) {
 #pragma unroll
-        for (int v = 0; v < PV; ++v) f(i, 0, v, wc * 8 * CX + cb * 8 + 2 * (lane & 3), c[i][cb][v]);
+    for (int t = 0; t < NIT / 3; ++t)
+#pragma unroll
+      for (int cb = 0; cb < CX; ++cb)
+        f(t, 0, wc * 8 * CX + cb * 8 + 2 * (lane & 3), c[3 * t][cb], c[3 * t + 1][cb], c[3 * t + 2][cb]);
   }
   // g(i, rr, r): thread-local row index rr of slot i is row r of the 8-row group
   template <typename G>
@@ -601,13 +650,18 @@ struct Acc<float, NIT, CX> {
     }
   }
   template <typename F>
-  __device__ __forceinline__ void foreach2(int wc, int lane, F &&f) {
+  __device__ __forceinline__ void foreach_tile(int wc, int lane, F &&f) {
 #pragma unroll
     for (int i = 0; i < NIT; ++i)
 #pragma unroll
-      for (int r = 0; r < 8; ++r)
+      for (int r = 0; r < 8; ++r) f(i, r, wc * 32 * CX + lane * CX, c[i][r]);
+  }
+  template <typename F>
+  __device__ __forceinline__ void foreach_triple(int wc, int lane, F &&f) {
 #pragma unroll
-        for (int v = 0; v < PV; ++v) f(i, r, v, wc * 32 * CX + lane * CX, c[i][r][v]);
+    for (int t = 0; t < NIT / 3; ++t)
+#pragma unroll
+      for (int r = 0; r < 8; ++r) f(t, r, wc * 32 * CX + lane * CX, c[3 * t][r], c[3 * t + 1][r], c[3 * t + 2][r]);
   }
   template <typename G>
   __device__ __forceinline__ void foreach_row(int lane, G &&g) {

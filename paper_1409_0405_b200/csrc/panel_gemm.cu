@@ -64,7 +64,7 @@ void panel_gemm_run(const PanelOp<T> &op, long long N, T c1, const T *B, long lo
   a.epi = PlainEpilogue<T>{C, ldc, bsC, cm, c1, c2};
   a.npanels = (N + pw - 1) / pw;
   a.nbatch = nbatch;
-  const size_t smem = panel_smem_bytes(op, (size_t)op.KC * (PV * op.NE + 4));
+  const size_t smem = panel_smem_bytes(op);
 #define FR_CASE(NIT_, CX_)                                     \
   if (op.NIT == NIT_ && op.CX == CX_) {                        \
     launch_shape<T, NIT_, CX_>(a, smem, s);                    \

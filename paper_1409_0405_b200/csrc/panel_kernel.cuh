@@ -25,7 +25,6 @@ struct PlainProducer {
   MatRef<T> src[2];
   ColMap cm;
   static constexpr bool kTransform = false;
-  __device__ __forceinline__ size_t stage_elems(int KC, int LDB) const { return (size_t)KC * LDB; }
   __device__ __forceinline__ void issue(const ChunkDesc &cd, long long batch, long long pl, T *stage, int LDB, int NE, int tid,
                                         int nthreads) const {
     // Each thread owns one fixed 16-byte column piece (variable v, elements e..e+CTV) and walks down the rows, so the
@@ -61,7 +60,6 @@ struct PlainProducer {
     }
   }
   __device__ __forceinline__ void transform(const ChunkDesc &, long long, long long, T *, int, int, int, int) const {}
-  __device__ __forceinline__ const T *bstage(const T *stage) const { return stage; }
 };
 
 // ---- epilogue: C <- c1*acc + c2*C
@@ -80,27 +78,31 @@ struct PlainEpilogue {
     const bool interior = vb + (PV - 1) * cm.vlim + (cm.pstride > cm.vstride ? cm.vstride : cm.pstride) <= cm.lim;
     int mrow[ACC::NSLOT][ACC::ROWS];
     acc.foreach_row(lane, [&](int i, int rr, int r) { mrow[i][rr] = rowmap[(slot0 + i) * 8 + r]; });
-    acc.foreach2(wc, lane, [&](int i, int rr, int v, int e, T *val) {
+    acc.foreach_tile(wc, lane, [&](int i, int rr, int e, T(&tile)[PV][EW]) {
       const int m = mrow[i][rr];
       if (m < 0) return;
-      T *cp = Cb + (long long)m * ldc + v * cm.vstride + e;
-      const long long room = interior ? EW : cm.lim - (vb + v * cm.vlim + e);
-      if (room >= EW) {
-        T out[EW];
-        if (c2 != T(0)) {
 #pragma unroll
-          for (int j = 0; j < EW; ++j) out[j] = fma(c1, val[j], c2 * cp[j]);
+      for (int v = 0; v < PV; ++v) {
+        T *val = tile[v];
+        T *cp = Cb + (long long)m * ldc + v * cm.vstride + e;
+        const long long room = interior ? EW : cm.lim - (vb + v * cm.vlim + e);
+        if (room >= EW) {
+          T out[EW];
+          if (c2 != T(0)) {
+#pragma unroll
+            for (int j = 0; j < EW; ++j) out[j] = fma(c1, val[j], c2 * cp[j]);
+          } else {
+#pragma unroll
+            for (int j = 0; j < EW; ++j) out[j] = c1 * val[j];
+          }
+          if (EW == 2 && sizeof(T) == 8) *reinterpret_cast<double2 *>(cp) = *reinterpret_cast<double2 *>(out);
+          else if (EW == 2) *reinterpret_cast<float2 *>(cp) = *reinterpret_cast<float2 *>(out);
+          else cp[0] = out[0];
         } else {
 #pragma unroll
-          for (int j = 0; j < EW; ++j) out[j] = c1 * val[j];
+          for (int j = 0; j < EW; ++j)
+            if (j < room) cp[j] = (c2 != T(0)) ? fma(c1, val[j], c2 * cp[j]) : c1 * val[j];
         }
-        if (EW == 2 && sizeof(T) == 8) *reinterpret_cast<double2 *>(cp) = *reinterpret_cast<double2 *>(out);
-        else if (EW == 2) *reinterpret_cast<float2 *>(cp) = *reinterpret_cast<float2 *>(out);
-        else cp[0] = out[0];
-      } else {
-#pragma unroll
-        for (int j = 0; j < EW; ++j)
-          if (j < room) cp[j] = (c2 != T(0)) ? fma(c1, val[j], c2 * cp[j]) : c1 * val[j];
       }
     });
   }
@@ -120,7 +122,7 @@ __device__ __forceinline__ void panel_mainloop(const PanelOp<T> &op, const Prod 
   op_smem_load(smem, op, tid, nthreads);
   pcp_commit();
   T *ring = reinterpret_cast<T *>(ringp);
-  const size_t stage_elems = prod.stage_elems(op.KC, LDB);
+  const size_t stage_elems = (size_t)op.stage_elems;
   const long long ntot = npanels_per_batch * nbatch;
   const long long first = blockIdx.x, stride = gridDim.x;
   const long long mine = first < ntot ? (ntot - first + stride - 1) / stride : 0;
@@ -158,10 +160,13 @@ __device__ __forceinline__ void panel_mainloop(const PanelOp<T> &op, const Prod 
     pcp_commit();
     T *stage = ring + cstage * stage_elems;
     if (Prod::kTransform) {
-      prod.transform(A.chunks[cc], cbatch, cpl, stage, LDB, NE, tid, nthreads);
-      __syncthreads();
+      const ChunkDesc cd = A.chunks[cc];
+      if (cd.kind != KIND_PLAIN) {                   // uniform over the CTA
+        prod.transform(cd, cbatch, cpl, stage, LDB, NE, tid, nthreads);
+        __syncthreads();
+      }
     }
-    acc.mac_chunk(A, cc, NS, wr * NIT, prod.bstage(stage), LDB, NE, wc, lane);
+    acc.mac_chunk(A, cc, NS, wr * NIT, stage, LDB, NE, wc, lane);
     if (++cstage == PANEL_NSTAGE) cstage = 0;
     if (++cc == nchunks) {
       epi(acc, A.rowmap, wr * NIT, cbatch, cpl, wc, lane);
@@ -182,10 +187,50 @@ __device__ __forceinline__ void panel_mainloop(const PanelOp<T> &op, const Prod 
 #define FR_PANEL_SHAPES_F64(X) \
   X(1, 1) X(2, 1) X(3, 1) X(4, 1) X(5, 1) X(6, 1) X(7, 1) X(8, 1) X(1, 2) X(2, 2) X(3, 2) X(4, 2)
 #define FR_PANEL_SHAPES_F32(X) X(1, 1) X(2, 1) X(3, 1) X(4, 1) X(1, 2) X(2, 2)
+// triple-packed operators (gradient): NIT a multiple of 3
+#define FR_PANEL_TRIPLES_F64(X) X(3, 1) X(6, 1) X(3, 2)
+#define FR_PANEL_TRIPLES_F32(X) X(3, 1)
 
 template <typename T>
-inline size_t panel_smem_bytes(const PanelOp<T> &op, size_t stage_elems) {
-  return op.smem_op + PANEL_NSTAGE * stage_elems * sizeof(T) + 16;
+inline size_t panel_smem_bytes(const PanelOp<T> &op) {
+  return op.smem_op + (size_t)PANEL_NSTAGE * op.stage_elems * sizeof(T) + 16;
+}
+
+// cp.async of `nrows` rows of a [rows][5][ld] state matrix into stage rows (pitch LDB, column v*NE + e); every thread owns a
+// fixed 16-byte column piece and walks down the rows.  gsrc points at (first row, v = 0, first element of the panel).
+template <typename T>
+__device__ __forceinline__ void cp_rows5(T *sdst, int LDB, int NE, const T *gsrc, long long gld, long long vstride, int nrows,
+                                         int tid, int nthreads) {
+  constexpr int CTV = 16 / (int)sizeof(T);
+  const int lg = 31 - __clz(NE / CTV);
+  const int ppr = PV << lg;
+  const bool wide = nthreads >= ppr;
+  const int rpi = wide ? nthreads / ppr : 1;
+  const int sub = wide ? tid / ppr : 0;
+  if (sub >= rpi) return;
+  for (int col = tid - sub * ppr; col < ppr; col += wide ? ppr : nthreads) {
+    const int v = col >> lg, e = (col - (v << lg)) * CTV;
+    const T *g = gsrc + (long long)sub * gld + v * vstride + e;
+    T *sp = sdst + sub * LDB + v * NE + e;
+    const long long gstep = (long long)rpi * gld;
+    const int sstep = rpi * LDB;
+    for (int r = sub; r < nrows; r += rpi) {
+      pcp_async16(sp, g, 16);
+      g += gstep;
+      sp += sstep;
+    }
+  }
+}
+// same for rows of NE contiguous elements (metric terms): stage pitch NE
+template <typename T>
+__device__ __forceinline__ void cp_rows1(T *sdst, int NE, const T *gsrc, long long gld, int nrows, int tid, int nthreads) {
+  constexpr int CTV = 16 / (int)sizeof(T);
+  const int lg = 31 - __clz(NE / CTV);
+  const int np = nrows << lg;
+  for (int p = tid; p < np; p += nthreads) {
+    const int r = p >> lg, e = (p - (r << lg)) * CTV;
+    pcp_async16(sdst + r * NE + e, gsrc + (long long)r * gld + e, 16);
+  }
 }
 
 }  // namespace frb
