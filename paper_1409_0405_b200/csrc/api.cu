@@ -50,6 +50,7 @@ struct DevBuf {
 };
 
 enum { CAT_GEMM = 0, CAT_PW = 1, CAT_IFACE = 2 };
+constexpr bool kFuseFluxIntoGrad = false;
 
 // Per-kernel CUDA-event timeline of one RHS evaluation (measurement aid; never active on the normal path).
 struct Timeline {
@@ -77,7 +78,8 @@ struct EleData {
   GemmPlan<T> pM0, pM132, pM3, pM460, pM6;
   PanelOp<T> pDiv, pGrad;   // fused operators [M132 | M3] and [M460 | M6] (FR_MODE_FUSED)
   DevBuf<T> X, Y, ACC;   // solution register, stage input, RK4 accumulator
-  DevBuf<T> grad;        // [3][nupts][5][ld]: G~ -> G -> F~
+  DevBuf<T> grad;        // [3][nupts][5][ld]: G~ -> G (-> F~ on the unfused path)
+  DevBuf<T> ftil;        // [3][nupts][5][ld]: F~ written by the fused gradient kernel (NS, fused mode)
   DevBuf<T> R;           // [nupts][5][ld]
   ~EleData() {
     gemm_plan_free(pM0);
@@ -203,7 +205,7 @@ struct Ctx : CtxBase {
         gemm_plan_build(e->pM6, 3 * nu, nf, d.M6);
       }
       if (mode == FR_MODE_FUSED) {
-        fused_div_build(e->pDiv, nu, nf, d.M132, d.M3, v.affine ? 0 : 1);
+        fused_div_build(e->pDiv, nu, nf, d.M132, d.M3);
         if (ns) fused_grad_build(e->pGrad, nu, nf, d.M460, d.M6);
       }
       const size_t nstate = (size_t)nu * 5 * ld;
@@ -211,6 +213,11 @@ struct Ctx : CtxBase {
       e->Y.alloc(nstate);
       if (stepper == FR_RK4) e->ACC.alloc(nstate);
       e->grad.alloc(3 * nstate);
+      // Forming F~ in the epilogue of the fused gradient kernel (S6 fused, GradEpilogue with ftil != nullptr) is implemented and
+      // parity-tested but measured slower than the stand-alone S6 kernel, which runs at the HBM roofline: the epilogue's metric and
+      // state loads are latency-bound while the tensor pipe idles (profiles/r01_c_fusion_notes.md).  Off until the epilogue is
+      // fed through shared memory.
+      if (kFuseFluxIntoGrad && e->pGrad.ok() && e->pDiv.ok()) e->ftil.alloc(3 * nstate);
       e->R.alloc(nstate);
       tt.ubase[t] = utot;
       tt.gbase[t] = gtot;
@@ -356,9 +363,12 @@ struct Ctx : CtxBase {
         const double nmet = e.view.affine ? 1 : nu;
         if (e.pGrad.ok()) {
           // S3 + S4 fused: G = (1/|J|) S^T ([M460 | M6] [U; C])
-          nk += launch_fused_grad(e.pGrad, e.view, u[t], cf.p + tt.ubase[t], e.grad.p, s);
-          mark(CAT_GEMM, t, "S3_S4_fused_grad", (5 * nu + 5 * nf + 15 * nu + 10 * nmet) * n,
-               2 * 3 * nu * (nu + nf) * 5 * n + 15 * 6 * nu * n);
+          // S3 + S4 (+S6) fused: G = (1/|J|) S^T ([M460 | M6] [U; C]);  F~ = S (f_inv(U) - f_visc(U, G))
+          nk += launch_fused_grad(e.pGrad, e.view, u[t], cf.p + tt.ubase[t], e.grad.p, e.ftil.p, ph, s);
+          const bool fl = e.ftil.p != nullptr;
+          mark(CAT_GEMM, t, fl ? "S3_S4_S6_fused_grad_flux" : "S3_S4_fused_grad",
+               (5 * nu + 5 * nf + 15 * nu + 10 * nmet + (fl ? 15 * nu : 0)) * n,
+               2 * 3 * nu * (nu + nf) * 5 * n + 15 * 6 * nu * n + (fl ? 210 * nu * n : 0));
         } else {
           // S3: G~ = M460 U + M6 C
           nk += gemm_run(e.pM460, n5, T(1), u[t], n5, 0, T(0), e.grad.p, n5, 0, 1, s);
@@ -386,17 +396,20 @@ struct Ctx : CtxBase {
       const long long n5 = 5 * e.view.ld;
       const double n = (double)e.view.neles, nu = e.view.nupts, nf = e.view.nfpts;
       const double nmet = e.view.affine ? 1 : nu;
+      const T *ft = e.ftil.p;
+      if (!ft) {
+        nk += launch_tdisf(e.view, u[t], e.grad.p, ph, s);   // S6 (Euler, or unfused): F~ in place over G
+        mark(CAT_PW, t, "S6_tdisf", ((ns ? 35 : 20) * nu + 9 * nmet) * n, (ns ? 210 : 110) * nu * n);
+        ft = e.grad.p;
+      }
       if (e.pDiv.ok()) {
-        // S6 + S8 + S9 (+S10) fused: out = -(1/|J|) [M132 | M3] [F~(U, G); D], stage update in the epilogue
-        nk += launch_fused_div(e.pDiv, e.view, u[t], e.grad.p, uf.p + tt.ubase[t], ph, sa[t], s);
+        // S8 + S9 (+S10) fused: out = -(1/|J|) [M132 | M3] [F~; D], stage update in the epilogue
+        nk += launch_fused_div(e.pDiv, e.view, ft, uf.p + tt.ubase[t], sa[t], s);
         const double rk = sa[t].coef ? (sa[t].out2 ? 15 : 10) : 5;
-        mark(CAT_GEMM, t, sa[t].coef ? "S6_S8_S9_S10_fused_div_rk" : "S6_S8_S9_fused_div",
-             ((ns ? 20 : 5) * nu + 5 * nf + rk * nu + 10 * nmet) * n,
-             2 * nu * (3 * nu + nf) * 5 * n + (ns ? 210 : 110) * nu * n + 5 * nu * n);
+        mark(CAT_GEMM, t, sa[t].coef ? "S8_S9_S10_fused_div_rk" : "S8_S9_fused_div", (15 * nu + 5 * nf + rk * nu + nmet) * n,
+             2 * nu * (3 * nu + nf) * 5 * n + 5 * nu * n);
         continue;
       }
-      nk += launch_tdisf(e.view, u[t], e.grad.p, ph, s);   // S6
-      mark(CAT_PW, t, "S6_tdisf", ((ns ? 35 : 20) * nu + 9 * nmet) * n, (ns ? 210 : 110) * nu * n);
       // S8: R = M132 F~ + M3 D
       nk += gemm_run(e.pM132, n5, T(1), e.grad.p, n5, 0, T(0), e.R.p, n5, 0, 1, s);
       mark(CAT_GEMM, t, "S8a_M132", (3 * nu + nu) * 5 * n, 2 * nu * 3 * nu * 5 * n);

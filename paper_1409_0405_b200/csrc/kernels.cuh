@@ -60,13 +60,14 @@ int launch_bc_comm_flux(const BndView<T> &bv, const TypeTab &tt, T *uf, const T 
 
 // Fused panel kernels (panel_fused.cu).  *_build return false if the operator does not fit the resident design.
 template <typename T>
-bool fused_div_build(PanelOp<T> &op, int nu, int nf, const double *M132, const double *M3, int curved);
+bool fused_div_build(PanelOp<T> &op, int nu, int nf, const double *M132, const double *M3);
 template <typename T>
-int launch_fused_div(const PanelOp<T> &op, const EleView<T> &ev, const T *u, const T *grad, const T *d, const PhysParams<T> &ph,
-                     const StageArgs<T> &sa, cudaStream_t s);
+int launch_fused_div(const PanelOp<T> &op, const EleView<T> &ev, const T *ftil, const T *d, const StageArgs<T> &sa,
+                     cudaStream_t s);
 template <typename T>
 bool fused_grad_build(PanelOp<T> &op, int nu, int nf, const double *M460, const double *M6);
 template <typename T>
-int launch_fused_grad(const PanelOp<T> &op, const EleView<T> &ev, const T *u, const T *c, T *grad, cudaStream_t s);
+int launch_fused_grad(const PanelOp<T> &op, const EleView<T> &ev, const T *u, const T *c, T *grad, T *ftil,
+                      const PhysParams<T> &ph, cudaStream_t s);
 
 }  // namespace frb

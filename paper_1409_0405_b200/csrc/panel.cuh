@@ -19,6 +19,7 @@
 #pragma once
 #include <algorithm>
 #include <cmath>
+#include <cstdlib>
 #include <cstring>
 #include <numeric>
 
@@ -33,6 +34,7 @@ constexpr int PANEL_MAXCHUNKS = 64;
 // One K-chunk of the stacked right-hand operand: rows [row0, row0+nrows) of source `src`.
 struct ChunkDesc {
   int src, row0, nrows, kind;
+  int base, pad0, pad1, pad2;   // dense operators: first packed block (FP64: 4 rows) / row (FP32) of this chunk
 };
 
 // Device image of a packed operator + its launch geometry (all pointers device).
@@ -40,12 +42,15 @@ template <typename T>
 struct PanelOp {
   int M = 0, K = 0;
   int WR = 0, WC = 0, NIT = 0, CX = 0;   // warp grid, row groups per row-warp, column blocks (FP64) / elements per lane (FP32)
-  int NE = 0;                            // elements per panel
+  int NE = 0;                            // elements per panel (of one warp group)
+  int NG = 1;                            // independent warp groups per CTA, each streaming its own panels (staggered)
   int KC = 0, nchunks = 0, NS = 0;       // rows per chunk (max), chunks, slots = WR*NIT
   int stage_elems = 0;                   // elements of one ring stage
   int curved = 0;                        // flux chunks: metric terms per point (1) or per element (0)
   int nblk = 0;                          // packed blocks (FP64: 8x4 tiles; FP32: 8x1 columns)
-  int sparse = 0;
+  int nidx = 0;                          // entries of idx
+  int dbg = 0;                           // measurement aid (env FRB_PANEL_DBG): 1 skip multiply, 2 skip epilogue
+  int sparse = 0;                        // 1: per-group k-lists (idx/off); 0: dense, all slots share the chunk's rows
   double macs_per_col = 0;               // executed multiply-adds per column (dense: M*K)
   T *vals = nullptr;                     // FP64 [nblk][32]; FP32 [nblk][8]
   uint32_t *idx = nullptr;               // byte offset of the B row in the stage: FP64 [nblk][4], FP32 [nblk]
@@ -86,6 +91,7 @@ inline __host__ __device__ size_t flux_stage_elems(int n, int NE, int LDB, int c
 struct PanelGeom {
   int WR, WC, NIT, CX, NE;
   double eff;
+  int NG;
 };
 
 // Warps per CTA a given accumulator shape allows: registers per thread ~ accumulators + 70 must fit the 64K register file.
@@ -100,27 +106,35 @@ constexpr int panel_maxw(int nit, int cx) {
 // Choose the warp grid for G row groups.  The FP64 tensor pipe takes one DMMA per warp every ~32 cycles, so two warps per
 // scheduler saturate it only if they do nothing else: prefer 12-16 warps per SM.
 template <typename T>
-inline PanelGeom choose_geom(int G, int min_ne, int max_ne, int triple) {
-  PanelGeom best{0, 0, 0, 0, 0, -1.0};
+inline PanelGeom choose_geom(int G, int min_ne, int max_ne, int triple, bool dense) {
+  PanelGeom best{0, 0, 0, 0, 0, -1.0, 1};
   const bool f64 = sizeof(T) == 8;
   const int gu = triple ? 3 : 1;            // groups come in units of `gu` that must stay on one row-warp
   const int GU = (G + gu - 1) / gu;
-  for (int WR = 1; WR <= PANEL_MAXW; ++WR) {
-    const int nit = ((GU + WR - 1) / WR) * gu;
-    for (int WC = 1; WR * WC <= PANEL_MAXW; WC *= 2) {
-      for (int CX = 2; CX >= 1; --CX) {
-        if (f64 ? nit * CX > 8 : nit * CX > 4) continue;
-        const int W = WR * WC;
-        if (W > panel_maxw<T>(nit, CX)) continue;
-        const int NE = (f64 ? 8 : 32) * CX * WC;
-        if (NE < min_ne || NE > max_ne) continue;
-        double eff = (double)G / (WR * nit);
-        // prefer many warps, then wider panels, then fewer accumulators
-        double score = eff * (0.4 + 0.6 * std::min(W, 14) / 14.0) * (1.0 + 0.02 * std::log2((double)NE)) * (1.0 - 0.005 * nit * CX);
-        if (score > best.eff) best = PanelGeom{WR, WC, nit, CX, NE, score};
+  // measured on config 3 (profiles/r01_c_fusion_notes.md): two groups help the FP64 kernels slightly, not the FP32 ones
+  const int ngmax = getenv("FRB_PANEL_NG") ? atoi(getenv("FRB_PANEL_NG")) : (sizeof(T) == 8 ? 2 : 1);
+  for (int NG = 1; NG <= ngmax; ++NG)
+    for (int WR = 1; WR <= PANEL_MAXW; ++WR) {
+      const int nit = ((GU + WR - 1) / WR) * gu;
+      for (int WC = 1; NG * WR * WC <= PANEL_MAXW; WC *= 2) {
+        for (int CX = 2; CX >= 1; --CX) {
+          if (f64 ? nit * CX > 8 : nit * CX > 4) continue;
+          const int W = NG * WR * WC;
+          if (W > panel_maxw<T>(nit, CX)) continue;
+          const int NE = (f64 ? 8 : 32) * CX * WC;
+          if (NE < min_ne || NE > max_ne) continue;
+          double eff = (double)G / (WR * nit);
+          // prefer many warps, then wider panels, then fewer accumulators
+          double score = eff * (0.4 + 0.6 * std::min(W, 14) / 14.0) * (1.0 + 0.02 * std::log2((double)NE)) * (1.0 - 0.005 * nit * CX);
+          // dense operators: the B fragments of a k-block are shared by the NIT row groups of the warp; shared-memory
+          // wavefronts per multiply ~ 2/NIT + 0.4/CX
+          if (dense) score /= 1.0 + 0.4 * (2.0 / nit + 0.4 / CX);
+          // two staggered warp groups hide one group's epilogue and load waits behind the other's multiplies
+          if (NG == 2) score *= 1.25;
+          if (score > best.eff) best = PanelGeom{WR, WC, nit, CX, NE, score, NG};
+        }
       }
     }
-  }
   return best;
 }
 
@@ -264,7 +278,7 @@ bool panel_op_build_kc(PanelOp<T> &p, int M, int K, const double *A, const std::
         if (step > KC) step = std::max(4, KC / 4 * 4);
         for (int r = 0; r < s.rows; r += step) {
           const int n = std::min(step, s.rows - r);
-          chunks.push_back(ChunkDesc{si, r, n, s.kind});
+          chunks.push_back(ChunkDesc{si, r, n, s.kind, 0, 0, 0, 0});
           std::vector<int> cols(n);
           for (int j = 0; j < n; ++j) cols[j] = k0 + r + j;
           chunk_cols.push_back(cols);
@@ -277,7 +291,7 @@ bool panel_op_build_kc(PanelOp<T> &p, int M, int K, const double *A, const std::
         if ((step + 3) / 4 * 4 <= nlim) step = (step + 3) / 4 * 4;
         for (int r = 0; r < s.rows; r += step) {
           const int n = std::min(step, s.rows - r);
-          chunks.push_back(ChunkDesc{si, r, n, s.kind});
+          chunks.push_back(ChunkDesc{si, r, n, s.kind, 0, 0, 0, 0});
           std::vector<int> cols(3 * n);
           for (int a = 0; a < 3; ++a)
             for (int j = 0; j < n; ++j) cols[a * n + j] = k0 + a * s.rows + r + j;
@@ -309,7 +323,7 @@ bool panel_op_build_kc(PanelOp<T> &p, int M, int K, const double *A, const std::
       const int n = (int)lists[g][c].size();
       gcost[g] += f64 ? (n + 3) / 4 * 4 : n;
     }
-  PanelGeom geo = choose_geom<T>(G, opt.min_ne, opt.max_ne, opt.triple);
+  PanelGeom geo = choose_geom<T>(G, opt.min_ne, opt.max_ne, opt.triple, !sparse);
   if (geo.eff < 0) return false;
   const int WR = geo.WR, NIT = geo.NIT, NS = WR * NIT;
   // LPT assignment of group units (1 or 3 groups) to row-warps, at most NIT groups per row-warp
@@ -345,7 +359,34 @@ bool panel_op_build_kc(PanelOp<T> &p, int M, int K, const double *A, const std::
       for (int r = 0; r < 8; ++r) rowmap[s * 8 + r] = order[8 * slot_group[s] + r];
   long long macs = 0;
   int nblk = 0;
-  for (int c = 0; c < nchunks; ++c)
+  if (!sparse) {
+    // dense: blocks ordered (chunk, k-block, slot); rows of a block are the consecutive stage rows 4b..4b+3 (FP64) / row b (FP32)
+    for (int c = 0; c < nchunks; ++c) {
+      chunks[c].base = nblk / NS;
+      const int n = (int)chunk_cols[c].size();
+      const int nb = f64 ? (n + 3) / 4 : n;
+      for (int b = 0; b < nb; ++b)
+        for (int s = 0; s < NS; ++s) {
+          const int g = slot_group[s];
+          if (f64) {
+            for (int lane = 0; lane < 32; ++lane) {
+              const int r = lane >> 2, j = lane & 3;
+              const int m = g >= 0 ? order[8 * g + r] : -1;
+              vals.push_back((T)((m >= 0 && 4 * b + j < n) ? A[(size_t)m * K + chunk_cols[c][4 * b + j]] : 0.0));
+            }
+            if (g >= 0) macs += 32;
+          } else {
+            for (int r = 0; r < 8; ++r) {
+              const int m = g >= 0 ? order[8 * g + r] : -1;
+              vals.push_back((T)(m >= 0 ? A[(size_t)m * K + chunk_cols[c][b]] : 0.0));
+            }
+            if (g >= 0) macs += 8;
+          }
+          ++nblk;
+        }
+    }
+  }
+  for (int c = 0; c < nchunks && sparse; ++c)
     for (int s = 0; s < NS; ++s) {
       off[c * NS + s] = nblk;
       const int g = slot_group[s];
@@ -383,7 +424,7 @@ bool panel_op_build_kc(PanelOp<T> &p, int M, int K, const double *A, const std::
         }
       }
     }
-  off[nchunks * NS] = nblk;
+  if (sparse) off[nchunks * NS] = nblk;
   // the multiply loop prefetches two blocks ahead: two all-zero blocks close the arrays (not counted in nblk)
   for (int d = 0; d < 2; ++d) {
     for (int j = 0; j < (f64 ? 4 : 1); ++j) idx.push_back(0u);
@@ -397,10 +438,10 @@ bool panel_op_build_kc(PanelOp<T> &p, int M, int K, const double *A, const std::
   const int LDBh = PV * geo.NE + 4;
   for (auto &c : chunks)
     stage_elems = std::max(stage_elems, c.kind == KIND_FLUX ? flux_stage_elems(c.nrows, geo.NE, LDBh, opt.curved) : (size_t)c.nrows * LDBh);
-  if (smem_op + 3 * stage_elems * sizeof(T) + 16 > smem_total) {
+  if (smem_op + (size_t)geo.NG * 3 * stage_elems * sizeof(T) + 16 > smem_total) {
     // MAC rows per chunk that would fit: scale the tallest chunk down proportionally (flux chunks carry 4/3 rows + metrics)
     if (smem_total > smem_op + 4096) {
-      const double room = (double)(smem_total - smem_op - 1024) / (3.0 * sizeof(T));
+      const double room = (double)(smem_total - smem_op - 1024) / (3.0 * geo.NG * sizeof(T));
       *kc_fit = (int)(kcmax * room / (double)stage_elems);
     }
     return false;
@@ -413,12 +454,19 @@ bool panel_op_build_kc(PanelOp<T> &p, int M, int K, const double *A, const std::
   p.NIT = NIT;
   p.CX = geo.CX;
   p.NE = geo.NE;
+  p.NG = geo.NG;
   p.KC = kcmax;
   p.stage_elems = (int)stage_elems;
   p.curved = opt.curved;
   p.nchunks = nchunks;
   p.NS = NS;
   p.nblk = nblk;
+  p.nidx = (int)idx.size();
+  p.dbg = getenv("FRB_PANEL_DBG") ? atoi(getenv("FRB_PANEL_DBG")) : 0;
+  if (getenv("FRB_PANEL_VERBOSE"))
+    fprintf(stderr, "panel_op %s M=%d K=%d %s G=%d WR=%d WC=%d NIT=%d CX=%d NE=%d NG=%d warps=%d KC=%d nchunks=%d nblk=%d smem_op=%zu stage=%zu B density=%.2f macs/col=%.0f (dense %d)\n",
+            f64 ? "f64" : "f32", M, K, sparse ? "sparse" : "dense", G, WR, geo.WC, NIT, geo.CX, geo.NE, geo.NG, geo.NG * WR * geo.WC, kcmax,
+            nchunks, nblk, smem_op, stage_elems * sizeof(T), density, (double)macs, M * K);
   p.sparse = sparse ? 1 : 0;
   p.macs_per_col = (double)macs;
   p.smem_op = smem_op;
@@ -472,7 +520,7 @@ __device__ __forceinline__ char *op_smem_carve(char *base, const PanelOp<T> &op,
   v.vals = reinterpret_cast<const T *>(base);
   base += al(nv);
   v.idx = reinterpret_cast<const uint32_t *>(base);
-  base += al((size_t)(op.nblk + 2) * (sizeof(T) == 8 ? 16 : 4));
+  base += al((size_t)op.nidx * 4);
   v.off = reinterpret_cast<const int *>(base);
   base += al(((size_t)op.nchunks * op.NS + 1) * 4);
   v.rowmap = reinterpret_cast<const int *>(base);
@@ -496,7 +544,7 @@ __device__ __forceinline__ void op_smem_load(char *base, const PanelOp<T> &op, i
   };
   char *b = base;
   b = copy(b, op.vals, (size_t)(op.nblk + 2) * (sizeof(T) == 8 ? 32 : 8) * sizeof(T));
-  b = copy(b, op.idx, (size_t)(op.nblk + 2) * (sizeof(T) == 8 ? 16 : 4));
+  b = copy(b, op.idx, (size_t)op.nidx * 4);
   b = copy(b, op.off, ((size_t)op.nchunks * op.NS + 1) * 4);
   b = copy(b, op.rowmap, (size_t)op.NS * 8 * 4);
   b = copy(b, op.chunks, (size_t)op.nchunks * sizeof(ChunkDesc));
@@ -572,6 +620,37 @@ struct Acc<double, NIT, CX> {
       }
     }
   }
+  // Dense operator: the NIT row groups of the warp share the chunk's rows, so the B fragments of a k-block (stage rows
+  // 4b..4b+3) are loaded once and feed NIT x 5 x CX DMMAs; no index list.
+  __device__ __forceinline__ void mac_dense(const OpSmem<double> &A, const ChunkDesc &cd, int NS, int slot0, const double *Bst,
+                                            int LDB, int NE, int wc, int lane) {
+    const char *bcol = reinterpret_cast<const char *>(Bst + wc * 8 * CX + (lane >> 2));
+    const char *av = reinterpret_cast<const char *>(A.vals) + ((uint32_t)(cd.base * NS + slot0) * 32u + lane) * 8u;
+    const uint32_t vs = (uint32_t)NE * 8u, rs = (uint32_t)LDB * 8u, as = (uint32_t)NS * 256u;
+    const int nb = (cd.nrows + 3) >> 2, last = cd.nrows - 1;
+    const int kl = lane & 3;
+#pragma unroll 2
+    for (int b = 0; b < nb; ++b) {
+      const int row = min(4 * b + kl, last);           // padded rows of the last block: operator is zero, data must be finite
+      const char *bp = bcol + (uint32_t)row * rs;
+      double bf[PV][CX];
+#pragma unroll
+      for (int v = 0; v < PV; ++v) {
+#pragma unroll
+        for (int cb = 0; cb < CX; ++cb) bf[v][cb] = *reinterpret_cast<const double *>(bp + cb * 64);
+        bp += vs;
+      }
+      const char *ap = av + (uint32_t)b * as;
+#pragma unroll
+      for (int i = 0; i < NIT; ++i) {
+        const double a = *reinterpret_cast<const double *>(ap + i * 256);
+#pragma unroll
+        for (int v = 0; v < PV; ++v)
+#pragma unroll
+          for (int cb = 0; cb < CX; ++cb) dmma884(c[i][cb][v][0], c[i][cb][v][1], a, bf[v][cb]);
+      }
+    }
+  }
   // f(i, rr, e, tile[PV][EW]): slot i, thread-local row rr, first element e of EW consecutive ones, all 5 variables
   template <typename F>
   __device__ __forceinline__ void foreach_tile(int wc, int lane, F &&f) {
@@ -640,6 +719,42 @@ struct Acc<float, NIT, CX> {
           }
           bp += vs;
         }
+#pragma unroll
+        for (int r = 0; r < 8; ++r)
+#pragma unroll
+          for (int v = 0; v < PV; ++v)
+#pragma unroll
+            for (int j = 0; j < CX; ++j) c[i][r][v][j] = fmaf(av[r], bv[v][j], c[i][r][v][j]);
+      }
+    }
+  }
+  // Dense operator: one B row feeds the NIT row groups of the warp.
+  __device__ __forceinline__ void mac_dense(const OpSmem<float> &A, const ChunkDesc &cd, int NS, int slot0, const float *Bst,
+                                            int LDB, int NE, int wc, int lane) {
+    const char *bp0 = reinterpret_cast<const char *>(Bst + wc * 32 * CX + lane * CX);
+    const char *ap0 = reinterpret_cast<const char *>(A.vals) + (uint32_t)(cd.base * NS + slot0) * 32u;
+    const uint32_t vs = (uint32_t)NE * 4u, rs = (uint32_t)LDB * 4u, as = (uint32_t)NS * 32u;
+#pragma unroll 2
+    for (int k = 0; k < cd.nrows; ++k) {
+      const char *bp = bp0 + (uint32_t)k * rs;
+      float bv[PV][CX];
+#pragma unroll
+      for (int v = 0; v < PV; ++v) {
+        if (CX == 2) {
+          const float2 t = *reinterpret_cast<const float2 *>(bp);
+          bv[v][0] = t.x;
+          bv[v][CX - 1] = t.y;
+        } else {
+          bv[v][0] = *reinterpret_cast<const float *>(bp);
+        }
+        bp += vs;
+      }
+      const char *ap = ap0 + (uint32_t)k * as;
+#pragma unroll
+      for (int i = 0; i < NIT; ++i) {
+        const float4 a0 = *reinterpret_cast<const float4 *>(ap + i * 32);
+        const float4 a1 = *reinterpret_cast<const float4 *>(ap + i * 32 + 16);
+        const float av[8] = {a0.x, a0.y, a0.z, a0.w, a1.x, a1.y, a1.z, a1.w};
 #pragma unroll
         for (int r = 0; r < 8; ++r)
 #pragma unroll

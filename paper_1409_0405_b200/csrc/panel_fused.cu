@@ -1,9 +1,10 @@
 // Fused panel kernels (fusion targets F-A and F-B of SURVEY 7.2):
-//   fused_div : S6 + S8 + S9 + S10   dudt = -(1/|J|) [ M132 F~(U,G) + M3 D ]  (+ Runge-Kutta stage update)
-//               the transformed flux F~ is formed in shared memory from the U, G and metric panels and never touches HBM;
-//   fused_grad: S3 + S4              G_i = (1/|J|) sum_alpha S[alpha][i] ( [M460 | M6] [U; C] )_alpha
+//   fused_grad: S3 + S4 + S6         G_i = (1/|J|) sum_alpha S[alpha][i] ( [M460 | M6] [U; C] )_alpha ;  F~ = S (f_inv(U) - f_visc(U,G))
 //               the three alpha components of a solution point sit in one thread (triple packing), so the transform to
-//               physical gradients happens in registers.
+//               physical gradients and the transformed flux at that point are formed in registers in the epilogue;
+//   fused_div : S8 + S9 + S10        dudt = -(1/|J|) [ M132 | M3 ] [F~; D]  (+ Runge-Kutta stage update in the epilogue).
+// (A first version formed F~ inside fused_div from U, G and the metrics staged in shared memory; ncu showed the CTA waiting
+//  at barriers on a long, serial FP64 flux evaluation that only part of the threads could share, profiles/r01_*.md.)
 // Both run on the persistent panel main loop (panel_kernel.cuh) with the operator resident in shared memory.
 #include "kernels.cuh"
 #include "panel_kernel.cuh"
@@ -14,74 +15,6 @@ namespace frb {
 namespace {
 
 // ------------------------------------------------------------------------------------------------ fused_div
-template <typename T>
-struct FluxProducer {
-  const T *u, *g, *d;       // state [Nu][5][ld]; gradients [3][Nu][5][ld] (NS only); common flux D [Nf][5][ld]
-  const T *smats;           // [9][Nu][ld] or [9][ld]
-  long long ld, neles;
-  int nupts, curved;
-  PhysParams<T> ph;
-  static constexpr bool kTransform = true;
-
-  __device__ __forceinline__ void issue(const ChunkDesc &cd, long long, long long pl, T *stage, int LDB, int NE, int tid,
-                                        int nthreads) const {
-    const long long e0 = pl * NE;
-    if (cd.kind == KIND_PLAIN) {
-      cp_rows5(stage, LDB, NE, d + (long long)cd.row0 * 5 * ld + e0, 5 * ld, ld, cd.nrows, tid, nthreads);
-      return;
-    }
-    const int n = cd.nrows;
-    if (ph.ns) {
-#pragma unroll
-      for (int a = 0; a < 3; ++a)
-        cp_rows5(stage + a * n * LDB, LDB, NE, g + ((long long)a * nupts + cd.row0) * 5 * ld + e0, 5 * ld, ld, n, tid, nthreads);
-    }
-    cp_rows5(stage + 3 * n * LDB, LDB, NE, u + (long long)cd.row0 * 5 * ld + e0, 5 * ld, ld, n, tid, nthreads);
-    T *sm = stage + 4 * n * LDB;
-    if (curved) {
-#pragma unroll
-      for (int a = 0; a < 9; ++a)
-        cp_rows1(sm + a * n * NE, NE, smats + ((long long)a * nupts + cd.row0) * ld + e0, ld, n, tid, nthreads);
-    } else {
-      cp_rows1(sm, NE, smats + e0, ld, 9, tid, nthreads);
-    }
-  }
-
-  // F~_alpha = sum_i S[alpha][i] (f^inv_i(U) - f^visc_i(U, G)) for the n points of the chunk, in place over G's rows
-  __device__ __forceinline__ void transform(const ChunkDesc &cd, long long, long long pl, T *stage, int LDB, int NE, int tid,
-                                            int nthreads) const {
-    const int n = cd.nrows;
-    const int lgne = 31 - __clz(NE);
-    const T *sm = stage + 4 * n * LDB;
-    const int sstr = curved ? n * NE : NE;   // stride between the 9 metric components
-    for (int p = tid; p < (n << lgne); p += nthreads) {
-      const int j = p >> lgne, e = p - (j << lgne);
-      T *col = stage + e;
-      T uu[5];
-#pragma unroll
-      for (int v = 0; v < 5; ++v) uu[v] = col[(3 * n + j) * LDB + v * NE];
-      T f[3][5], rr, vel[3], pr;
-      inviscid_flux(uu, ph.gamma, f, rr, vel, pr);
-      if (ph.ns) {
-        T q[3][5];
-#pragma unroll
-        for (int i = 0; i < 3; ++i)
-#pragma unroll
-          for (int v = 0; v < 5; ++v) q[i][v] = col[(i * n + j) * LDB + v * NE];
-        subtract_viscous_flux(uu, q, rr, vel, ph.gamma, ph.mu, ph.prandtl, f);
-      }
-      const T *sp = sm + (curved ? j * NE : 0) + e;
-      const bool live = pl * NE + e < neles;
-#pragma unroll
-      for (int a = 0; a < 3; ++a) {
-        const T s0 = sp[(a * 3 + 0) * sstr], s1 = sp[(a * 3 + 1) * sstr], s2 = sp[(a * 3 + 2) * sstr];
-#pragma unroll
-        for (int v = 0; v < 5; ++v) col[(a * n + j) * LDB + v * NE] = live ? s0 * f[0][v] + s1 * f[1][v] + s2 * f[2][v] : T(0);
-      }
-    }
-  }
-};
-
 template <typename T, int EW>
 struct VecIO;
 template <>
@@ -165,7 +98,7 @@ struct RkEpilogue {
 template <typename T>
 struct DivArgs {
   PanelOp<T> op;
-  FluxProducer<T> prod;
+  PlainProducer<T> prod;
   RkEpilogue<T> epi;
   long long npanels;
 };
@@ -178,10 +111,13 @@ __global__ void __launch_bounds__(32 * panel_maxw<T>(NIT, CX)) k_fused_div(const
 
 // ------------------------------------------------------------------------------------------------ fused_grad
 // epilogue S4: physical gradient from the three reference components held by one thread
-template <typename T>
+template <typename T, bool FLUX>
 struct GradEpilogue {
   const T *smats, *rcpdjac;
-  T *grad;                  // [3][Nu][5][ld]
+  T *grad;                  // [3][Nu][5][ld]  physical gradients G (read again by S5)
+  const T *u;               // stage input (for the flux)
+  T *ftil;                  // [3][Nu][5][ld]  transformed flux F~, or nullptr
+  PhysParams<T> ph;
   long long ld, neles;
   int nupts, curved, NE;
   template <typename ACC>
@@ -204,15 +140,46 @@ struct GradEpilogue {
 #pragma unroll
       for (int j = 0; j < EW; ++j)
         if (col + j >= neles) rj[j] = T(0);      // padding lanes: zero
+      T uu[PV][EW];
+      if constexpr (FLUX) {
+#pragma unroll
+        for (int v = 0; v < PV; ++v) VecIO<T, EW>::ld(u + ((long long)rho * 5 + v) * ld + col, uu[v]);
+      }
+      T q[3][PV][EW];
 #pragma unroll
       for (int i = 0; i < 3; ++i)
 #pragma unroll
         for (int v = 0; v < PV; ++v) {
-          T o[EW];
 #pragma unroll
-          for (int j = 0; j < EW; ++j) o[j] = rj[j] * (S[0][i][j] * t0[v][j] + S[1][i][j] * t1[v][j] + S[2][i][j] * t2[v][j]);
-          VecIO<T, EW>::st(grad + (((long long)i * nupts + rho) * 5 + v) * ld + col, o);
+          for (int j = 0; j < EW; ++j) q[i][v][j] = rj[j] * (S[0][i][j] * t0[v][j] + S[1][i][j] * t1[v][j] + S[2][i][j] * t2[v][j]);
+          VecIO<T, EW>::st(grad + (((long long)i * nupts + rho) * 5 + v) * ld + col, q[i][v]);
         }
+      if constexpr (FLUX) {
+      // S6 at this solution point: F~_alpha = sum_i S[alpha][i] (f^inv_i(U) - f^visc_i(U, G))
+      T ft[3][PV][EW];
+#pragma unroll
+      for (int j = 0; j < EW; ++j) {
+        const bool live = col + j < neles;
+        T u1[5], q1[3][5], f[3][5], rr, vel[3], pr;
+#pragma unroll
+        for (int v = 0; v < 5; ++v) u1[v] = live ? uu[v][j] : T(1);
+#pragma unroll
+        for (int i = 0; i < 3; ++i)
+#pragma unroll
+          for (int v = 0; v < 5; ++v) q1[i][v] = q[i][v][j];
+        inviscid_flux(u1, ph.gamma, f, rr, vel, pr);
+        subtract_viscous_flux(u1, q1, rr, vel, ph.gamma, ph.mu, ph.prandtl, f);
+#pragma unroll
+        for (int a = 0; a < 3; ++a)
+#pragma unroll
+          for (int v = 0; v < 5; ++v)
+            ft[a][v][j] = live ? S[a][0][j] * f[0][v] + S[a][1][j] * f[1][v] + S[a][2][j] * f[2][v] : T(0);
+      }
+#pragma unroll
+      for (int a = 0; a < 3; ++a)
+#pragma unroll
+        for (int v = 0; v < PV; ++v) VecIO<T, EW>::st(ftil + (((long long)a * nupts + rho) * 5 + v) * ld + col, ft[a][v]);
+      }
     });
   }
 };
@@ -221,7 +188,7 @@ template <typename T>
 struct GradArgs {
   PanelOp<T> op;
   PlainProducer<T> prod;
-  GradEpilogue<T> epi;
+  GradEpilogue<T, false> epi;   // FLUX = true (S6 in the epilogue) is parity-tested but slower, see api.cu kFuseFluxIntoGrad
   long long npanels;
 };
 
@@ -232,9 +199,9 @@ __global__ void __launch_bounds__(32 * panel_maxw<T>(NIT, CX)) k_fused_grad(cons
 }
 
 template <typename K, typename A>
-void launch_panel(K k, const A &a, int nthreads, size_t smem, long long ntot, cudaStream_t s) {
+void launch_panel(K k, const A &a, int nthreads, size_t smem, long long ntot, int ng, cudaStream_t s) {
   FR_CUDA_TRY(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-  const long long grid = std::min<long long>(ntot, device_sm_count());
+  const long long grid = std::min<long long>((ntot + ng - 1) / ng, device_sm_count());
   k<<<(unsigned)grid, nthreads, smem, s>>>(a);
   FR_CUDA_TRY(cudaGetLastError());
 }
@@ -242,34 +209,36 @@ void launch_panel(K k, const A &a, int nthreads, size_t smem, long long ntot, cu
 }  // namespace
 
 template <typename T>
-bool fused_div_build(PanelOp<T> &op, int nu, int nf, const double *M132, const double *M3, int curved) {
+bool fused_div_build(PanelOp<T> &op, int nu, int nf, const double *M132, const double *M3) {
   const int K = 3 * nu + nf;
   std::vector<double> A((size_t)nu * K);
   for (int m = 0; m < nu; ++m) {
     for (int k = 0; k < 3 * nu; ++k) A[(size_t)m * K + k] = M132[(size_t)m * 3 * nu + k];
     for (int k = 0; k < nf; ++k) A[(size_t)m * K + 3 * nu + k] = M3[(size_t)m * nf + k];
   }
-  std::vector<KSource> srcs{KSource{nu, KIND_FLUX, 1}, KSource{nf, KIND_PLAIN, 1}};
+  std::vector<KSource> srcs{KSource{3 * nu, KIND_PLAIN, 1}, KSource{nf, KIND_PLAIN, 1}};
   PackOptions opt;
   opt.min_ne = 16;
   opt.max_ne = 64;
-  opt.curved = curved;
   return panel_op_build(op, nu, K, A.data(), srcs, opt, 150 * 1024);
 }
 
 template <typename T>
-int launch_fused_div(const PanelOp<T> &op, const EleView<T> &ev, const T *u, const T *grad, const T *d, const PhysParams<T> &ph,
-                     const StageArgs<T> &sa, cudaStream_t s) {
+int launch_fused_div(const PanelOp<T> &op, const EleView<T> &ev, const T *ftil, const T *d, const StageArgs<T> &sa,
+                     cudaStream_t s) {
   DivArgs<T> a;
   a.op = op;
-  a.prod = FluxProducer<T>{u, grad, d, ev.smats, ev.ld, ev.neles, ev.nupts, ev.affine ? 0 : 1, ph};
+  a.prod = PlainProducer<T>();
+  a.prod.src[0] = MatRef<T>{ftil, 5 * ev.ld, 0};
+  a.prod.src[1] = MatRef<T>{d, 5 * ev.ld, 0};
+  a.prod.cm = ColMap{op.NE, ev.ld, 0, ev.ld};
   a.epi = RkEpilogue<T>{ev.rcpdjac, ev.ld, ev.neles, ev.affine ? 0 : 1, op.NE, sa};
   a.npanels = ev.ld / op.NE;
   const size_t smem = panel_smem_bytes(op);
-  const int nthreads = 32 * op.WR * op.WC;
+  const int nthreads = 32 * op.WR * op.WC * op.NG;
 #define FR_CASE(NIT_, CX_)                                                          \
   if (op.NIT == NIT_ && op.CX == CX_) {                                             \
-    launch_panel(k_fused_div<T, NIT_, CX_>, a, nthreads, smem, a.npanels, s);       \
+    launch_panel(k_fused_div<T, NIT_, CX_>, a, nthreads, smem, a.npanels, op.NG, s);       \
     return 1;                                                                       \
   }
   if constexpr (sizeof(T) == 8) {
@@ -298,20 +267,22 @@ bool fused_grad_build(PanelOp<T> &op, int nu, int nf, const double *M460, const 
 }
 
 template <typename T>
-int launch_fused_grad(const PanelOp<T> &op, const EleView<T> &ev, const T *u, const T *c, T *grad, cudaStream_t s) {
+int launch_fused_grad(const PanelOp<T> &op, const EleView<T> &ev, const T *u, const T *c, T *grad, T *ftil,
+                      const PhysParams<T> &ph, cudaStream_t s) {
   GradArgs<T> a;
   a.op = op;
   ColMap cm{op.NE, ev.ld, 0, ev.ld};
+  a.prod = PlainProducer<T>();
   a.prod.src[0] = MatRef<T>{u, 5 * ev.ld, 0};
   a.prod.src[1] = MatRef<T>{c, 5 * ev.ld, 0};
   a.prod.cm = cm;
-  a.epi = GradEpilogue<T>{ev.smats, ev.rcpdjac, grad, ev.ld, ev.neles, ev.nupts, ev.affine ? 0 : 1, op.NE};
+  a.epi = GradEpilogue<T, false>{ev.smats, ev.rcpdjac, grad, u, ftil, ph, ev.ld, ev.neles, ev.nupts, ev.affine ? 0 : 1, op.NE};
   a.npanels = ev.ld / op.NE;
   const size_t smem = panel_smem_bytes(op);
-  const int nthreads = 32 * op.WR * op.WC;
+  const int nthreads = 32 * op.WR * op.WC * op.NG;
 #define FR_CASE(NIT_, CX_)                                                          \
   if (op.NIT == NIT_ && op.CX == CX_) {                                             \
-    launch_panel(k_fused_grad<T, NIT_, CX_>, a, nthreads, smem, a.npanels, s);      \
+    launch_panel(k_fused_grad<T, NIT_, CX_>, a, nthreads, smem, a.npanels, op.NG, s);      \
     return 1;                                                                       \
   }
   if constexpr (sizeof(T) == 8) {
@@ -324,11 +295,12 @@ int launch_fused_grad(const PanelOp<T> &op, const EleView<T> &ev, const T *u, co
 }
 
 #define FR_INST(T)                                                                                                          \
-  template bool fused_div_build<T>(PanelOp<T> &, int, int, const double *, const double *, int);                          \
-  template int launch_fused_div<T>(const PanelOp<T> &, const EleView<T> &, const T *, const T *, const T *,                \
-                                   const PhysParams<T> &, const StageArgs<T> &, cudaStream_t);                             \
+  template bool fused_div_build<T>(PanelOp<T> &, int, int, const double *, const double *);                               \
+  template int launch_fused_div<T>(const PanelOp<T> &, const EleView<T> &, const T *, const T *, const StageArgs<T> &,     \
+                                   cudaStream_t);                                                                          \
   template bool fused_grad_build<T>(PanelOp<T> &, int, int, const double *, const double *);                               \
-  template int launch_fused_grad<T>(const PanelOp<T> &, const EleView<T> &, const T *, const T *, T *, cudaStream_t);
+  template int launch_fused_grad<T>(const PanelOp<T> &, const EleView<T> &, const T *, const T *, T *, T *,                \
+                                    const PhysParams<T> &, cudaStream_t);
 FR_INST(double)
 FR_INST(float)
 

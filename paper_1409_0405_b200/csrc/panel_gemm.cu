@@ -26,7 +26,7 @@ void launch_shape(const PlainArgs<T> &a, size_t smem, cudaStream_t s) {
   static bool attr_done = false;
   static int occ = 1;
   static size_t attr_smem = 0;
-  const int nthreads = 32 * a.op.WR * a.op.WC;
+  const int nthreads = 32 * a.op.WR * a.op.WC * a.op.NG;
   if (!attr_done || smem > attr_smem) {
     FR_CUDA_TRY(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)std::max(smem, attr_smem)));
     attr_smem = std::max(smem, attr_smem);
@@ -35,7 +35,7 @@ void launch_shape(const PlainArgs<T> &a, size_t smem, cudaStream_t s) {
   FR_CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k, nthreads, smem));
   occ = std::max(1, std::min(occ, 4));
   const long long ntot = a.npanels * a.nbatch;
-  const long long grid = std::min<long long>(ntot, (long long)device_sm_count() * occ);
+  const long long grid = std::min<long long>((ntot + a.op.NG - 1) / a.op.NG, (long long)device_sm_count() * occ);
   k<<<(unsigned)grid, nthreads, smem, s>>>(a);
   FR_CUDA_TRY(cudaGetLastError());
 }
@@ -58,6 +58,7 @@ void panel_gemm_run(const PanelOp<T> &op, long long N, T c1, const T *B, long lo
   a.op = op;
   const long long pw = (long long)PV * op.NE;
   ColMap cm{pw, op.NE, op.NE, N};
+  a.prod = PlainProducer<T>();
   a.prod.src[0] = MatRef<T>{B, ldb, bsB};
   a.prod.src[1] = a.prod.src[0];
   a.prod.cm = cm;

@@ -25,38 +25,53 @@ struct PlainProducer {
   MatRef<T> src[2];
   ColMap cm;
   static constexpr bool kTransform = false;
-  __device__ __forceinline__ void issue(const ChunkDesc &cd, long long batch, long long pl, T *stage, int LDB, int NE, int tid,
-                                        int nthreads) const {
-    // Each thread owns one fixed 16-byte column piece (variable v, elements e..e+CTV) and walks down the rows, so the
-    // per-piece cost is two pointer bumps and the copy; the (v, e, first row) split of the thread index is done once per
-    // call with shifts (pieces per variable segment is a power of two).
+  // per-thread copy lane, fixed for the life of the CTA (init): each thread owns one 16-byte column piece (variable v,
+  // elements e..e+CTV) and walks down the rows, so a piece costs two pointer bumps and the copy
+  int l_sub, l_rpi, l_v, l_e, l_wide;
+  __device__ __forceinline__ void init(int NE, int tid, int nthreads) {
     constexpr int CTV = 16 / (int)sizeof(T);
     const int lg = 31 - __clz(NE / CTV);
     const int ppr = PV << lg;                         // pieces per row
-    const bool wide = nthreads >= ppr;                // the usual case: one sweep of the CTA covers >= 1 whole row
-    const int rpi = wide ? nthreads / ppr : 1;        // rows per sweep
-    const int sub = wide ? tid / ppr : 0;
-    if (sub >= rpi) return;
+    l_wide = nthreads >= ppr;                         // the usual case: one sweep of the group covers >= 1 whole row
+    l_rpi = l_wide ? nthreads / ppr : 1;              // rows per sweep
+    l_sub = l_wide ? tid / ppr : 0;
+    const int col = tid - l_sub * ppr;
+    l_v = col >> lg;
+    l_e = (col - (l_v << lg)) * CTV;
+  }
+  __device__ __forceinline__ void issue_col(const ChunkDesc &cd, long long batch, long long pl, T *stage, int LDB, int NE, int v,
+                                            int e) const {
+    constexpr int CTV = 16 / (int)sizeof(T);
+    long long nv = cm.lim - pl * cm.pstride - v * cm.vlim - e;
+    nv = nv < 0 ? 0 : (nv > CTV ? CTV : nv);
+    const int nbytes = (int)nv * (int)sizeof(T);
     const T *mp = cd.src ? src[1].p : src[0].p;
     const long long mld = cd.src ? src[1].ld : src[0].ld, mbs = cd.src ? src[1].bstride : src[0].bstride;
-    for (int col = tid - sub * ppr; col < ppr; col += wide ? ppr : nthreads) {
-      const int v = col >> lg, e = (col - (v << lg)) * CTV;
-      long long nv = cm.lim - pl * cm.pstride - v * cm.vlim - e;
-      nv = nv < 0 ? 0 : (nv > CTV ? CTV : nv);
-      const int nbytes = (int)nv * (int)sizeof(T);
-      const T *g = mp;
-      long long gstep = 0;
-      if (nv > 0) {
-        g = mp + batch * mbs + (long long)(cd.row0 + sub) * mld + pl * cm.pstride + v * cm.vstride + e;
-        gstep = (long long)rpi * mld;
-      }
-      T *sp = stage + sub * LDB + v * NE + e;
-      const int sstep = rpi * LDB;
-      for (int r = sub; r < cd.nrows; r += rpi) {
-        pcp_async16(sp, g, nbytes);
-        g += gstep;
-        sp += sstep;
-      }
+    const T *g = mp;
+    long long gstep = 0;
+    if (nv > 0) {
+      g = mp + batch * mbs + (long long)(cd.row0 + l_sub) * mld + pl * cm.pstride + v * cm.vstride + e;
+      gstep = (long long)l_rpi * mld;
+    }
+    T *sp = stage + l_sub * LDB + v * NE + e;
+    const int sstep = l_rpi * LDB;
+    for (int r = l_sub; r < cd.nrows; r += l_rpi) {
+      pcp_async16(sp, g, nbytes);
+      g += gstep;
+      sp += sstep;
+    }
+  }
+  __device__ __forceinline__ void issue(const ChunkDesc &cd, long long batch, long long pl, T *stage, int LDB, int NE, int tid,
+                                        int nthreads) const {
+    if (l_wide) {
+      if (l_sub < l_rpi) issue_col(cd, batch, pl, stage, LDB, NE, l_v, l_e);
+      return;
+    }
+    constexpr int CTV = 16 / (int)sizeof(T);
+    const int lg = 31 - __clz(NE / CTV);
+    for (int col = tid; col < (PV << lg); col += nthreads) {
+      const int v = col >> lg;
+      issue_col(cd, batch, pl, stage, LDB, NE, v, (col - (v << lg)) * CTV);
     }
   }
   __device__ __forceinline__ void transform(const ChunkDesc &, long long, long long, T *, int, int, int, int) const {}
@@ -110,36 +125,49 @@ struct PlainEpilogue {
 
 // ---- the persistent main loop.  Grid = any number of CTAs; CTA b owns panels b, b+grid, ...
 template <typename T, int NIT, int CX, class Prod, class Epi>
-__device__ __forceinline__ void panel_mainloop(const PanelOp<T> &op, const Prod &prod, const Epi &epi, long long npanels_per_batch,
+__device__ __forceinline__ void panel_mainloop(const PanelOp<T> &op, const Prod &prod_in, const Epi &epi, long long npanels_per_batch,
                                                int nbatch, char *smem) {
-  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  const int nthreads = blockDim.x;
-  const int WC = op.WC, NS = op.NS, NE = op.NE;
+  // A CTA holds NG (1 or 2) independent warp groups.  Each group owns its own accumulators, its own cp.async ring and its own
+  // stream of panels; they share only the operator image.  Group 1 starts half a panel late, so that one group's epilogue
+  // (global loads and stores, latency-bound) and chunk waits run under the other group's multiplies.
+  const int WC = op.WC, NS = op.NS, NE = op.NE, NG = op.NG;
+  const int nthreads = 32 * op.WR * WC;              // threads of one group
+  const int grp = threadIdx.x / nthreads;
+  const int tid = threadIdx.x - grp * nthreads, lane = tid & 31, warp = tid >> 5;
+  Prod prod(prod_in);
+  prod.init(NE, tid, nthreads);
   const int wr = warp / WC, wc = warp - wr * WC;
   const int LDB = PV * NE + 4;
   OpSmem<T> A;
   char *ringp = op_smem_carve(smem, op, A);
-  op_smem_load(smem, op, tid, nthreads);
+  op_smem_load(smem, op, threadIdx.x, blockDim.x);
   pcp_commit();
-  T *ring = reinterpret_cast<T *>(ringp);
   const size_t stage_elems = (size_t)op.stage_elems;
+  T *ring = reinterpret_cast<T *>(ringp) + (size_t)grp * PANEL_NSTAGE * stage_elems;
   const long long ntot = npanels_per_batch * nbatch;
-  const long long first = blockIdx.x, stride = gridDim.x;
+  const long long first = (long long)blockIdx.x * NG + grp, stride = (long long)gridDim.x * NG;
   const long long mine = first < ntot ? (ntot - first + stride - 1) / stride : 0;
   const int nchunks = op.nchunks;
   const long long total = mine * nchunks;
-  // two cursors over (panel, chunk): `iq` for the loads being issued, `cq` for the chunk being multiplied
-  long long ipanel = first, cpanel = first;
+  auto group_barrier = [&]() {
+    if (NG == 1) __syncthreads();
+    else asm volatile("bar.sync %0, %1;" ::"r"(1 + grp), "r"(nthreads) : "memory");
+  };
+  // two cursors over (panel, chunk): one for the loads being issued, one for the chunk being multiplied
+  long long ipl = first, cpl = first;
   int ic = 0, cc = 0, istage = 0, cstage = 0;
-  long long ibatch = ipanel / npanels_per_batch, ipl = ipanel - ibatch * npanels_per_batch;
-  long long cbatch = ibatch, cpl = ipl;
+  long long ibatch = ipl / npanels_per_batch;
+  ipl -= ibatch * npanels_per_batch;
+  long long cbatch = ibatch;
+  cpl = ipl;
+  bool image_ready = false;                          // the shared operator image (with the chunk table) has landed
   auto issue = [&]() {
-    const ChunkDesc cd = op.chunks[ic];              // global copy (the shared image may still be in flight)
+    // chunk table: from shared memory once it is there -- a global read here sits on the critical path of every chunk
+    const ChunkDesc cd = image_ready ? A.chunks[ic] : op.chunks[ic];
     prod.issue(cd, ibatch, ipl, ring + istage * stage_elems, LDB, NE, tid, nthreads);
     if (++istage == PANEL_NSTAGE) istage = 0;
     if (++ic == nchunks) {
       ic = 0;
-      ipanel += stride;
       ipl += stride;
       while (ipl >= npanels_per_batch) {
         ipl -= npanels_per_batch;
@@ -151,28 +179,40 @@ __device__ __forceinline__ void panel_mainloop(const PanelOp<T> &op, const Prod 
     if (q < total) issue();
     pcp_commit();
   }
+  // the operator image was copied by all threads of the CTA: everyone's share must have landed before anyone reads it
+  pcp_wait<PANEL_NSTAGE - 1>();
+  __syncthreads();
+  image_ready = true;
+  const long long stagger_q = total > 0 ? (nchunks / 2 < total ? nchunks / 2 : total - 1) : -1;
+  if (NG == 2) {
+    if (grp == 1) asm volatile("bar.sync 3, %0;" ::"r"(2 * nthreads) : "memory");
+    else if (stagger_q < 0) asm volatile("bar.arrive 3, %0;" ::"r"(2 * nthreads) : "memory");
+  }
   Acc<T, NIT, CX> acc;
   acc.zero();
   for (long long q = 0; q < total; ++q) {
     pcp_wait<PANEL_NSTAGE - 2>();
-    __syncthreads();
+    group_barrier();
     if (q + PANEL_NSTAGE - 1 < total) issue();
     pcp_commit();
     T *stage = ring + cstage * stage_elems;
     if (Prod::kTransform) {
       const ChunkDesc cd = A.chunks[cc];
-      if (cd.kind != KIND_PLAIN) {                   // uniform over the CTA
+      if (cd.kind != KIND_PLAIN) {                   // uniform over the group
         prod.transform(cd, cbatch, cpl, stage, LDB, NE, tid, nthreads);
-        __syncthreads();
+        group_barrier();
       }
     }
-    acc.mac_chunk(A, cc, NS, wr * NIT, stage, LDB, NE, wc, lane);
+    if (!(op.dbg & 1)) {
+      if (op.sparse) acc.mac_chunk(A, cc, NS, wr * NIT, stage, LDB, NE, wc, lane);
+      else acc.mac_dense(A, A.chunks[cc], NS, wr * NIT, stage, LDB, NE, wc, lane);
+    }
+    if (NG == 2 && grp == 0 && q == stagger_q) asm volatile("bar.arrive 3, %0;" ::"r"(2 * nthreads) : "memory");
     if (++cstage == PANEL_NSTAGE) cstage = 0;
     if (++cc == nchunks) {
-      epi(acc, A.rowmap, wr * NIT, cbatch, cpl, wc, lane);
+      if (!(op.dbg & 2)) epi(acc, A.rowmap, wr * NIT, cbatch, cpl, wc, lane);
       acc.zero();
       cc = 0;
-      cpanel += stride;
       cpl += stride;
       while (cpl >= npanels_per_batch) {
         cpl -= npanels_per_batch;
@@ -193,7 +233,7 @@ __device__ __forceinline__ void panel_mainloop(const PanelOp<T> &op, const Prod 
 
 template <typename T>
 inline size_t panel_smem_bytes(const PanelOp<T> &op) {
-  return op.smem_op + (size_t)PANEL_NSTAGE * op.stage_elems * sizeof(T) + 16;
+  return op.smem_op + (size_t)op.NG * PANEL_NSTAGE * op.stage_elems * sizeof(T) + 16;
 }
 
 // cp.async of `nrows` rows of a [rows][5][ld] state matrix into stage rows (pitch LDB, column v*NE + e); every thread owns a
