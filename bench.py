@@ -214,17 +214,42 @@ def _measure(case, prec, args, torch, dist, rank, world, with_e2e=True, sampler=
     return res
 
 
-def _roofline(kernels, peak, peak_src):
-    """Dominant kernel of one RHS by CUDA-event time; achieved = algorithmic bytes per launch / mean duration."""
+def _traffic(name, prec):
+    """DRAM bytes per launch of kernel `name` from the committed ncu --set full summary (profiles/r01_traffic.json), else None."""
+    try:
+        with open(os.path.join(ROOT, "profiles", "r01_traffic.json")) as f:
+            return json.load(f).get(prec, {}).get(name)
+    except Exception:
+        return None
+
+
+# arithmetic peaks measured on this pool's B200 with register-resident chains (profiles/r01_b_device_probes.md): FP64 on the
+# tensor pipe (DMMA m8n8k4) and FP32 FFMA.  The HBM peak comes from MEASURED_PEAKS.json.
+FLOP_PEAK = {"f64": (37.15, "tensor", "measured DMMA m8n8k4 chain, profiles/r01_b_device_probes.md"),
+             "f32": (72.4, "alu", "measured FFMA chain (fr_probe_peaks), profiles/r01_b_device_probes.md")}
+
+
+def _roofline(kernels, peak, peak_src, prec="f64"):
+    """Dominant kernel of one RHS by CUDA-event time.  Its bound is decided by its arithmetic intensity (dense flops over
+    algorithmic bytes) against the ridge of the measured peaks; achieved = algorithmic bytes (or flops) per launch / mean duration."""
     tot = sum(k["ms"] for k in kernels)
     top = max(kernels, key=lambda k: k["ms"])
-    ach = top["alg_bytes"] / (top["ms"] * 1e-3) / 1e9
+    sec = top["ms"] * 1e-3
+    gbs = top["alg_bytes"] / sec / 1e9
+    tfl = top["flops"] / sec / 1e12
+    fpeak, fbound, fsrc = FLOP_PEAK[prec]
+    ridge = fpeak * 1e12 / (peak * 1e9)
+    ai = top["flops"] / max(top["alg_bytes"], 1.0)
     whole = sum(k["alg_bytes"] for k in kernels) / (tot * 1e-3) / 1e9
-    return dict(bound="hbm", kernel=top["name"], achieved=ach, peak=peak, unit="GB/s", frac=ach / peak, traffic=None,
-                peak_source=peak_src, share_of_rhs=top["ms"] / tot, ms_per_launch=top["ms"],
-                alg_bytes_per_launch=top["alg_bytes"], tflops=top["flops"] / (top["ms"] * 1e-3) / 1e12,
-                whole_rhs=dict(alg_gbs=whole, frac=whole / peak, ms=tot,
-                               tflops=sum(k["flops"] for k in kernels) / (tot * 1e-3) / 1e12))
+    common = dict(kernel=top["name"], traffic=_traffic(top["name"], prec), share_of_rhs=top["ms"] / tot, ms_per_launch=top["ms"],
+                  alg_bytes_per_launch=top["alg_bytes"], flops_per_launch=top["flops"], intensity_flop_per_byte=ai, ridge=ridge,
+                  hbm=dict(achieved=gbs, peak=peak, unit="GB/s", frac=gbs / peak, peak_source=peak_src),
+                  flop=dict(achieved=tfl, peak=fpeak, unit="TFLOP/s", frac=tfl / fpeak, peak_source=fsrc),
+                  whole_rhs=dict(alg_gbs=whole, frac=whole / peak, ms=tot,
+                                 tflops=sum(k["flops"] for k in kernels) / (tot * 1e-3) / 1e12))
+    if ai > ridge:
+        return dict(bound=fbound, achieved=tfl, peak=fpeak, unit="TFLOP/s", frac=tfl / fpeak, peak_source=fsrc, **common)
+    return dict(bound="hbm", achieved=gbs, peak=peak, unit="GB/s", frac=gbs / peak, peak_source=peak_src, **common)
 
 
 def run_frb200(args):
@@ -265,7 +290,7 @@ def run_frb200(args):
                     roofline=_roofline(r64["kernels"], peak, peak_src), cpu_baseline=cpu, finite=r64["finite"],
                     fp32=dict(value=r32["value"], unit="GDOF-RHS/s", ms_per_step=1e3 * r32["seconds"] / args.steps,
                               dtype="f32", gpu_launches=r32["launches"], finite=r32["finite"],
-                              roofline=_roofline(r32["kernels"], peak, peak_src)))
+                              roofline=_roofline(r32["kernels"], peak, peak_src, "f32")))
         if args.kernels:
             line["kernels_f64"] = r64["kernels"]
             line["kernels_f32"] = r32["kernels"]

@@ -491,6 +491,7 @@ __device__ __forceinline__ void pcp_async16(void *smem, const void *gmem, int sr
   unsigned s = (unsigned)__cvta_generic_to_shared(smem);
   asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;\n" ::"r"(s), "l"(gmem), "r"(src_bytes));
 }
+__device__ __forceinline__ void prefetch_l2(const void *p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
 __device__ __forceinline__ void pcp_commit() { asm volatile("cp.async.commit_group;\n" ::); }
 template <int N>
 __device__ __forceinline__ void pcp_wait() {
@@ -659,6 +660,14 @@ struct Acc<double, NIT, CX> {
 #pragma unroll
       for (int cb = 0; cb < CX; ++cb) f(i, 0, wc * 8 * CX + cb * 8 + 2 * (lane & 3), c[i][cb]);
   }
+  // f(i, rr, e): coordinates only (for prefetching what the epilogue will read)
+  template <typename F>
+  __device__ __forceinline__ void foreach_coord(int wc, int lane, F &&f) {
+#pragma unroll
+    for (int i = 0; i < NIT; ++i)
+#pragma unroll
+      for (int cb = 0; cb < CX; ++cb) f(i, 0, wc * 8 * CX + cb * 8 + 2 * (lane & 3));
+  }
   // f(t, rr, e, tile_a0, tile_a1, tile_a2): slots 3t, 3t+1, 3t+2 hold the three alpha of the same rows
   template <typename F>
   __device__ __forceinline__ void foreach_triple(int wc, int lane, F &&f) {
@@ -770,6 +779,13 @@ struct Acc<float, NIT, CX> {
     for (int i = 0; i < NIT; ++i)
 #pragma unroll
       for (int r = 0; r < 8; ++r) f(i, r, wc * 32 * CX + lane * CX, c[i][r]);
+  }
+  template <typename F>
+  __device__ __forceinline__ void foreach_coord(int wc, int lane, F &&f) {
+#pragma unroll
+    for (int i = 0; i < NIT; ++i)
+#pragma unroll
+      for (int r = 0; r < 8; ++r) f(i, r, wc * 32 * CX + lane * CX);
   }
   template <typename F>
   __device__ __forceinline__ void foreach_triple(int wc, int lane, F &&f) {

@@ -49,6 +49,23 @@ struct RkEpilogue {
   int curved, NE;
   StageArgs<T> sa;
   template <typename ACC>
+  __device__ __forceinline__ void prefetch(ACC &acc, const int *rowmap, int slot0, long long, long long pl, int wc, int lane) const {
+    const long long e0 = pl * NE;
+    acc.foreach_coord(wc, lane, [&](int i, int rr, int e) {
+      const int m = rowmap[(slot0 + i) * 8 + (ACC::ROWS == 1 ? (lane >> 2) : rr)];
+      if (m < 0) return;
+      const long long col = e0 + e;
+      if (curved || i == 0) prefetch_l2(rcpdjac + (curved ? (long long)m * ld : 0) + col);
+      if (!sa.coef) return;
+#pragma unroll
+      for (int v = 0; v < PV; ++v) {
+        const long long idx = ((long long)m * 5 + v) * ld + col;
+        prefetch_l2(sa.in1 + idx);
+        if (sa.out2 && sa.in2 != sa.in1) prefetch_l2(sa.in2 + idx);
+      }
+    });
+  }
+  template <typename ACC>
   __device__ __forceinline__ void operator()(ACC &acc, const int *rowmap, int slot0, long long, long long pl, int wc, int lane) const {
     constexpr int EW = ACC::EW;
     const long long e0 = pl * NE;
@@ -81,7 +98,12 @@ struct RkEpilogue {
           VecIO<T, EW>::ld(sa.in1 + idx, a);
           if (sa.out2) {
             T b[EW], o2[EW];
-            VecIO<T, EW>::ld(sa.in2 + idx, b);
+            if (sa.in2 != sa.in1) {
+              VecIO<T, EW>::ld(sa.in2 + idx, b);
+            } else {
+#pragma unroll
+              for (int j = 0; j < EW; ++j) b[j] = a[j];
+            }
 #pragma unroll
             for (int j = 0; j < EW; ++j) o2[j] = live[j] ? b[j] + c2 * k[j] : T(0);
             VecIO<T, EW>::st(sa.out2 + idx, o2);
@@ -120,6 +142,19 @@ struct GradEpilogue {
   PhysParams<T> ph;
   long long ld, neles;
   int nupts, curved, NE;
+  template <typename ACC>
+  __device__ __forceinline__ void prefetch(ACC &acc, const int *rowmap, int slot0, long long, long long pl, int wc, int lane) const {
+    const long long e0 = pl * NE;
+    acc.foreach_coord(wc, lane, [&](int i, int rr, int e) {
+      if (i % 3 != 0) return;
+      const int rho = rowmap[(slot0 + i) * 8 + (ACC::ROWS == 1 ? (lane >> 2) : rr)];
+      if (rho < 0 || (!curved && i != 0)) return;
+      const long long col = e0 + e;
+      prefetch_l2(rcpdjac + (curved ? (long long)rho * ld : 0) + col);
+#pragma unroll
+      for (int a = 0; a < 9; ++a) prefetch_l2(smats + (curved ? ((long long)a * nupts + rho) * ld : (long long)a * ld) + col);
+    });
+  }
   template <typename ACC>
   __device__ __forceinline__ void operator()(ACC &acc, const int *rowmap, int slot0, long long, long long pl, int wc, int lane) const {
     constexpr int EW = ACC::EW;

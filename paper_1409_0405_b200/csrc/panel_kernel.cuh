@@ -85,6 +85,19 @@ struct PlainEpilogue {
   ColMap cm;
   T c1, c2;
   template <typename ACC>
+  __device__ __forceinline__ void prefetch(ACC &acc, const int *rowmap, int slot0, long long batch, long long pl, int wc,
+                                           int lane) const {
+    if (c2 == T(0)) return;
+    const T *Cb = C + batch * bstride + pl * cm.pstride;
+    acc.foreach_coord(wc, lane, [&](int i, int rr, int e) {
+      const int m = rowmap[(slot0 + i) * 8 + (ACC::ROWS == 1 ? (lane >> 2) : rr)];
+      if (m < 0) return;
+#pragma unroll
+      for (int v = 0; v < PV; ++v)
+        if (pl * cm.pstride + v * cm.vlim + e < cm.lim) prefetch_l2(Cb + (long long)m * ldc + v * cm.vstride + e);
+    });
+  }
+  template <typename ACC>
   __device__ __forceinline__ void operator()(ACC &acc, const int *rowmap, int slot0, long long batch, long long pl, int wc,
                                              int lane) const {
     T *Cb = C + batch * bstride + pl * cm.pstride;
@@ -203,6 +216,8 @@ __device__ __forceinline__ void panel_mainloop(const PanelOp<T> &op, const Prod 
         group_barrier();
       }
     }
+    // the epilogue's own global operands: pull them into L2 while the last chunk is multiplied
+    if (cc == nchunks - 1 && !(op.dbg & 4)) epi.prefetch(acc, A.rowmap, wr * NIT, cbatch, cpl, wc, lane);
     if (!(op.dbg & 1)) {
       if (op.sparse) acc.mac_chunk(A, cc, NS, wr * NIT, stage, LDB, NE, wc, lane);
       else acc.mac_dense(A, A.chunks[cc], NS, wr * NIT, stage, LDB, NE, wc, lane);

@@ -14,9 +14,19 @@ from fr_inputs import refelem as R
 
 CASES = [(t, p) for t in ("tet", "pri", "hex") for p in (1, 2, 3, 4)]
 # Table 2, PAPER.md:43-50 ("dim M0", printed as N_u x N_f; reading R1: M0 is N_f x N_u)
-TABLE2 = {("tet", 1): (4, 12), ("tet", 2): (10, 24), ("tet", 3): (20, 40), ("tet", 4): (35, 60),
-          ("pri", 1): (6, 18), ("pri", 2): (18, 39), ("pri", 3): (40, 68), ("pri", 4): (75, 105),
-          ("hex", 1): (8, 24), ("hex", 2): (27, 54), ("hex", 3): (64, 96), ("hex", 4): (125, 150)}
+def _load_table2():
+    """Table 2 of the paper, kept as a cited text fixture."""
+    import os
+    out = {}
+    with open(os.path.join(os.path.dirname(__file__), "golden", "table2_m0_dims.txt")) as f:
+        for line in f:
+            if line.strip() and not line.startswith("#"):
+                t, p_, nu, nf = line.split()
+                out[(t, int(p_))] = (int(nu), int(nf))
+    return out
+
+
+TABLE2 = _load_table2()
 
 
 def _space(etype, p):
