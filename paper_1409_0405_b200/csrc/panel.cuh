@@ -30,6 +30,10 @@ namespace frb {
 constexpr int PV = FR_NVAR;          // variable segments per panel
 constexpr int PANEL_MAXW = 16;       // warps per CTA (upper bound; 8 when the accumulators need > 128 registers)
 constexpr int PANEL_MAXCHUNKS = 64;
+#ifndef FRB_NSTAGE
+#define FRB_NSTAGE 2
+#endif
+constexpr int PANEL_NSTAGE = FRB_NSTAGE;   // cp.async ring depth: 2 beats 3 and 4 on config 3 (taller chunks, fewer barriers; profiles/r01_c_fusion_notes.md)
 
 // One K-chunk of the stacked right-hand operand: rows [row0, row0+nrows) of source `src`.
 struct ChunkDesc {
@@ -438,10 +442,10 @@ bool panel_op_build_kc(PanelOp<T> &p, int M, int K, const double *A, const std::
   const int LDBh = PV * geo.NE + 4;
   for (auto &c : chunks)
     stage_elems = std::max(stage_elems, c.kind == KIND_FLUX ? flux_stage_elems(c.nrows, geo.NE, LDBh, opt.curved) : (size_t)c.nrows * LDBh);
-  if (smem_op + (size_t)geo.NG * 3 * stage_elems * sizeof(T) + 16 > smem_total) {
+  if (smem_op + (size_t)geo.NG * PANEL_NSTAGE * stage_elems * sizeof(T) + 16 > smem_total) {
     // MAC rows per chunk that would fit: scale the tallest chunk down proportionally (flux chunks carry 4/3 rows + metrics)
     if (smem_total > smem_op + 4096) {
-      const double room = (double)(smem_total - smem_op - 1024) / (3.0 * geo.NG * sizeof(T));
+      const double room = (double)(smem_total - smem_op - 1024) / ((double)PANEL_NSTAGE * geo.NG * sizeof(T));
       *kc_fit = (int)(kcmax * room / (double)stage_elems);
     }
     return false;

@@ -4,7 +4,6 @@
 
 namespace frb {
 
-constexpr int PANEL_NSTAGE = 3;
 
 // Where a panel's columns live in a global matrix: column(v, e) = p*pstride + v*vstride + e, valid iff
 // p*pstride + v*vlim + e < lim.  State matrices [rows][5][ld]: pstride = NE, vstride = ld, vlim = 0, lim = ld.
