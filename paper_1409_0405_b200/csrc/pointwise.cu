@@ -143,6 +143,16 @@ __global__ void __launch_bounds__(PW_BLOCK) k_con_u(IfaceView<T> iv, const __gri
   side_addr<T>(tt, pr.le, pr.lts, ul, gl, ldl, gcl);
   side_addr<T>(tt, pr.re, pr.rts, ur, gr, ldr, gcr);
   const T wl = T(0.5) - beta, wr = T(0.5) + beta;
+  if (wl == T(0)) {
+    // beta = 1/2 (the default, reading R9): C = u_R on both sides, the L state is not needed
+#pragma unroll
+    for (int v = 0; v < 5; ++v) {
+      const T c = wr * uf[ur + v * ldr];
+      cf[ul + v * ldl] = c;
+      cf[ur + v * ldr] = c;
+    }
+    return;
+  }
 #pragma unroll
   for (int v = 0; v < 5; ++v) {
     const T c = wl * uf[ul + v * ldl] + wr * uf[ur + v * ldr];
