@@ -56,3 +56,70 @@ def gpu_rhs(ctx, us):
     torch.cuda.synchronize()
     raw = [t.cpu().numpy().astype(np.float64) for t in d_out]
     return [r[:, :, :u.shape[2]] for r, u in zip(raw, us)], raw
+
+
+def subcase(case, seeds, rings=2):
+    """Cut the `rings`-neighbourhood of the seed elements out of a case (same dict layout, elements renumbered).
+    seeds: per element type an int array of element ids.  Returns (sub-case, per type the positions of the seeds in it).
+    The right-hand side at an element depends on its neighbours (common flux) and, for Navier-Stokes, on their neighbours
+    (their gradients need their common solution), so with rings = 2 the oracle evaluated on the sub-case reproduces the
+    full-mesh values at the seeds exactly; flux points on the cut are simply left unpaired."""
+    ifc = case["ifc"]
+    nt = len(case["eles"])
+    inset = [np.zeros(e["neles"], dtype=bool) for e in case["eles"]]
+    for t in range(nt):
+        inset[t][np.asarray(seeds[t], dtype=np.int64)] = True
+    for _ in range(rings):
+        lin = np.zeros(len(ifc["l_et"]), dtype=bool)
+        rin = np.zeros(len(ifc["l_et"]), dtype=bool)
+        for t in range(nt):
+            ml, mr = ifc["l_et"] == t, ifc["r_et"] == t
+            lin[ml] = inset[t][ifc["l_ele"][ml]]
+            rin[mr] = inset[t][ifc["r_ele"][mr]]
+        touch = lin | rin
+        for t in range(nt):
+            ml, mr = touch & (ifc["l_et"] == t), touch & (ifc["r_et"] == t)
+            inset[t][ifc["l_ele"][ml]] = True
+            inset[t][ifc["r_ele"][mr]] = True
+    ids = [np.flatnonzero(m) for m in inset]
+    remap = [np.full(len(m), -1, dtype=np.int64) for m in inset]
+    for t in range(nt):
+        remap[t][ids[t]] = np.arange(len(ids[t]))
+    sub = dict(cfg=case["cfg"], etypes=case["etypes"], order=case["order"], eles=[], bcs=[])
+    for t, e in enumerate(case["eles"]):
+        e2 = dict(e)
+        e2["neles"] = len(ids[t])
+        for k in ("smats", "rcpdjac", "djac"):
+            e2[k] = np.ascontiguousarray(e[k][..., ids[t]])
+        e2["xu"] = np.ascontiguousarray(e["xu"][:, ids[t], :])
+        sub["eles"].append(e2)
+    keep = np.ones(len(ifc["l_et"]), dtype=bool)
+    for t in range(nt):
+        ml, mr = ifc["l_et"] == t, ifc["r_et"] == t
+        keep[ml] &= inset[t][ifc["l_ele"][ml]]
+        keep[mr] &= inset[t][ifc["r_ele"][mr]]
+    s = {k: (v[keep] if v.ndim == 1 else v[:, keep]) for k, v in ifc.items()}
+    for side in ("l", "r"):
+        ne = s[side + "_ele"].copy()
+        for t in range(nt):
+            m = s[side + "_et"] == t
+            ne[m] = remap[t][s[side + "_ele"][m]]
+        s[side + "_ele"] = ne
+    sub["ifc"] = s
+    for b in case["bcs"]:
+        kb = np.zeros(len(b["et"]), dtype=bool)
+        for t in range(nt):
+            m = b["et"] == t
+            kb[m] = inset[t][b["ele"][m]]
+        b2 = dict(b)
+        for k in ("et", "fpt", "ele", "mag"):
+            b2[k] = b[k][kb]
+        b2["n"] = b["n"][:, kb]
+        ne = b2["ele"].copy()
+        for t in range(nt):
+            m = b2["et"] == t
+            ne[m] = remap[t][b2["ele"][m]]
+        b2["ele"] = ne
+        sub["bcs"].append(b2)
+    sub["u0"] = [np.ascontiguousarray(u[:, :, ids[t]]) for t, u in enumerate(case["u0"])]
+    return sub, [remap[t][np.asarray(seeds[t], dtype=np.int64)] for t in range(nt)]

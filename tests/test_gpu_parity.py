@@ -168,3 +168,70 @@ def test_setup_rejects_bad_input():
     bad["eles"][0]["nupts"] = 11
     with pytest.raises(FrError):
         Context(bad)
+
+
+# ---------------------------------------------------------------------------- T5: design order on the isentropic vortex (config 2 sweep)
+@pytest.mark.parametrize("p,ns_,min_order", [(2, (8, 16), 2.2), (3, (16, 32), 3.6)])
+def test_T5_vortex_convergence_order_on_gpu(p, ns_, min_order):
+    """BASELINE.json configs[1]: "a convergence-order sweep on 8^3/16^3/32^3".  Euler (mu = 0), RK4 through fr_rk_run with a time step
+    small enough that the temporal error is negligible, quadrature-weighted L2 error of the density against the exact solution (the
+    vortex translated by v_inf t).  Observed on B200: 2.40 / 2.36 for p = 2 (8->16->32, pre-asymptotic: the vortex radius is 0.1) and
+    3.46 / 4.05 for p = 3; design order is p + 1."""
+    errs = []
+    for n in ns_:
+        case = cases.config2(n, p, "euler")
+        ctx = _ctx(case, "f64", stepper="rk4")
+        ctx.set_state(case["u0"])
+        dt = 1.25e-4 * 16 / n
+        nsteps = int(round(0.05 / dt))
+        ctx.rk_run(dt, nsteps)
+        ctx.sync()
+        us = ctx.get_state()
+        ctx.close()
+        num = 0.0
+        for e, u in zip(case["eles"], us):
+            ex = state.isentropic_vortex(e["xu"], t=nsteps * dt)
+            w = e["wts"][:, None] * e["djac"]
+            num += (w * (u[:, 0, :] - ex[:, 0, :]) ** 2).sum()
+        errs.append(np.sqrt(num))
+    order = np.log2(errs[0] / errs[1])
+    assert order >= min_order, (errs, order)
+
+
+# ---------------------------------------------------------------------------- full-size parity on sampled elements (bench configuration)
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+def test_config3_full_size_sampled_parity(prec):
+    """BASELINE.json configs[2] at the size and launch configuration bench.py times (120 000 prisms + 360 000 tets, p = 4, NS,
+    boundaries): the GPU right-hand side of the whole mesh against the oracle evaluated on the two-ring neighbourhoods of sampled
+    elements (tests/gpu_util.subcase), which reproduces the full-mesh values at those elements.  Samples: seeded random interior
+    elements of both types plus elements on the wall and on the far-field boundary; the first and last element of each type
+    (ragged tail of the last panel) are always included."""
+    from gpu_util import subcase
+    case = cases.config3()
+    rng = np.random.Generator(np.random.PCG64(cases.SEEDS["c3"] + 1))
+    seeds = []
+    for t, e in enumerate(case["eles"]):
+        s = list(rng.integers(0, e["neles"], 24)) + [0, e["neles"] - 1]
+        for b in case["bcs"]:
+            on = b["ele"][b["et"] == t]
+            if len(on):
+                s += list(rng.choice(on, 6))
+        seeds.append(np.unique(np.array(s, dtype=np.int64)))
+    sub, pos = subcase(case, seeds, rings=2)
+    c = round_case_to_f32(sub) if prec == "f32" else sub
+    ref, amp = oracle_rhs_with_amplification(c)
+    ctx = _ctx(case, prec)
+    got, raw = gpu_rhs(ctx, case["u0"])
+    ctx.close()
+    g = [got[t][:, :, seeds[t]] for t in range(len(seeds))]
+    r = [ref[t][:, :, pos[t]] for t in range(len(seeds))]
+    assert all(np.isfinite(x).all() for x in got)
+    err, den = field_errors(g, r)
+    # normalise by the global max of the oracle over the sub-case (reading R16 on the sampled neighbourhood)
+    den_all = np.zeros(5)
+    for x in ref:
+        den_all = np.maximum(den_all, np.abs(x).max(axis=(0, 2)))
+    err = err * den / den_all
+    assert np.all(err <= _tolerance(prec, amp)), (prec, err, _tolerance(prec, amp))
+    for rr, u in zip(raw, case["u0"]):
+        assert np.all(rr[:, :, u.shape[2]:] == 0)
