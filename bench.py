@@ -143,6 +143,20 @@ def run_reference(args):
 
 
 # ------------------------------------------------------------------------------------------------ CUDA arm
+def max_over_ranks(seconds, world, dist, torch, device):
+    """Replicas only: every rank times the same work on its own GPU; the job's time is the slowest rank's."""
+    if world <= 1:
+        return seconds
+    t = torch.tensor([seconds], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def aggregate_rate(ndof, rhs_per_step, steps, seconds, world):
+    """Whole-job GDOF-RHS/s: the units all `world` replicas processed over the max-over-ranks time."""
+    return world * ndof * rhs_per_step * steps / seconds / 1e9
+
+
 def _time_steps(ctx, stream, dt, steps, torch):
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     e0.record(stream)
@@ -171,12 +185,9 @@ def _measure(case, prec, args, torch, dist, rank, world, with_e2e=True, sampler=
     torch.cuda.synchronize()
     clocks = sampler.stop() if sampler is not None else None
     launches = ctx.launch_count() - n0
-    if world > 1:
-        t = torch.tensor([sec], dtype=torch.float64, device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        sec = float(t.item())
+    sec = max_over_ranks(sec, world, dist, torch, "cuda")
     nstage = 5
-    res = dict(seconds=sec, value=world * ndof * nstage * args.steps / sec / 1e9, launches=launches, clocks=clocks,
+    res = dict(seconds=sec, value=aggregate_rate(ndof, nstage, args.steps, sec, world), launches=launches, clocks=clocks,
                ndof=ndof)
     # state must still be finite after the timed steps (a blown-up run would be timing NaN arithmetic)
     chk = ctx.get_state()
@@ -203,12 +214,9 @@ def _measure(case, prec, args, torch, dist, rank, world, with_e2e=True, sampler=
             ctx.rk_step_host(DT, ptrs)
         torch.cuda.synchronize()
         t1 = time.perf_counter() - t0
-        if world > 1:
-            t = torch.tensor([t1], dtype=torch.float64, device="cuda")
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            t1 = float(t.item())
+        t1 = max_over_ranks(t1, world, dist, torch, "cuda")
         nb = int(sum(h.numel() * h.element_size() for h in hbuf))
-        res["e2e"] = dict(value=world * ndof * nstage * ne2e / t1 / 1e9, unit="GDOF-RHS/s", h2d_bytes_per_step=nb,
+        res["e2e"] = dict(value=aggregate_rate(ndof, nstage, ne2e, t1, world), unit="GDOF-RHS/s", h2d_bytes_per_step=nb,
                           d2h_bytes_per_step=nb, steps=ne2e)
     ctx.close()
     return res

@@ -236,9 +236,86 @@ struct Ctx : CtxBase {
       gf.alloc(gtot);
     }
     build_views(c);
+    if (mode == FR_MODE_FUSED) autotune(c);
     coef.alloc(8);
     FR_CUDA_TRY(cudaMallocHost(&coef_host, 8 * sizeof(StageCoef)));
     FR_CUDA_TRY(cudaDeviceSynchronize());
+  }
+
+  // ------------------------------------------------------------------ geometry autotuning
+  // The static score of choose_geom ranks the (warps x row groups x column blocks x warp groups) candidates of an operator;
+  // which one is fastest depends on things it does not model (register allocation, barrier skew, epilogue latency).  For
+  // meshes large enough to time reliably, fr_setup launches the first kTuneCands candidates on the context's own arrays and
+  // keeps the fastest.  Results do not depend on the choice (the summation order over k is the same for every geometry).
+  static constexpr int kTuneCands = 10;
+  static constexpr long long kTuneMinEles = 16384;
+  template <typename B, typename L>
+  void tune(PanelOp<T> &cur, B build, L launch, const char *what) {
+    if (!cur.ok()) return;
+    cudaEvent_t e0, e1;
+    FR_CUDA_TRY(cudaEventCreate(&e0));
+    FR_CUDA_TRY(cudaEventCreate(&e1));
+    auto time_op = [&](const PanelOp<T> &op) {
+      launch(op);
+      cudaEventRecord(e0, stream);
+      launch(op);
+      launch(op);
+      cudaEventRecord(e1, stream);
+      FR_CUDA_TRY(cudaEventSynchronize(e1));
+      float ms = 0;
+      cudaEventElapsedTime(&ms, e0, e1);
+      return ms * 0.5f;
+    };
+    PanelOp<T> best = cur;
+    float bt = time_op(best);
+    const bool verbose = getenv("FRB_PANEL_VERBOSE") != nullptr;
+    if (verbose) fprintf(stderr, "autotune %s cand 0: %.3f ms\n", what, bt);
+    for (int k = 1; k < kTuneCands; ++k) {
+      PanelOp<T> op;
+      if (!build(op, k)) break;
+      const float t = time_op(op);
+      if (verbose) fprintf(stderr, "autotune %s cand %d: %.3f ms\n", what, k, t);
+      if (t < bt) {
+        panel_op_free(best);
+        best = op;
+        bt = t;
+      } else {
+        panel_op_free(op);
+      }
+    }
+    cur = best;
+    cudaEventDestroy(e0);
+    cudaEventDestroy(e1);
+  }
+
+  void autotune(const fr_config *c) {
+    const char *env = getenv("FRB_AUTOTUNE");
+    if (env && atoi(env) == 0) return;
+    const bool ns = ph.ns;
+    for (int t = 0; t < nt; ++t) {
+      EleData<T> &e = *el[t];
+      if (e.view.neles < kTuneMinEles) continue;
+      const fr_eles_desc &d = c->eles[t];
+      const int nu = e.view.nupts, nf = e.view.nfpts;
+      const long long n5 = 5 * e.view.ld;
+      T *ufp = uf.p + tt.ubase[t];
+      std::string tag = std::string(tname[t]);
+      if (e.pM0.pop)
+        tune(*e.pM0.pop, [&](PanelOp<T> &op, int k) { return panel_gemm_build(op, nf, nu, d.M0, k); },
+             [&](const PanelOp<T> &op) { panel_gemm_run(op, n5, T(1), (const T *)e.X.p, n5, 0, T(0), ufp, n5, 0, 1, stream); },
+             (tag + ":M0").c_str());
+      StageArgs<T> plain{nullptr, nullptr, nullptr, e.R.p, nullptr};
+      tune(e.pDiv, [&](PanelOp<T> &op, int k) { return fused_div_build(op, nu, nf, d.M132, d.M3, k); },
+           [&](const PanelOp<T> &op) { launch_fused_div(op, e.view, (const T *)e.grad.p, (const T *)ufp, plain, stream); },
+           (tag + ":[M132|M3]").c_str());
+      if (ns)
+        tune(e.pGrad, [&](PanelOp<T> &op, int k) { return fused_grad_build(op, nu, nf, d.M460, d.M6, k); },
+             [&](const PanelOp<T> &op) {
+               launch_fused_grad(op, e.view, (const T *)e.X.p, (const T *)(cf.p + tt.ubase[t]), e.grad.p, (T *)nullptr, ph, stream);
+             },
+             (tag + ":[M460|M6]").c_str());
+    }
+    FR_CUDA_TRY(cudaStreamSynchronize(stream));
   }
 
   void build_views(const fr_config *c) {

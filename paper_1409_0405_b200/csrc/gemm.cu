@@ -19,7 +19,7 @@
 namespace frb {
 
 template <typename T>
-bool panel_gemm_build(PanelOp<T> &op, int M, int K, const double *A);
+bool panel_gemm_build(PanelOp<T> &op, int M, int K, const double *A, int cand = 0);
 template <typename T>
 void panel_gemm_run(const PanelOp<T> &op, long long N, T c1, const T *B, long long ldb, long long bsB, T c2, T *C,
                     long long ldc, long long bsC, int nbatch, cudaStream_t s);

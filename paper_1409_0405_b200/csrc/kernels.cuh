@@ -60,14 +60,21 @@ int launch_bc_comm_flux(const BndView<T> &bv, const TypeTab &tt, T *uf, const T 
 
 // Fused panel kernels (panel_fused.cu).  *_build return false if the operator does not fit the resident design.
 template <typename T>
-bool fused_div_build(PanelOp<T> &op, int nu, int nf, const double *M132, const double *M3);
+bool fused_div_build(PanelOp<T> &op, int nu, int nf, const double *M132, const double *M3, int cand = 0);
 template <typename T>
 int launch_fused_div(const PanelOp<T> &op, const EleView<T> &ev, const T *ftil, const T *d, const StageArgs<T> &sa,
                      cudaStream_t s);
 template <typename T>
-bool fused_grad_build(PanelOp<T> &op, int nu, int nf, const double *M460, const double *M6);
+bool fused_grad_build(PanelOp<T> &op, int nu, int nf, const double *M460, const double *M6, int cand = 0);
 template <typename T>
 int launch_fused_grad(const PanelOp<T> &op, const EleView<T> &ev, const T *u, const T *c, T *grad, T *ftil,
                       const PhysParams<T> &ph, cudaStream_t s);
+
+// Plain operator product on the panel kernels (panel_gemm.cu); `cand` as above.
+template <typename T>
+bool panel_gemm_build(PanelOp<T> &op, int M, int K, const double *A, int cand = 0);
+template <typename T>
+void panel_gemm_run(const PanelOp<T> &op, long long N, T c1, const T *B, long long ldb, long long bsB, T c2, T *C,
+                    long long ldc, long long bsC, int nbatch, cudaStream_t s);
 
 }  // namespace frb

@@ -110,8 +110,8 @@ constexpr int panel_maxw(int nit, int cx) {
 // Choose the warp grid for G row groups.  The FP64 tensor pipe takes one DMMA per warp every ~32 cycles, so two warps per
 // scheduler saturate it only if they do nothing else: prefer 12-16 warps per SM.
 template <typename T>
-inline PanelGeom choose_geom(int G, int min_ne, int max_ne, int triple, bool dense) {
-  PanelGeom best{0, 0, 0, 0, 0, -1.0, 1};
+inline std::vector<PanelGeom> list_geoms(int G, int min_ne, int max_ne, int triple, bool dense) {
+  std::vector<PanelGeom> all;
   const bool f64 = sizeof(T) == 8;
   const int gu = triple ? 3 : 1;            // groups come in units of `gu` that must stay on one row-warp
   const int GU = (G + gu - 1) / gu;
@@ -135,11 +135,20 @@ inline PanelGeom choose_geom(int G, int min_ne, int max_ne, int triple, bool den
           if (dense) score /= 1.0 + 0.4 * (2.0 / nit + 0.4 / CX);
           // two staggered warp groups hide one group's epilogue and load waits behind the other's multiplies
           if (NG == 2) score *= 1.25;
-          if (score > best.eff) best = PanelGeom{WR, WC, nit, CX, NE, score, NG};
+          all.push_back(PanelGeom{WR, WC, nit, CX, NE, score, NG});
         }
       }
     }
-  return best;
+  std::stable_sort(all.begin(), all.end(), [](const PanelGeom &x, const PanelGeom &y) { return x.eff > y.eff; });
+  return all;
+}
+
+// Best geometry by the static score; fr_setup may instead time the first few candidates on the real arrays (PackOptions::cand).
+template <typename T>
+inline PanelGeom choose_geom(int G, int min_ne, int max_ne, int triple, bool dense, int cand = 0) {
+  const std::vector<PanelGeom> all = list_geoms<T>(G, min_ne, max_ne, triple, dense);
+  if (cand < 0 || cand >= (int)all.size()) return PanelGeom{0, 0, 0, 0, 0, -1.0, 1};
+  return all[cand];
 }
 
 // Greedy clustering of rows into groups of 8 with similar column support (sparse operators only).
@@ -191,6 +200,7 @@ struct PackOptions {
   int kc = 0;              // rows per chunk (0 = default)
   int allow_sparse = 1;
   int curved = 0;          // flux sources: per-point metric terms
+  int cand = 0;            // k-th best geometry by static score (autotuning)
 };
 
 // Pack A (M x K, host FP64, row-major) for the panel kernels.  `srcs` stacks the K dimension.  Returns false if the
@@ -327,7 +337,7 @@ bool panel_op_build_kc(PanelOp<T> &p, int M, int K, const double *A, const std::
       const int n = (int)lists[g][c].size();
       gcost[g] += f64 ? (n + 3) / 4 * 4 : n;
     }
-  PanelGeom geo = choose_geom<T>(G, opt.min_ne, opt.max_ne, opt.triple, !sparse);
+  PanelGeom geo = choose_geom<T>(G, opt.min_ne, opt.max_ne, opt.triple, !sparse, opt.cand);
   if (geo.eff < 0) return false;
   const int WR = geo.WR, NIT = geo.NIT, NS = WR * NIT;
   // LPT assignment of group units (1 or 3 groups) to row-warps, at most NIT groups per row-warp

@@ -281,7 +281,7 @@ void launch_panel(K k, const A &a, int nthreads, size_t smem, long long ntot, in
 }  // namespace
 
 template <typename T>
-bool fused_div_build(PanelOp<T> &op, int nu, int nf, const double *M132, const double *M3) {
+bool fused_div_build(PanelOp<T> &op, int nu, int nf, const double *M132, const double *M3, int cand) {
   const int K = 3 * nu + nf;
   std::vector<double> A((size_t)nu * K);
   for (int m = 0; m < nu; ++m) {
@@ -292,6 +292,7 @@ bool fused_div_build(PanelOp<T> &op, int nu, int nf, const double *M132, const d
   PackOptions opt;
   opt.min_ne = 16;
   opt.max_ne = 64;
+  opt.cand = cand;
   return panel_op_build(op, nu, K, A.data(), srcs, opt, 150 * 1024);
 }
 
@@ -323,7 +324,7 @@ int launch_fused_div(const PanelOp<T> &op, const EleView<T> &ev, const T *ftil, 
 }
 
 template <typename T>
-bool fused_grad_build(PanelOp<T> &op, int nu, int nf, const double *M460, const double *M6) {
+bool fused_grad_build(PanelOp<T> &op, int nu, int nf, const double *M460, const double *M6, int cand) {
   const int K = nu + nf, M = 3 * nu;
   std::vector<double> A((size_t)M * K);
   for (int m = 0; m < M; ++m) {
@@ -335,6 +336,7 @@ bool fused_grad_build(PanelOp<T> &op, int nu, int nf, const double *M460, const 
   opt.min_ne = 16;
   opt.max_ne = 64;
   opt.triple = 1;
+  opt.cand = cand;
   return panel_op_build(op, M, K, A.data(), srcs, opt, 150 * 1024);
 }
 
@@ -367,10 +369,10 @@ int launch_fused_grad(const PanelOp<T> &op, const EleView<T> &ev, const T *u, co
 }
 
 #define FR_INST(T)                                                                                                          \
-  template bool fused_div_build<T>(PanelOp<T> &, int, int, const double *, const double *);                               \
+  template bool fused_div_build<T>(PanelOp<T> &, int, int, const double *, const double *, int);                             \
   template int launch_fused_div<T>(const PanelOp<T> &, const EleView<T> &, const T *, const T *, const StageArgs<T> &,     \
                                    cudaStream_t);                                                                          \
-  template bool fused_grad_build<T>(PanelOp<T> &, int, int, const double *, const double *);                               \
+  template bool fused_grad_build<T>(PanelOp<T> &, int, int, const double *, const double *, int);                             \
   template int launch_fused_grad<T>(const PanelOp<T> &, const EleView<T> &, const T *, const T *, T *, T *,                \
                                     const PhysParams<T> &, cudaStream_t);
 FR_INST(double)

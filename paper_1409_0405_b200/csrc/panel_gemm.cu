@@ -43,11 +43,12 @@ void launch_shape(const PlainArgs<T> &a, size_t smem, cudaStream_t s) {
 }  // namespace
 
 template <typename T>
-bool panel_gemm_build(PanelOp<T> &op, int M, int K, const double *A) {
+bool panel_gemm_build(PanelOp<T> &op, int M, int K, const double *A, int cand) {
   std::vector<KSource> srcs{KSource{K, 0, 1}};
   PackOptions opt;
   opt.min_ne = sizeof(T) == 8 ? 16 : 32;
   opt.max_ne = 64;
+  opt.cand = cand;
   return panel_op_build(op, M, K, A, srcs, opt, 150 * 1024);
 }
 
@@ -80,8 +81,8 @@ void panel_gemm_run(const PanelOp<T> &op, long long N, T c1, const T *B, long lo
   throw Error{FR_ESTATE, "panel_gemm_run: no kernel for this accumulator shape"};
 }
 
-template bool panel_gemm_build<double>(PanelOp<double> &, int, int, const double *);
-template bool panel_gemm_build<float>(PanelOp<float> &, int, int, const double *);
+template bool panel_gemm_build<double>(PanelOp<double> &, int, int, const double *, int);
+template bool panel_gemm_build<float>(PanelOp<float> &, int, int, const double *, int);
 template void panel_gemm_run<double>(const PanelOp<double> &, long long, double, const double *, long long, long long, double,
                                      double *, long long, long long, int, cudaStream_t);
 template void panel_gemm_run<float>(const PanelOp<float> &, long long, float, const float *, long long, long long, float, float *,

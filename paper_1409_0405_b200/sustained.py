@@ -1,0 +1,90 @@
+"""Sustained time-marching run (BASELINE.json configs[4]): the cylinder-like O-mesh of config 3, scaled up, p = 3, FP32 (or FP64),
+RK45[2R+] with fixed dt replayed as CUDA graphs (`fr_rk_run`) for `--steps` steps.  Reports GDOF-RHS/s, the totals of the five
+conserved quantities and the kinetic energy (quadrature-weighted, accumulated in FP64 on the host from `fr_get_state`) at steps
+0 / 10 / 100 / 1000, and the per-kernel-group time breakdown of one right-hand side (`fr_profile_rhs`: operator products incl. fused
+point-wise work, stand-alone point-wise kernels, interface kernels).
+
+  python -m paper_1409_0405_b200.sustained [--scale 2] [--p 3] [--prec f32] [--steps 1000] [--dt 4e-6] [--json out.json]
+
+`--scale s` multiplies the circumferential and spanwise cell counts of config 3 (100 x 15) by s: elements = 480 000 s^2.  Config 5
+itself is s = 6 (17.3 M elements, ~150 GB); the mesh generator is host-side numpy and its memory, not the library, bounds s.
+"""
+import argparse
+import json
+import sys
+import time
+
+import numpy as np
+
+
+def totals(case, us):
+    """sum over elements and points of omega |J| u_k (k = 0..4) and of the kinetic energy; FP64."""
+    tot = np.zeros(6)
+    for e, u in zip(case["eles"], us):
+        w = e["wts"][:, None] * e["djac"]
+        for k in range(5):
+            tot[k] += (w * u[:, k, :]).sum()
+        tot[5] += (w * 0.5 * (u[:, 1, :] ** 2 + u[:, 2, :] ** 2 + u[:, 3, :] ** 2) / u[:, 0, :]).sum()
+    return tot
+
+
+def main():
+    import torch
+    from fr_inputs import cases
+    from . import Context
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--scale", type=int, default=2)
+    ap.add_argument("--p", type=int, default=3)
+    ap.add_argument("--prec", default="f32", choices=["f32", "f64"])
+    ap.add_argument("--steps", type=int, default=1000)
+    ap.add_argument("--dt", type=float, default=4e-6)
+    ap.add_argument("--json", default=None)
+    args = ap.parse_args()
+    if not torch.cuda.is_available():
+        raise SystemExit("sustained needs a CUDA device (no CPU fallback)")
+    t0 = time.time()
+    case = cases.config3(p=args.p, ntheta=100 * args.scale, nz=15 * args.scale, seed=cases.SEEDS["c5"])
+    ndof = cases.ndof(case)
+    ne = {e["etype"]: e["neles"] for e in case["eles"]}
+    print("mesh: %s elements, %d DOF, generated in %.0f s" % (ne, ndof, time.time() - t0), flush=True)
+    stream = torch.cuda.Stream()
+    ctx = Context(case, prec=args.prec, stepper="rk45", stream=stream.cuda_stream)
+    ctx.set_state(case["u0"])
+    marks = sorted(set(m for m in (0, 10, 100, 1000, args.steps) if m <= args.steps))
+    out = dict(workload="config3 generator x%d: %d pri + %d tet, p=%d, NS, RK45[2R+], %s" % (
+        args.scale, ne.get("pri", 0), ne.get("tet", 0), args.p, args.prec), dof=ndof, dt=args.dt, checkpoints=[])
+    done, gpu_s = 0, 0.0
+    for m in marks:
+        if m > done:
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(stream)
+            ctx.rk_run(args.dt, m - done)
+            e1.record(stream)
+            e1.synchronize()
+            gpu_s += e0.elapsed_time(e1) * 1e-3
+            done = m
+        us = ctx.get_state()
+        finite = bool(all(np.isfinite(u).all() for u in us))
+        tot = totals(case, us) if finite else np.full(6, np.nan)
+        out["checkpoints"].append(dict(step=m, finite=finite, mass=tot[0], mom=[tot[1], tot[2], tot[3]], energy=tot[4], kinetic=tot[5]))
+        print("step %5d finite %s totals %s" % (m, finite, " ".join("%.10e" % x for x in tot)), flush=True)
+        if not finite:
+            break
+    out["steps"] = done
+    out["gdof_rhs_per_s"] = ndof * 5 * done / gpu_s / 1e9 if gpu_s > 0 else None
+    out["ms_per_step"] = 1e3 * gpu_s / max(done, 1)
+    c0 = out["checkpoints"][0]
+    cl = out["checkpoints"][-1]
+    out["relative_drift"] = dict(mass=(cl["mass"] - c0["mass"]) / abs(c0["mass"]), energy=(cl["energy"] - c0["energy"]) / abs(c0["energy"]),
+                                 kinetic=(cl["kinetic"] - c0["kinetic"]) / abs(c0["kinetic"]))
+    out["rhs_breakdown_ms"] = ctx.profile_rhs(reps=3)
+    out["kernels_launched"] = ctx.launch_count()
+    print(json.dumps(out))
+    if args.json:
+        with open(args.json, "w") as f:
+            json.dump(out, f, indent=1)
+    ctx.close()
+
+
+if __name__ == "__main__":
+    sys.exit(main())
