@@ -176,7 +176,7 @@ struct Ctx : CtxBase {
       v.nfpts = nf;
       v.affine = d.affine ? 1 : 0;
       v.neles = d.neles;
-      v.ld = (d.neles + 63) / 64 * 64;   // whole panels of up to 64 elements (panel.cuh); 512-byte rows
+      v.ld = (d.neles + 127) / 128 * 128;   // whole panels of up to 128 elements (panel.cuh)
       const long long ld = v.ld, ne = d.neles;
       // metric terms, padded with the identity so padding lanes stay finite
       const long long npt = v.affine ? 1 : nu;

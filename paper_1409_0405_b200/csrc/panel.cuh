@@ -102,8 +102,10 @@ struct PanelGeom {
 // FP64: NIT*CX*10 doubles per thread; FP32: NIT*CX*40 floats.
 template <typename T>
 constexpr int panel_maxw(int nit, int cx) {
+  // FP32 tiles also keep 8 operator values and 5*CX state values live per k and index more arrays: with only +70 registers of
+  // head-room the CX = 2 shapes spilled inside the multiply loop (8x slower), so FP32 with CX = 2 budgets +110.
   const int acc_regs = sizeof(T) == 8 ? nit * cx * 20 : nit * cx * 40;
-  const int w = 2048 / (acc_regs + 70);
+  const int w = 2048 / (acc_regs + ((sizeof(T) == 4 && cx == 2) ? 110 : 70));
   return w > 16 ? 16 : (w < 1 ? 1 : w);
 }
 
@@ -128,6 +130,7 @@ inline std::vector<PanelGeom> list_geoms(int G, int min_ne, int max_ne, int trip
           const int NE = (f64 ? 8 : 32) * CX * WC;
           if (NE < min_ne || NE > max_ne) continue;
           double eff = (double)G / (WR * nit);
+          if (eff < 0.7) continue;                       // more than 30 % of the row slots empty: never worth timing
           // prefer many warps, then wider panels, then fewer accumulators
           double score = eff * (0.4 + 0.6 * std::min(W, 14) / 14.0) * (1.0 + 0.02 * std::log2((double)NE)) * (1.0 - 0.005 * nit * CX);
           // dense operators: the B fragments of a k-block are shared by the NIT row groups of the warp; shared-memory

@@ -291,7 +291,7 @@ bool fused_div_build(PanelOp<T> &op, int nu, int nf, const double *M132, const d
   std::vector<KSource> srcs{KSource{3 * nu, KIND_PLAIN, 1}, KSource{nf, KIND_PLAIN, 1}};
   PackOptions opt;
   opt.min_ne = 16;
-  opt.max_ne = 64;
+  opt.max_ne = sizeof(T) == 8 ? 64 : 128;
   opt.cand = cand;
   return panel_op_build(op, nu, K, A.data(), srcs, opt, 150 * 1024);
 }
@@ -334,7 +334,7 @@ bool fused_grad_build(PanelOp<T> &op, int nu, int nf, const double *M460, const 
   std::vector<KSource> srcs{KSource{nu, KIND_PLAIN, 1}, KSource{nf, KIND_PLAIN, 1}};
   PackOptions opt;
   opt.min_ne = 16;
-  opt.max_ne = 64;
+  opt.max_ne = sizeof(T) == 8 ? 64 : 128;
   opt.triple = 1;
   opt.cand = cand;
   return panel_op_build(op, M, K, A.data(), srcs, opt, 150 * 1024);

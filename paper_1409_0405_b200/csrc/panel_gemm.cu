@@ -47,7 +47,7 @@ bool panel_gemm_build(PanelOp<T> &op, int M, int K, const double *A, int cand) {
   std::vector<KSource> srcs{KSource{K, 0, 1}};
   PackOptions opt;
   opt.min_ne = sizeof(T) == 8 ? 16 : 32;
-  opt.max_ne = 64;
+  opt.max_ne = sizeof(T) == 8 ? 64 : 128;
   opt.cand = cand;
   return panel_op_build(op, M, K, A, srcs, opt, 150 * 1024);
 }
