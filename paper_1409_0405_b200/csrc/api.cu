@@ -247,7 +247,7 @@ struct Ctx : CtxBase {
   // which one is fastest depends on things it does not model (register allocation, barrier skew, epilogue latency).  For
   // meshes large enough to time reliably, fr_setup launches the first kTuneCands candidates on the context's own arrays and
   // keeps the fastest.  Results do not depend on the choice (the summation order over k is the same for every geometry).
-  static constexpr int kTuneCands = 10;
+  static constexpr int kTuneCands = 14;
   static constexpr long long kTuneMinEles = 16384;
   template <typename B, typename L>
   void tune(PanelOp<T> &cur, B build, L launch, const char *what) {

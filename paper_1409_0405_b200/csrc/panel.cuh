@@ -48,6 +48,7 @@ struct PanelOp {
   int WR = 0, WC = 0, NIT = 0, CX = 0;   // warp grid, row groups per row-warp, column blocks (FP64) / elements per lane (FP32)
   int NE = 0;                            // elements per panel (of one warp group)
   int NG = 1;                            // independent warp groups per CTA, each streaming its own panels (staggered)
+  int occ = 1;                           // CTAs per SM the plan was sized for (shared memory and registers)
   int KC = 0, nchunks = 0, NS = 0;       // rows per chunk (max), chunks, slots = WR*NIT
   int stage_elems = 0;                   // elements of one ring stage
   int curved = 0;                        // flux chunks: metric terms per point (1) or per element (0)
@@ -96,6 +97,7 @@ struct PanelGeom {
   int WR, WC, NIT, CX, NE;
   double eff;
   int NG;
+  int occ;
 };
 
 // Warps per CTA a given accumulator shape allows: registers per thread ~ accumulators + 70 must fit the 64K register file.
@@ -138,7 +140,10 @@ inline std::vector<PanelGeom> list_geoms(int G, int min_ne, int max_ne, int trip
           if (dense) score /= 1.0 + 0.4 * (2.0 / nit + 0.4 / CX);
           // two staggered warp groups hide one group's epilogue and load waits behind the other's multiplies
           if (NG == 2) score *= 1.25;
-          all.push_back(PanelGeom{WR, WC, nit, CX, NE, score, NG});
+          all.push_back(PanelGeom{WR, WC, nit, CX, NE, score, NG, 1});
+          // two CTAs per SM (half the shared memory and registers each): another way to overlap one panel's epilogue and
+          // load waits with another's multiplies; only timing (fr_setup autotuning) tells which wins
+          if (NG == 1 && 2 * W <= panel_maxw<T>(nit, CX)) all.push_back(PanelGeom{WR, WC, nit, CX, NE, score * 0.9, NG, 2});
         }
       }
     }
@@ -150,7 +155,7 @@ inline std::vector<PanelGeom> list_geoms(int G, int min_ne, int max_ne, int trip
 template <typename T>
 inline PanelGeom choose_geom(int G, int min_ne, int max_ne, int triple, bool dense, int cand = 0) {
   const std::vector<PanelGeom> all = list_geoms<T>(G, min_ne, max_ne, triple, dense);
-  if (cand < 0 || cand >= (int)all.size()) return PanelGeom{0, 0, 0, 0, 0, -1.0, 1};
+  if (cand < 0 || cand >= (int)all.size()) return PanelGeom{0, 0, 0, 0, 0, -1.0, 1, 1};
   return all[cand];
 }
 
@@ -450,7 +455,8 @@ bool panel_op_build_kc(PanelOp<T> &p, int M, int K, const double *A, const std::
   const size_t smem_op = ((vals.size() * sizeof(T) + 15) / 16 * 16) + ((idx.size() * 4 + 15) / 16 * 16) +
                          ((off.size() * 4 + 15) / 16 * 16) + ((rowmap.size() * 4 + 15) / 16 * 16) +
                          ((chunks.size() * sizeof(ChunkDesc) + 15) / 16 * 16);
-  if (smem_op > smem_budget) return false;
+  if (geo.occ == 2) smem_total = smem_total / 2 - 2048;
+  if (smem_op > smem_budget || smem_op + 8192 > smem_total) return false;
   size_t stage_elems = 0;
   const int LDBh = PV * geo.NE + 4;
   for (auto &c : chunks)
@@ -472,6 +478,7 @@ bool panel_op_build_kc(PanelOp<T> &p, int M, int K, const double *A, const std::
   p.CX = geo.CX;
   p.NE = geo.NE;
   p.NG = geo.NG;
+  p.occ = geo.occ;
   p.KC = kcmax;
   p.stage_elems = (int)stage_elems;
   p.curved = opt.curved;
@@ -481,8 +488,8 @@ bool panel_op_build_kc(PanelOp<T> &p, int M, int K, const double *A, const std::
   p.nidx = (int)idx.size();
   p.dbg = getenv("FRB_PANEL_DBG") ? atoi(getenv("FRB_PANEL_DBG")) : 0;
   if (getenv("FRB_PANEL_VERBOSE"))
-    fprintf(stderr, "panel_op %s M=%d K=%d %s G=%d WR=%d WC=%d NIT=%d CX=%d NE=%d NG=%d warps=%d KC=%d nchunks=%d nblk=%d smem_op=%zu stage=%zu B density=%.2f macs/col=%.0f (dense %d)\n",
-            f64 ? "f64" : "f32", M, K, sparse ? "sparse" : "dense", G, WR, geo.WC, NIT, geo.CX, geo.NE, geo.NG, geo.NG * WR * geo.WC, kcmax,
+    fprintf(stderr, "panel_op %s M=%d K=%d %s G=%d WR=%d WC=%d NIT=%d CX=%d NE=%d NG=%d occ=%d warps=%d KC=%d nchunks=%d nblk=%d smem_op=%zu stage=%zu B density=%.2f macs/col=%.0f (dense %d)\n",
+            f64 ? "f64" : "f32", M, K, sparse ? "sparse" : "dense", G, WR, geo.WC, NIT, geo.CX, geo.NE, geo.NG, geo.occ, geo.NG * WR * geo.WC, kcmax,
             nchunks, nblk, smem_op, stage_elems * sizeof(T), density, (double)macs, M * K);
   p.sparse = sparse ? 1 : 0;
   p.macs_per_col = (double)macs;

@@ -271,9 +271,9 @@ __global__ void __launch_bounds__(32 * panel_maxw<T>(NIT, CX)) k_fused_grad(cons
 }
 
 template <typename K, typename A>
-void launch_panel(K k, const A &a, int nthreads, size_t smem, long long ntot, int ng, cudaStream_t s) {
+void launch_panel(K k, const A &a, int nthreads, size_t smem, long long ntot, int ng, int occ, cudaStream_t s) {
   FR_CUDA_TRY(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-  const long long grid = std::min<long long>((ntot + ng - 1) / ng, device_sm_count());
+  const long long grid = std::min<long long>((ntot + ng - 1) / ng, (long long)device_sm_count() * occ);
   k<<<(unsigned)grid, nthreads, smem, s>>>(a);
   FR_CUDA_TRY(cudaGetLastError());
 }
@@ -311,7 +311,7 @@ int launch_fused_div(const PanelOp<T> &op, const EleView<T> &ev, const T *ftil, 
   const int nthreads = 32 * op.WR * op.WC * op.NG;
 #define FR_CASE(NIT_, CX_)                                                          \
   if (op.NIT == NIT_ && op.CX == CX_) {                                             \
-    launch_panel(k_fused_div<T, NIT_, CX_>, a, nthreads, smem, a.npanels, op.NG, s);       \
+    launch_panel(k_fused_div<T, NIT_, CX_>, a, nthreads, smem, a.npanels, op.NG, op.occ, s);       \
     return 1;                                                                       \
   }
   if constexpr (sizeof(T) == 8) {
@@ -356,7 +356,7 @@ int launch_fused_grad(const PanelOp<T> &op, const EleView<T> &ev, const T *u, co
   const int nthreads = 32 * op.WR * op.WC * op.NG;
 #define FR_CASE(NIT_, CX_)                                                          \
   if (op.NIT == NIT_ && op.CX == CX_) {                                             \
-    launch_panel(k_fused_grad<T, NIT_, CX_>, a, nthreads, smem, a.npanels, op.NG, s);      \
+    launch_panel(k_fused_grad<T, NIT_, CX_>, a, nthreads, smem, a.npanels, op.NG, op.occ, s);      \
     return 1;                                                                       \
   }
   if constexpr (sizeof(T) == 8) {

@@ -33,7 +33,7 @@ void launch_shape(const PlainArgs<T> &a, size_t smem, cudaStream_t s) {
     attr_done = true;
   }
   FR_CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k, nthreads, smem));
-  occ = std::max(1, std::min(occ, 4));
+  occ = std::max(1, std::min(occ, a.op.occ));
   const long long ntot = a.npanels * a.nbatch;
   const long long grid = std::min<long long>((ntot + a.op.NG - 1) / a.op.NG, (long long)device_sm_count() * occ);
   k<<<(unsigned)grid, nthreads, smem, s>>>(a);
