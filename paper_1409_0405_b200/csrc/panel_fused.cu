@@ -25,6 +25,13 @@ struct VecIO<double, 2> {
     x[1] = t.y;
   }
   static __device__ __forceinline__ void st(double *p, const double (&x)[2]) { *reinterpret_cast<double2 *>(p) = make_double2(x[0], x[1]); }
+  // read-only data (metrics): ld.global.nc tells the compiler the load cannot alias the epilogue's stores, so the loads of the
+  // next tile may be hoisted above the stores of this one
+  static __device__ __forceinline__ void ldg(const double *p, double (&x)[2]) {
+    const double2 t = __ldg(reinterpret_cast<const double2 *>(p));
+    x[0] = t.x;
+    x[1] = t.y;
+  }
 };
 template <>
 struct VecIO<float, 2> {
@@ -34,11 +41,17 @@ struct VecIO<float, 2> {
     x[1] = t.y;
   }
   static __device__ __forceinline__ void st(float *p, const float (&x)[2]) { *reinterpret_cast<float2 *>(p) = make_float2(x[0], x[1]); }
+  static __device__ __forceinline__ void ldg(const float *p, float (&x)[2]) {
+    const float2 t = __ldg(reinterpret_cast<const float2 *>(p));
+    x[0] = t.x;
+    x[1] = t.y;
+  }
 };
 template <>
 struct VecIO<float, 1> {
   static __device__ __forceinline__ void ld(const float *p, float (&x)[1]) { x[0] = *p; }
   static __device__ __forceinline__ void st(float *p, const float (&x)[1]) { *p = x[0]; }
+  static __device__ __forceinline__ void ldg(const float *p, float (&x)[1]) { x[0] = __ldg(p); }
 };
 
 // K = -R/|J| (S9), then the stage update out1 = in1 + c1 K, out2 = in2 + c2 K (S10) or plain out1 = K
@@ -83,7 +96,7 @@ struct RkEpilogue {
       const long long col = e0 + e;
       const long long idx0 = (long long)m * 5 * ld + col;
       T rj[EW];
-      VecIO<T, EW>::ld(rcpdjac + (curved ? (long long)m * ld : 0) + col, rj);
+      VecIO<T, EW>::ldg(rcpdjac + (curved ? (long long)m * ld : 0) + col, rj);
       bool live[EW];
 #pragma unroll
       for (int j = 0; j < EW; ++j) live[j] = col + j < neles;
@@ -203,12 +216,12 @@ struct GradEpilogue {
       if (rho < 0) return;
       const long long col = e0 + e;
       T rj[EW], S[3][3][EW];
-      VecIO<T, EW>::ld(rcpdjac + (curved ? (long long)rho * ld : 0) + col, rj);
+      VecIO<T, EW>::ldg(rcpdjac + (curved ? (long long)rho * ld : 0) + col, rj);
 #pragma unroll
       for (int a = 0; a < 3; ++a)
 #pragma unroll
         for (int i = 0; i < 3; ++i)
-          VecIO<T, EW>::ld(smats + (curved ? ((long long)(a * 3 + i) * nupts + rho) * ld : (long long)(a * 3 + i) * ld) + col, S[a][i]);
+          VecIO<T, EW>::ldg(smats + (curved ? ((long long)(a * 3 + i) * nupts + rho) * ld : (long long)(a * 3 + i) * ld) + col, S[a][i]);
 #pragma unroll
       for (int j = 0; j < EW; ++j)
         if (col + j >= neles) rj[j] = T(0);      // padding lanes: zero
