@@ -121,6 +121,7 @@ struct Ctx : CtxBase {
   DevBuf<StageCoef> coef;
   StageCoef *coef_host = nullptr;   // pinned
   double coef_dt = std::nan("");
+  int jump = 0;                     // S2 stores C - U_f and the fused gradient operator is [M4 | M6] (all types fused)
   cudaGraphExec_t graph = nullptr;
   int graph_kernels = 0;
 
@@ -208,7 +209,7 @@ struct Ctx : CtxBase {
       }
       if (mode == FR_MODE_FUSED) {
         fused_div_build(e->pDiv, nu, nf, d.M132, d.M3);
-        if (ns) fused_grad_build(e->pGrad, nu, nf, d.M460, d.M6);
+        if (ns) fused_grad_build(e->pGrad, nu, nf, d.M460, d.M6, 0, d.M0);
       }
       const size_t nstate = (size_t)nu * 5 * ld;
       e->X.alloc(nstate);
@@ -230,6 +231,18 @@ struct Ctx : CtxBase {
       el.push_back(std::move(e));
     }
     for (int t = nt; t < FR_MAXTYPES; ++t) tt.ubase[t] = tt.gbase[t] = tt.ld[t] = tt.gcomp[t] = 0;
+    if (mode == FR_MODE_FUSED && ns) {
+      // the jump formulation of S2 needs every type on the fused gradient kernel; otherwise fall back to C itself
+      bool all = true;
+      for (int t = 0; t < nt; ++t) all = all && el[t]->pGrad.ok();
+      if (all) {
+        jump = 1;
+      } else {
+        for (int t = 0; t < nt; ++t)
+          if (el[t]->pGrad.ok())
+            fused_grad_build(el[t]->pGrad, el[t]->view.nupts, el[t]->view.nfpts, c->eles[t].M460, c->eles[t].M6, 0, nullptr);
+      }
+    }
     uf.alloc(utot);
     if (ns) {
       cf.alloc(utot);
@@ -309,7 +322,7 @@ struct Ctx : CtxBase {
            [&](const PanelOp<T> &op) { launch_fused_div(op, e.view, (const T *)e.grad.p, (const T *)ufp, plain, stream); },
            (tag + ":[M132|M3]").c_str());
       if (ns)
-        tune(e.pGrad, [&](PanelOp<T> &op, int k) { return fused_grad_build(op, nu, nf, d.M460, d.M6, k); },
+        tune(e.pGrad, [&](PanelOp<T> &op, int k) { return fused_grad_build(op, nu, nf, d.M460, d.M6, k, jump ? d.M0 : nullptr); },
              [&](const PanelOp<T> &op) {
                launch_fused_grad(op, e.view, (const T *)e.X.p, (const T *)(cf.p + tt.ubase[t]), e.grad.p, (T *)nullptr, ph, stream);
              },
@@ -438,9 +451,12 @@ struct Ctx : CtxBase {
       mark(CAT_GEMM, t, "S1_M0", (nu + nf) * 5 * n, 2 * nf * nu * 5 * n);
     }
     if (ns) {
-      nk += launch_con_u(iv, tt, uf.p, cf.p, ph.beta, s);   // S2
-      for (auto &b : bnd) nk += launch_bc_con_u(b->view, tt, uf.p, cf.p, ph.gamma, s);
-      mark(CAT_IFACE, -1, "S2_con_u", npr * (20 + 16 / w) + nbnd * (10 + 3 + 8 / w), npr * 15 + nbnd * 60);
+      nk += launch_con_u(iv, tt, uf.p, cf.p, ph.beta, jump, s);   // S2
+      for (auto &b : bnd) nk += launch_bc_con_u(b->view, tt, uf.p, cf.p, ph.gamma, jump, s);
+      {
+        const double words = jump ? (ph.beta == T(0.5) ? 15 : 20) : 20;
+        mark(CAT_IFACE, -1, jump ? "S2_con_u_jump" : "S2_con_u", npr * (words + 16 / w) + nbnd * (10 + 3 + 8 / w), npr * 15 + nbnd * 60);
+      }
       for (int t = 0; t < nt; ++t) {
         EleData<T> &e = *el[t];
         const long long n5 = 5 * e.view.ld;

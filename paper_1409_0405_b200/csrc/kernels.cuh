@@ -48,12 +48,12 @@ int launch_gradcoru(const EleView<T> &ev, T *g, cudaStream_t s);
 template <typename T>
 int launch_negdivconf(const EleView<T> &ev, const T *r, const StageArgs<T> &sa, cudaStream_t s);
 template <typename T>
-int launch_con_u(const IfaceView<T> &iv, const TypeTab &tt, const T *uf, T *cf, T beta, cudaStream_t s);
+int launch_con_u(const IfaceView<T> &iv, const TypeTab &tt, const T *uf, T *cf, T beta, int jump, cudaStream_t s);
 template <typename T>
 int launch_comm_flux(const IfaceView<T> &iv, const TypeTab &tt, T *uf, const T *gf, const PhysParams<T> &ph,
                      cudaStream_t s);
 template <typename T>
-int launch_bc_con_u(const BndView<T> &bv, const TypeTab &tt, const T *uf, T *cf, T gamma, cudaStream_t s);
+int launch_bc_con_u(const BndView<T> &bv, const TypeTab &tt, const T *uf, T *cf, T gamma, int jump, cudaStream_t s);
 template <typename T>
 int launch_bc_comm_flux(const BndView<T> &bv, const TypeTab &tt, T *uf, const T *gf, const PhysParams<T> &ph,
                         cudaStream_t s);
@@ -65,7 +65,7 @@ template <typename T>
 int launch_fused_div(const PanelOp<T> &op, const EleView<T> &ev, const T *ftil, const T *d, const StageArgs<T> &sa,
                      cudaStream_t s);
 template <typename T>
-bool fused_grad_build(PanelOp<T> &op, int nu, int nf, const double *M460, const double *M6, int cand = 0);
+bool fused_grad_build(PanelOp<T> &op, int nu, int nf, const double *M460, const double *M6, int cand = 0, const double *M0_jump = nullptr);
 template <typename T>
 int launch_fused_grad(const PanelOp<T> &op, const EleView<T> &ev, const T *u, const T *c, T *grad, T *ftil,
                       const PhysParams<T> &ph, cudaStream_t s);

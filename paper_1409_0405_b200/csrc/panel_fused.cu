@@ -337,12 +337,19 @@ int launch_fused_div(const PanelOp<T> &op, const EleView<T> &ev, const T *ftil, 
 }
 
 template <typename T>
-bool fused_grad_build(PanelOp<T> &op, int nu, int nf, const double *M460, const double *M6, int cand) {
+bool fused_grad_build(PanelOp<T> &op, int nu, int nf, const double *M460, const double *M6, int cand, const double *M0_jump) {
   const int K = nu + nf, M = 3 * nu;
   std::vector<double> A((size_t)M * K);
   for (int m = 0; m < M; ++m) {
     for (int k = 0; k < nu; ++k) A[(size_t)m * K + k] = M460[(size_t)m * nu + k];
     for (int k = 0; k < nf; ++k) A[(size_t)m * K + nu + k] = M6[(size_t)m * nf + k];
+    // jump formulation (k_con_u): the second operand is C - U_f, so the first block is M4 = M460 + M6 M0
+    if (M0_jump)
+      for (int k = 0; k < nu; ++k) {
+        double acc = 0;
+        for (int j = 0; j < nf; ++j) acc += M6[(size_t)m * nf + j] * M0_jump[(size_t)j * nu + k];
+        A[(size_t)m * K + k] += acc;
+      }
   }
   std::vector<KSource> srcs{KSource{nu, KIND_PLAIN, 1}, KSource{nf, KIND_PLAIN, 1}};
   PackOptions opt;
@@ -385,7 +392,7 @@ int launch_fused_grad(const PanelOp<T> &op, const EleView<T> &ev, const T *u, co
   template bool fused_div_build<T>(PanelOp<T> &, int, int, const double *, const double *, int);                             \
   template int launch_fused_div<T>(const PanelOp<T> &, const EleView<T> &, const T *, const T *, const StageArgs<T> &,     \
                                    cudaStream_t);                                                                          \
-  template bool fused_grad_build<T>(PanelOp<T> &, int, int, const double *, const double *, int);                             \
+  template bool fused_grad_build<T>(PanelOp<T> &, int, int, const double *, const double *, int, const double *);                             \
   template int launch_fused_grad<T>(const PanelOp<T> &, const EleView<T> &, const T *, const T *, T *, T *,                \
                                     const PhysParams<T> &, cudaStream_t);
 FR_INST(double)

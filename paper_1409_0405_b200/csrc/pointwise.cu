@@ -133,9 +133,12 @@ __device__ __forceinline__ void side_addr(const TypeTab &tt, int e, int ts, long
 }
 
 // S2: common solution C = (1/2 - beta) u_L + (1/2 + beta) u_R, stored at both flux points.
+// jump != 0: store the correction C - u_own instead (the fused gradient kernel then applies [M4 | M6] to [U; C - U_f], which equals
+// [M460 | M6][U; C] because M460 = M4 - M6 M0).  With beta = 1/2 the correction vanishes on the R side, whose entries stay at their
+// initial zero and are never written: the scattered R-side store of this kernel disappears.
 template <typename T>
 __global__ void __launch_bounds__(PW_BLOCK) k_con_u(IfaceView<T> iv, const __grid_constant__ TypeTab tt,
-                                                    const T *__restrict__ uf, T *cf, T beta) {
+                                                    const T *__restrict__ uf, T *cf, T beta, int jump) {
   const long long k = (long long)blockIdx.x * PW_BLOCK + threadIdx.x;
   if (k >= iv.npairs) return;
   const PairRec pr = iv.pairs[k];
@@ -143,6 +146,15 @@ __global__ void __launch_bounds__(PW_BLOCK) k_con_u(IfaceView<T> iv, const __gri
   side_addr<T>(tt, pr.le, pr.lts, ul, gl, ldl, gcl);
   side_addr<T>(tt, pr.re, pr.rts, ur, gr, ldr, gcr);
   const T wl = T(0.5) - beta, wr = T(0.5) + beta;
+  if (jump) {
+#pragma unroll
+    for (int v = 0; v < 5; ++v) {
+      const T d = uf[ur + v * ldr] - uf[ul + v * ldl];
+      cf[ul + v * ldl] = wr * d;
+      if (wl != T(0)) cf[ur + v * ldr] = -wl * d;
+    }
+    return;
+  }
   if (wl == T(0)) {
     // beta = 1/2 (the default, reading R9): C = u_R on both sides, the L state is not needed
 #pragma unroll
@@ -214,7 +226,7 @@ __device__ __forceinline__ void bc_states(int type, const T uL[5], const T n[3],
 // S2 at boundary flux points: C = u_visc(u_L).
 template <typename T>
 __global__ void __launch_bounds__(PW_BLOCK) k_bc_con_u(BndView<T> bv, const __grid_constant__ TypeTab tt,
-                                                       const T *__restrict__ uf, T *cf, T gamma) {
+                                                       const T *__restrict__ uf, T *cf, T gamma, int jump) {
   const long long k = (long long)blockIdx.x * PW_BLOCK + threadIdx.x;
   if (k >= bv.n) return;
   const BndRec br = bv.recs[k];
@@ -226,7 +238,7 @@ __global__ void __launch_bounds__(PW_BLOCK) k_bc_con_u(BndView<T> bv, const __gr
   const T n[3] = {bv.nrm[k], bv.nrm[bv.n + k], bv.nrm[2 * bv.n + k]};
   bc_states(bv.type, uL, n, gamma, bv.par, ub, uv);
 #pragma unroll
-  for (int v = 0; v < 5; ++v) cf[ul + v * ldl] = uv[v];
+  for (int v = 0; v < 5; ++v) cf[ul + v * ldl] = jump ? uv[v] - uL[v] : uv[v];
 }
 
 // S7 at boundary flux points: ghost state as u_R, G_f,R := G_f,L, only D_L stored.
@@ -282,9 +294,9 @@ int launch_negdivconf(const EleView<T> &ev, const T *r, const StageArgs<T> &sa, 
   return 1;
 }
 template <typename T>
-int launch_con_u(const IfaceView<T> &iv, const TypeTab &tt, const T *uf, T *cf, T beta, cudaStream_t s) {
+int launch_con_u(const IfaceView<T> &iv, const TypeTab &tt, const T *uf, T *cf, T beta, int jump, cudaStream_t s) {
   if (iv.npairs == 0) return 0;
-  k_con_u<T><<<blocks_for(iv.npairs), PW_BLOCK, 0, s>>>(iv, tt, uf, cf, beta);
+  k_con_u<T><<<blocks_for(iv.npairs), PW_BLOCK, 0, s>>>(iv, tt, uf, cf, beta, jump);
   FR_CUDA_TRY(cudaGetLastError());
   return 1;
 }
@@ -297,9 +309,9 @@ int launch_comm_flux(const IfaceView<T> &iv, const TypeTab &tt, T *uf, const T *
   return 1;
 }
 template <typename T>
-int launch_bc_con_u(const BndView<T> &bv, const TypeTab &tt, const T *uf, T *cf, T gamma, cudaStream_t s) {
+int launch_bc_con_u(const BndView<T> &bv, const TypeTab &tt, const T *uf, T *cf, T gamma, int jump, cudaStream_t s) {
   if (bv.n == 0) return 0;
-  k_bc_con_u<T><<<blocks_for(bv.n), PW_BLOCK, 0, s>>>(bv, tt, uf, cf, gamma);
+  k_bc_con_u<T><<<blocks_for(bv.n), PW_BLOCK, 0, s>>>(bv, tt, uf, cf, gamma, jump);
   FR_CUDA_TRY(cudaGetLastError());
   return 1;
 }
@@ -316,10 +328,10 @@ int launch_bc_comm_flux(const BndView<T> &bv, const TypeTab &tt, T *uf, const T 
   template int launch_tdisf<T>(const EleView<T> &, const T *, T *, const PhysParams<T> &, cudaStream_t);       \
   template int launch_gradcoru<T>(const EleView<T> &, T *, cudaStream_t);                                      \
   template int launch_negdivconf<T>(const EleView<T> &, const T *, const StageArgs<T> &, cudaStream_t);        \
-  template int launch_con_u<T>(const IfaceView<T> &, const TypeTab &, const T *, T *, T, cudaStream_t);        \
+  template int launch_con_u<T>(const IfaceView<T> &, const TypeTab &, const T *, T *, T, int, cudaStream_t);        \
   template int launch_comm_flux<T>(const IfaceView<T> &, const TypeTab &, T *, const T *, const PhysParams<T> &, \
                                    cudaStream_t);                                                               \
-  template int launch_bc_con_u<T>(const BndView<T> &, const TypeTab &, const T *, T *, T, cudaStream_t);       \
+  template int launch_bc_con_u<T>(const BndView<T> &, const TypeTab &, const T *, T *, T, int, cudaStream_t);       \
   template int launch_bc_comm_flux<T>(const BndView<T> &, const TypeTab &, T *, const T *, const PhysParams<T> &, \
                                       cudaStream_t);
 FR_INST(double)
