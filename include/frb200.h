@@ -142,8 +142,10 @@ fr_status fr_profile_rhs(fr_ctx *ctx, int32_t reps, double ms[4]);
 
 /* Per-kernel version of fr_profile_rhs: one entry per kernel (or kernel pair of one step) of a single RHS
  * evaluation, in launch order.  name = "<tet|pri>:<step>" or "<step>" for the interface kernels; ms = mean CUDA-event
- * time; alg_bytes / flops = ALGORITHMIC traffic and arithmetic of that launch (every operand read or written once,
- * dense 2*M*K*N flops for the operator products).  Writes min(*n, cap)
+ * time; alg_bytes / flops = ALGORITHMIC traffic and arithmetic of that launch (every operand read or written once;
+ * 2 flops per NON-ZERO operator entry and column for the products on the panel kernels -- structural zeros of the prism
+ * operators are skipped at set-up and not counted -- dense 2*M*K*N on the unfused fall-back).
+ * Writes min(*n, cap)
  * entries and sets *n to the number of kernels. */
 typedef struct {
   char name[48];

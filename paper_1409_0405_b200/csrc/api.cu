@@ -283,19 +283,21 @@ struct Ctx : CtxBase {
     float bt = time_op(best);
     const bool verbose = getenv("FRB_PANEL_VERBOSE") != nullptr;
     if (verbose) fprintf(stderr, "autotune %s cand 0: %.3f ms\n", what, bt);
-    for (int k = 1; k < kTuneCands; ++k) {
-      PanelOp<T> op;
-      if (!build(op, k)) break;
-      const float t = time_op(op);
-      if (verbose) fprintf(stderr, "autotune %s cand %d: %.3f ms\n", what, k, t);
-      if (t < bt) {
-        panel_op_free(best);
-        best = op;
-        bt = t;
-      } else {
-        panel_op_free(op);
+    const bool both = cur.density > 0.25 && cur.density < 0.95;   // intermediate density: also time the other packing
+    for (int pass = 0; pass < (both ? 2 : 1); ++pass)
+      for (int k = pass ? 1000 : 1; k < (pass ? 1000 + kTuneCands / 2 : kTuneCands); ++k) {
+        PanelOp<T> op;
+        if (!build(op, k)) break;
+        const float t = time_op(op);
+        if (verbose) fprintf(stderr, "autotune %s cand %d: %.3f ms\n", what, k, t);
+        if (t < bt) {
+          panel_op_free(best);
+          best = op;
+          bt = t;
+        } else {
+          panel_op_free(op);
+        }
       }
-    }
     cur = best;
     cudaEventDestroy(e0);
     cudaEventDestroy(e1);
@@ -448,7 +450,7 @@ struct Ctx : CtxBase {
       EleData<T> &e = *el[t];
       const double n = (double)e.view.neles, nu = e.view.nupts, nf = e.view.nfpts;
       nk += gemm_run(e.pM0, 5 * e.view.ld, T(1), u[t], 5 * e.view.ld, 0, T(0), uf.p + tt.ubase[t], 5 * e.view.ld, 0, 1, s);
-      mark(CAT_GEMM, t, "S1_M0", (nu + nf) * 5 * n, 2 * nf * nu * 5 * n);
+      mark(CAT_GEMM, t, "S1_M0", (nu + nf) * 5 * n, 2 * (e.pM0.pop ? e.pM0.pop->density : 1.0) * nf * nu * 5 * n);
     }
     if (ns) {
       nk += launch_con_u(iv, tt, uf.p, cf.p, ph.beta, jump, s);   // S2
@@ -469,7 +471,7 @@ struct Ctx : CtxBase {
           const bool fl = e.ftil.p != nullptr;
           mark(CAT_GEMM, t, fl ? "S3_S4_S6_fused_grad_flux" : "S3_S4_fused_grad",
                (5 * nu + 5 * nf + 15 * nu + 10 * nmet + (fl ? 15 * nu : 0)) * n,
-               2 * 3 * nu * (nu + nf) * 5 * n + 15 * 6 * nu * n + (fl ? 210 * nu * n : 0));
+               2 * e.pGrad.density * 3 * nu * (nu + nf) * 5 * n + 15 * 6 * nu * n + (fl ? 210 * nu * n : 0));
         } else {
           // S3: G~ = M460 U + M6 C
           nk += gemm_run(e.pM460, n5, T(1), u[t], n5, 0, T(0), e.grad.p, n5, 0, 1, s);
@@ -482,7 +484,7 @@ struct Ctx : CtxBase {
         // S5: G_f,i = M0 G_i, i = 0..2 (batched)
         nk += gemm_run(e.pM0, n5, T(1), e.grad.p, n5, (long long)e.view.nupts * n5, T(0), gf.p + tt.gbase[t], n5,
                        tt.gcomp[t], 3, s);
-        mark(CAT_GEMM, t, "S5_M0grad", (nu + nf) * 15 * n, 2 * nf * nu * 15 * n);
+        mark(CAT_GEMM, t, "S5_M0grad", (nu + nf) * 15 * n, 2 * (e.pM0.pop ? e.pM0.pop->density : 1.0) * nf * nu * 15 * n);
       }
     }
     nk += launch_comm_flux(iv, tt, uf.p, gf.p, ph, s);   // S7 (D overwrites U_f)
@@ -508,7 +510,7 @@ struct Ctx : CtxBase {
         nk += launch_fused_div(e.pDiv, e.view, ft, uf.p + tt.ubase[t], sa[t], s);
         const double rk = sa[t].coef ? (sa[t].out2 ? 15 : 10) : 5;
         mark(CAT_GEMM, t, sa[t].coef ? "S8_S9_S10_fused_div_rk" : "S8_S9_fused_div", (15 * nu + 5 * nf + rk * nu + nmet) * n,
-             2 * nu * (3 * nu + nf) * 5 * n + 5 * nu * n);
+             2 * e.pDiv.density * nu * (3 * nu + nf) * 5 * n + 5 * nu * n);
         continue;
       }
       // S8: R = M132 F~ + M3 D

@@ -57,6 +57,7 @@ struct PanelOp {
   int dbg = 0;                           // measurement aid (env FRB_PANEL_DBG): 1 skip multiply, 2 skip epilogue
   int sparse = 0;                        // 1: per-group k-lists (idx/off); 0: dense, all slots share the chunk's rows
   double macs_per_col = 0;               // executed multiply-adds per column (dense: M*K)
+  double density = 1;                    // fraction of non-zero entries of the operator
   T *vals = nullptr;                     // FP64 [nblk][32]; FP32 [nblk][8]
   uint32_t *idx = nullptr;               // byte offset of the B row in the stage: FP64 [nblk][4], FP32 [nblk]
   int *off = nullptr;                    // [nchunks*NS + 1]
@@ -221,7 +222,7 @@ bool panel_op_build_kc(PanelOp<T> &p, int M, int K, const double *A, const std::
 // with one persistent CTA per SM); first try whole sources, then the height that makes three stages fit `smem_total`.
 template <typename T>
 bool panel_op_build(PanelOp<T> &p, int M, int K, const double *A, const std::vector<KSource> &srcs, const PackOptions &opt,
-                    size_t smem_budget, size_t smem_total = 200 * 1024) {
+                    size_t smem_budget, size_t smem_total = 220 * 1024) {
   int kc = opt.kc > 0 ? opt.kc : 252;
   for (int attempt = 0; attempt < 6 && kc >= 4; ++attempt) {
     int fit = 0;
@@ -255,7 +256,10 @@ bool panel_op_build_kc(PanelOp<T> &p, int M, int K, const double *A, const std::
         ++nnz;
       }
   const double density = (double)nnz / ((double)M * K);
-  const bool sparse = opt.allow_sparse && density < 0.6;
+  // automatic choice: k-lists below 60 % density; cand >= 1000 asks for the opposite packing (the autotuner times both for
+  // operators of intermediate density, e.g. [M4 | M6] of tetrahedra, 66 % dense, whose M6 half is zero for two faces per alpha)
+  const bool flip = opt.cand >= 1000 && density < 0.95;
+  const bool sparse = (opt.allow_sparse && density < 0.6) != flip;
   // ---- rows -> groups of 8
   std::vector<int> order;   // virtual row -> actual row or -1
   if (opt.triple) {
@@ -345,7 +349,7 @@ bool panel_op_build_kc(PanelOp<T> &p, int M, int K, const double *A, const std::
       const int n = (int)lists[g][c].size();
       gcost[g] += f64 ? (n + 3) / 4 * 4 : n;
     }
-  PanelGeom geo = choose_geom<T>(G, opt.min_ne, opt.max_ne, opt.triple, !sparse, opt.cand);
+  PanelGeom geo = choose_geom<T>(G, opt.min_ne, opt.max_ne, opt.triple, !sparse, opt.cand % 1000);
   if (geo.eff < 0) return false;
   const int WR = geo.WR, NIT = geo.NIT, NS = WR * NIT;
   // LPT assignment of group units (1 or 3 groups) to row-warps, at most NIT groups per row-warp
@@ -493,6 +497,7 @@ bool panel_op_build_kc(PanelOp<T> &p, int M, int K, const double *A, const std::
             nchunks, nblk, smem_op, stage_elems * sizeof(T), density, (double)macs, M * K);
   p.sparse = sparse ? 1 : 0;
   p.macs_per_col = (double)macs;
+  p.density = density;
   p.smem_op = smem_op;
   auto up = [](auto *&dst, const auto &h) {
     using E = typename std::remove_reference<decltype(h[0])>::type;
