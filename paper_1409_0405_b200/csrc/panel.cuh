@@ -120,8 +120,9 @@ inline std::vector<PanelGeom> list_geoms(int G, int min_ne, int max_ne, int trip
   const bool f64 = sizeof(T) == 8;
   const int gu = triple ? 3 : 1;            // groups come in units of `gu` that must stay on one row-warp
   const int GU = (G + gu - 1) / gu;
-  // measured on config 3 (profiles/r01_c_fusion_notes.md): two groups help the FP64 kernels slightly, not the FP32 ones
-  const int ngmax = getenv("FRB_PANEL_NG") ? atoi(getenv("FRB_PANEL_NG")) : (sizeof(T) == 8 ? 2 : 1);
+  // two groups help some FP64 kernels and hurt most FP32 ones (profiles/r01_c_fusion_notes.md): both are candidates, the static
+  // score favours them in FP64 only, and the autotuner decides on large meshes
+  const int ngmax = getenv("FRB_PANEL_NG") ? atoi(getenv("FRB_PANEL_NG")) : 2;
   for (int NG = 1; NG <= ngmax; ++NG)
     for (int WR = 1; WR <= PANEL_MAXW; ++WR) {
       const int nit = ((GU + WR - 1) / WR) * gu;
@@ -140,7 +141,7 @@ inline std::vector<PanelGeom> list_geoms(int G, int min_ne, int max_ne, int trip
           // wavefronts per multiply ~ 2/NIT + 0.4/CX
           if (dense) score /= 1.0 + 0.4 * (2.0 / nit + 0.4 / CX);
           // two staggered warp groups hide one group's epilogue and load waits behind the other's multiplies
-          if (NG == 2) score *= 1.25;
+          if (NG == 2) score *= f64 ? 1.25 : 0.85;
           all.push_back(PanelGeom{WR, WC, nit, CX, NE, score, NG, 1});
           // two CTAs per SM (half the shared memory and registers each): another way to overlap one panel's epilogue and
           // load waits with another's multiplies; only timing (fr_setup autotuning) tells which wins
