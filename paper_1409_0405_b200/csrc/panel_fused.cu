@@ -133,6 +133,27 @@ struct RkEpilogue {
             VecIO<T, EW>::st(sa.out1 + idx, o1);
           }
         }
+      } else if (sa.coef && same) {
+        // FP64, RK45[2R+] (both updates start from the same register X): the five loads of the tile together, then the stores
+        T a[PV][EW];
+#pragma unroll
+        for (int v = 0; v < PV; ++v) VecIO<T, EW>::ld(sa.in1 + idx0 + v * ld, a[v]);
+#pragma unroll
+        for (int v = 0; v < PV; ++v) {
+          const long long idx = idx0 + v * ld;
+          T k[EW], o1[EW];
+#pragma unroll
+          for (int j = 0; j < EW; ++j) k[j] = live[j] ? -tile[v][j] * rj[j] : T(0);
+          if (sa.out2) {
+            T o2[EW];
+#pragma unroll
+            for (int j = 0; j < EW; ++j) o2[j] = live[j] ? a[v][j] + c2 * k[j] : T(0);
+            VecIO<T, EW>::st(sa.out2 + idx, o2);
+          }
+#pragma unroll
+          for (int j = 0; j < EW; ++j) o1[j] = live[j] ? a[v][j] + c1 * k[j] : T(0);
+          VecIO<T, EW>::st(sa.out1 + idx, o1);
+        }
       } else {
 #pragma unroll
         for (int v = 0; v < PV; ++v) {
