@@ -79,7 +79,8 @@ void panel_op_free(PanelOp<T> &p) {
 
 // How the K dimension of the operator is fed: a list of sources stacked along K, each cut into chunks of at most KC rows.
 // kind 0: `rows` plain rows of a global matrix <-> `rows` columns of A.
-// kind 1: transformed flux at `rows` solution points <-> 3*rows columns of A (alpha-major: column alpha*rows + nu); a chunk
+// kind 1 (kept for producers that transform a chunk in shared memory -- kTransform in panel_kernel.cuh; not used by the kernels of
+//         this round, see panel_fused.cu for why): transformed flux at `rows` solution points <-> 3*rows columns of A (alpha-major: column alpha*rows + nu); a chunk
 //         of n points occupies stage rows [0,3n) (alpha-major within the chunk: row alpha*n + j) for G -> F~, rows [3n,4n)
 //         for U, followed by the metric terms (flux_stage_elems).
 struct KSource {

@@ -250,41 +250,4 @@ inline size_t panel_smem_bytes(const PanelOp<T> &op) {
   return op.smem_op + (size_t)op.NG * PANEL_NSTAGE * op.stage_elems * sizeof(T) + 16;
 }
 
-// cp.async of `nrows` rows of a [rows][5][ld] state matrix into stage rows (pitch LDB, column v*NE + e); every thread owns a
-// fixed 16-byte column piece and walks down the rows.  gsrc points at (first row, v = 0, first element of the panel).
-template <typename T>
-__device__ __forceinline__ void cp_rows5(T *sdst, int LDB, int NE, const T *gsrc, long long gld, long long vstride, int nrows,
-                                         int tid, int nthreads) {
-  constexpr int CTV = 16 / (int)sizeof(T);
-  const int lg = 31 - __clz(NE / CTV);
-  const int ppr = PV << lg;
-  const bool wide = nthreads >= ppr;
-  const int rpi = wide ? nthreads / ppr : 1;
-  const int sub = wide ? tid / ppr : 0;
-  if (sub >= rpi) return;
-  for (int col = tid - sub * ppr; col < ppr; col += wide ? ppr : nthreads) {
-    const int v = col >> lg, e = (col - (v << lg)) * CTV;
-    const T *g = gsrc + (long long)sub * gld + v * vstride + e;
-    T *sp = sdst + sub * LDB + v * NE + e;
-    const long long gstep = (long long)rpi * gld;
-    const int sstep = rpi * LDB;
-    for (int r = sub; r < nrows; r += rpi) {
-      pcp_async16(sp, g, 16);
-      g += gstep;
-      sp += sstep;
-    }
-  }
-}
-// same for rows of NE contiguous elements (metric terms): stage pitch NE
-template <typename T>
-__device__ __forceinline__ void cp_rows1(T *sdst, int NE, const T *gsrc, long long gld, int nrows, int tid, int nthreads) {
-  constexpr int CTV = 16 / (int)sizeof(T);
-  const int lg = 31 - __clz(NE / CTV);
-  const int np = nrows << lg;
-  for (int p = tid; p < np; p += nthreads) {
-    const int r = p >> lg, e = (p - (r << lg)) * CTV;
-    pcp_async16(sdst + r * NE + e, gsrc + (long long)r * gld + e, 16);
-  }
-}
-
 }  // namespace frb
