@@ -229,12 +229,16 @@ def _measure(case, prec, args, torch, dist, rank, world, with_e2e=True, sampler=
 
 
 def _traffic(name, prec):
-    """DRAM bytes per launch of kernel `name` from the committed ncu --set full summary (profiles/r01_traffic.json), else None."""
+    """DRAM bytes per launch of kernel `name` from the committed ncu --set full summary (profiles/r01_traffic.csv), else None."""
     try:
-        with open(os.path.join(ROOT, "profiles", "r01_traffic.json")) as f:
-            return json.load(f).get(prec, {}).get(name)
+        with open(os.path.join(ROOT, "profiles", "r01_traffic.csv")) as f:
+            for line in f:
+                a = line.strip().split(",")
+                if len(a) == 3 and a[0] == prec and a[1] == name:
+                    return float(a[2])
     except Exception:
-        return None
+        pass
+    return None
 
 
 # arithmetic peaks measured on this pool's B200 with register-resident chains (profiles/r01_b_device_probes.md): FP64 on the
