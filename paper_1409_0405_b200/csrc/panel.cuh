@@ -225,6 +225,13 @@ bool panel_op_build_kc(PanelOp<T> &p, int M, int K, const double *A, const std::
 template <typename T>
 bool panel_op_build(PanelOp<T> &p, int M, int K, const double *A, const std::vector<KSource> &srcs, const PackOptions &opt,
                     size_t smem_budget, size_t smem_total = 220 * 1024) {
+  // FRB_FORCE_CAND=k: build candidate k (geometry + 1000 * opposite packing) where the caller asked for the default; falls back
+  // to the default if k does not exist for this operator.  Lets the parity tests cover every candidate the autotuner may pick.
+  if (opt.cand == 0 && getenv("FRB_FORCE_CAND")) {
+    PackOptions o2 = opt;
+    o2.cand = atoi(getenv("FRB_FORCE_CAND"));
+    if (o2.cand != 0 && panel_op_build(p, M, K, A, srcs, o2, smem_budget, smem_total)) return true;
+  }
   int kc = opt.kc > 0 ? opt.kc : 252;
   for (int attempt = 0; attempt < 6 && kc >= 4; ++attempt) {
     int fit = 0;

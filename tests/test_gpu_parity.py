@@ -235,3 +235,16 @@ def test_config3_full_size_sampled_parity(prec):
     assert np.all(err <= _tolerance(prec, amp)), (prec, err, _tolerance(prec, amp))
     for rr, u in zip(raw, case["u0"]):
         assert np.all(rr[:, :, u.shape[2]:] == 0)
+
+
+# ---------------------------------------------------------------------------- every panel geometry the autotuner may pick
+@pytest.mark.parametrize("cand", [1, 2, 3, 4, 5, 6, 8, 10, 13, 1000, 1001, 1003])
+def test_candidate_geometries_parity(cand, monkeypatch):
+    """fr_setup times candidate geometries only on large meshes, so the small parity meshes always run candidate 0.  Force
+    candidate `cand` (FRB_FORCE_CAND: geometry index + 1000 for the opposite dense / k-list packing) for every operator and check
+    the right-hand side of the mixed config-2 mesh at p = 4 and p = 2 in both precisions."""
+    monkeypatch.setenv("FRB_FORCE_CAND", str(cand))
+    for p in (4, 2):
+        case = cases.config2(6, p, "ns", numbering="random")
+        for prec in ("f64", "f32"):
+            _check_rhs(case, prec, "fused")
