@@ -41,7 +41,7 @@ typedef enum { FR_OK = 0, FR_EINVAL = 1, FR_ENOMEM = 2, FR_ECUDA = 3, FR_ESTATE 
 typedef enum { FR_F32 = 4, FR_F64 = 8 } fr_prec;                 /* P:23 "Precisions: Single, Double" */
 typedef enum { FR_EULER = 0, FR_NAVIER_STOKES = 1 } fr_system;   /* P:23 "Governing Systems" */
 typedef enum { FR_TET = 0, FR_PRI = 1, FR_HEX = 2 } fr_etype;    /* P:23; only FR_TET and FR_PRI are accepted by fr_setup */
-typedef enum { FR_RK4 = 0, FR_RK45_2R = 1 } fr_stepper;          /* P:23 "RK4, RK45"; P:116 RK45[2R+] */
+typedef enum { FR_RK4 = 0, FR_RK45_2R = 1, FR_EULER1 = 2 } fr_stepper;   /* P:23 "Time Steppers: Euler, RK4, RK45"; P:116 RK45[2R+] */
 typedef enum { FR_BC_NOSLIP_ISOTHERMAL_WALL = 0, FR_BC_CHAR_RIEMANN_INV = 1 } fr_bctype;
 typedef enum { FR_MODE_FUSED = 0, FR_MODE_UNFUSED = 1 } fr_mode; /* kernel chain: fused (default) or one kernel per step */
 
@@ -121,7 +121,7 @@ fr_status fr_rhs(fr_ctx *ctx, const void *const *u_dev, void *const *dudt_dev);
 fr_status fr_set_state(fr_ctx *ctx, const double *const *u_host);
 fr_status fr_get_state(fr_ctx *ctx, double *const *u_host);
 
-/* Advance the internal state by one step of the configured stepper with step dt (RK4: P:23; RK45[2R+]:
+/* Advance the internal state by one step of the configured stepper with step dt (forward Euler, RK4: P:23; RK45[2R+]:
  * P:116, coefficients reading R12; fixed dt, no error control).  The stage update is fused into the last
  * kernel of each RHS (S10).  The kernel sequence of a step is captured once into a CUDA graph and
  * replayed.  Asynchronous.  fr_rk_run = nsteps calls of fr_rk_step without host synchronisation. */

@@ -236,6 +236,11 @@ def rhs(cfg, eles, ifc, bcs, us, parts=None):
 
 
 # ----------------------------------------------------------------------------- time steppers
+def euler_step(f, us, dt):
+    """Forward Euler (Table 1, "Time Steppers: Euler, RK4, RK45"): u <- u + dt f(u)."""
+    return [u + dt * k for u, k in zip(us, f(us))]
+
+
 def rk4_step(f, us, dt):
     """Classical RK4 (Table 1). `f(list of U) -> list of dU/dt`."""
     k1 = f(us)

@@ -13,7 +13,7 @@ FR_OK, FR_EINVAL, FR_ENOMEM, FR_ECUDA, FR_ESTATE, FR_EUNSUPPORTED = range(6)
 FR_F32, FR_F64 = 4, 8
 FR_EULER, FR_NAVIER_STOKES = 0, 1
 FR_TET, FR_PRI, FR_HEX = 0, 1, 2
-FR_RK4, FR_RK45_2R = 0, 1
+FR_RK4, FR_RK45_2R, FR_EULER1 = 0, 1, 2
 FR_BC_NOSLIP_ISOTHERMAL_WALL, FR_BC_CHAR_RIEMANN_INV = 0, 1
 FR_MODE_FUSED, FR_MODE_UNFUSED = 0, 1
 
@@ -164,7 +164,7 @@ class Context:
         cfg = fr_config()
         cfg.system = FR_NAVIER_STOKES if cfgd["system"] == "ns" else FR_EULER
         cfg.prec = FR_F64 if prec == "f64" else FR_F32
-        cfg.stepper = FR_RK4 if stepper == "rk4" else FR_RK45_2R
+        cfg.stepper = {"rk4": FR_RK4, "rk45": FR_RK45_2R, "euler": FR_EULER1}[stepper]
         cfg.mode = FR_MODE_FUSED if mode == "fused" else FR_MODE_UNFUSED
         cfg.gamma, cfg.mu, cfg.prandtl = cfgd["gamma"], cfgd.get("mu", 0.0), cfgd.get("prandtl", 0.72)
         cfg.ldg_beta, cfg.ldg_tau = cfgd.get("ldg_beta", 0.5), cfgd.get("ldg_tau", 0.1)

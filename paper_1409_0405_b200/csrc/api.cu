@@ -571,12 +571,14 @@ struct Ctx : CtxBase {
   }
 
   // ------------------------------------------------------------------ Runge-Kutta (S10 fused into S9)
-  int nstages() const { return stepper == FR_RK4 ? 4 : 5; }
+  int nstages() const { return stepper == FR_RK4 ? 4 : (stepper == FR_EULER1 ? 1 : 5); }
 
   void fill_coefs(double dt) {
     if (stepper == FR_RK4) {
       const StageCoef c[4] = {{dt / 6, dt / 2}, {dt / 3, dt / 2}, {dt / 3, dt}, {dt / 6, 0.0}};
       for (int i = 0; i < 4; ++i) coef_host[i] = c[i];
+    } else if (stepper == FR_EULER1) {
+      coef_host[0] = StageCoef{dt, 0.0};              // forward Euler: X <- X + dt K
     } else {
       // RK4(3)5[2R+]C (reading R12): X += dt b_i K ; Y = X_old + dt a_i K
       static const double a[5] = {970286171893.0 / 4311952581923.0, 6584761158862.0 / 12103376702013.0,
@@ -602,6 +604,8 @@ struct Ctx : CtxBase {
           if (i == 0) sa[t] = StageArgs<T>{c, e.X.p, e.X.p, e.ACC.p, e.Y.p};
           else if (i < 3) sa[t] = StageArgs<T>{c, e.ACC.p, e.X.p, e.ACC.p, e.Y.p};
           else sa[t] = StageArgs<T>{c, e.ACC.p, nullptr, e.X.p, nullptr};
+        } else if (stepper == FR_EULER1) {
+          sa[t] = StageArgs<T>{c, e.X.p, nullptr, e.X.p, nullptr};
         } else {
           sa[t] = StageArgs<T>{c, e.X.p, e.X.p, e.X.p, i < S - 1 ? e.Y.p : nullptr};
         }
@@ -758,7 +762,7 @@ fr_status fr_setup(const fr_config *cfg, fr_ctx **out) {
     FR_REQUIRE(cfg && out, "cfg and out must be non-NULL");
     FR_REQUIRE(cfg->prec == FR_F32 || cfg->prec == FR_F64, "prec must be FR_F32 or FR_F64");
     FR_REQUIRE(cfg->system == FR_EULER || cfg->system == FR_NAVIER_STOKES, "unknown system");
-    FR_REQUIRE(cfg->stepper == FR_RK4 || cfg->stepper == FR_RK45_2R, "unknown stepper");
+    FR_REQUIRE(cfg->stepper == FR_RK4 || cfg->stepper == FR_RK45_2R || cfg->stepper == FR_EULER1, "unknown stepper");
     FR_REQUIRE(cfg->mode == FR_MODE_FUSED || cfg->mode == FR_MODE_UNFUSED, "unknown mode");
     require_device();
     std::unique_ptr<frb::CtxBase> impl;

@@ -110,14 +110,14 @@ def test_free_stream_and_empty_boundary_lists_on_gpu():
 
 # ---------------------------------------------------------------------------- Runge-Kutta steps
 @pytest.mark.parametrize("prec", ["f64", "f32"])
-@pytest.mark.parametrize("stepper", ["rk4", "rk45"])
+@pytest.mark.parametrize("stepper", ["rk4", "rk45", "euler"])
 def test_rk_step_parity(stepper, prec):
     from oracle import fr_oracle as O
     case = cases.config2(6, 2, "ns", numbering="random")
     c = round_case_to_f32(case) if prec == "f32" else case
     f = lambda us: O.rhs(c["cfg"], c["eles"], c["ifc"], c["bcs"], us)
     dt = 1e-4
-    step = O.rk4_step if stepper == "rk4" else O.rk45_step
+    step = {"rk4": O.rk4_step, "rk45": O.rk45_step, "euler": O.euler_step}[stepper]
     ref = c["u0"]
     for _ in range(3):
         ref = step(f, ref, dt)

@@ -37,7 +37,7 @@ def test_rk45_order_conditions_exact():
 def test_rk_slopes_on_linear_ode():
     lam = -1.3 + 0.7j
     f = lambda us: [lam * u for u in us]
-    for step, order in ((O.rk4_step, 4), (O.rk45_step, 4)):
+    for step, order in ((O.euler_step, 1), (O.rk4_step, 4), (O.rk45_step, 4)):
         errs = []
         for n in (8, 16, 32):
             u = [np.array([1.0 + 0j])]
