@@ -68,6 +68,17 @@ def config2(n=16, p=3, system="ns", mu=1e-3, numbering="natural", state_kind="vo
     return case
 
 
+def config_hex(n=8, p=3, system="ns", mu=1e-3, numbering="natural", warp=0.0, state_kind="vortex"):
+    """Hexahedral periodic box (NEXT-2 of SURVEY 8(f): the paper's second mesh type), same physics as config 2."""
+    m = _mesh.box_hex(n, 1.0, numbering=numbering, seed=SEEDS["c2"], warp=warp)
+    case = build_case(m, p, system=system, mu=mu if system == "ns" else 0.0)
+    if state_kind == "vortex":
+        case["u0"] = [state.isentropic_vortex(e["xu"]) for e in case["eles"]]
+    else:
+        case["u0"] = [state.smooth_periodic(e["xu"]) for e in case["eles"]]
+    return case
+
+
 def config3(p=4, ntheta=100, nz=15, nlayers=40, nr=40, numbering="morton", system="ns", amp=0.005, seed=None):
     """BASELINE.json configs[2] (and [4] when scaled): cylinder-like O-mesh, NS at Re=3900, M=0.2
     (PAPER.md:86-94,116), wall T_w = T_inf, far field = freestream, seeded 0.5 % perturbation."""

@@ -41,6 +41,13 @@ def shape(etype, x):
         dN = np.stack([np.stack([dL[i][0] * lo, dL[i][1] * lo, -L[i] / 2], 1) for i in range(3)]
                       + [np.stack([dL[i][0] * hi, dL[i][1] * hi, L[i] / 2], 1) for i in range(3)], axis=1)
         return N, dN
+    if etype == "hex":
+        # trilinear, vertex order of refelem (bottom quad counter-clockwise, then top quad)
+        sg = np.array(refelem._VERTS["hex"], dtype=np.float64)          # [8, 3] signs
+        fr, fs, ft = (1 + sg[None, :, 0] * r[:, None]), (1 + sg[None, :, 1] * s[:, None]), (1 + sg[None, :, 2] * t[:, None])
+        N = fr * fs * ft / 8
+        dN = np.stack([sg[None, :, 0] * fs * ft, fr * sg[None, :, 1] * ft, fr * fs * sg[None, :, 2]], axis=2) / 8
+        return N, dN
     raise ValueError(etype)
 
 
@@ -107,6 +114,8 @@ def _fix_orientation(etype, xv, vid, xref=None):
     neg = np.linalg.det(J) < 0
     if etype == "tet":
         sw = [0, 1, 3, 2]
+    elif etype == "hex":
+        sw = [4, 5, 6, 7, 0, 1, 2, 3]
     else:
         sw = [0, 2, 1, 3, 5, 4]
     xv[neg] = xv[neg][:, sw]
@@ -150,6 +159,13 @@ def _prisms(cells, coord_fn, dims, periodic, tri_axes=(0, 1), ext_axis=2):
     return _fix_orientation("pri", xv, vid)
 
 
+def _hexes(cells, coord_fn, dims, periodic):
+    """One hexahedron per lattice cell, vertices in the order of refelem."""
+    offs = ((np.array(refelem._VERTS["hex"]) + 1) // 2).astype(np.int64)
+    lat = cells[:, None, :] + offs[None, :, :]
+    return _fix_orientation("hex", coord_fn(lat).astype(np.float64), _grid_vid(lat, dims, periodic))
+
+
 def _renumber(mesh, numbering, seed):
     """Element numbering variants: natural, morton (of centroids), random (seeded)."""
     if numbering == "natural":
@@ -181,6 +197,26 @@ def box_tets(n, length=2 * np.pi, numbering="natural", seed=0):
     dims, per = (n, n, n), (True, True, True)
     xv, vid = _kuhn_tets(_cells(n, n, n), lambda lat: lat * h, dims, per)
     m = dict(etypes=["tet"], xv={"tet": xv}, vid={"tet": vid}, period=[length] * 3, bc_tag=None, n=n)
+    return _renumber(m, numbering, seed)
+
+
+def box_hex(n, length=1.0, numbering="natural", seed=0, warp=0.0):
+    """Periodic box of n^3 hexahedra (the paper's other mesh type).  warp > 0 displaces the
+    interior lattice smoothly (periodic sine field of relative amplitude `warp`), which makes the elements non-affine (trilinear)."""
+    h = length / n
+    dims, per = (n, n, n), (True, True, True)
+
+    def coord(lat):
+        x = lat * h
+        if warp > 0:
+            k = 2 * np.pi / length
+            d = warp * h * np.stack([np.sin(k * x[..., 1]) * np.sin(k * x[..., 2]), np.sin(k * x[..., 0]) * np.sin(k * x[..., 2]),
+                                     np.sin(k * x[..., 0]) * np.sin(k * x[..., 1])], axis=-1)
+            x = x + d
+        return x
+
+    xv, vid = _hexes(_cells(n, n, n), coord, dims, per)
+    m = dict(etypes=["hex"], xv={"hex": xv}, vid={"hex": vid}, period=[length] * 3, bc_tag=None, n=n)
     return _renumber(m, numbering, seed)
 
 

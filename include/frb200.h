@@ -40,7 +40,7 @@ typedef struct fr_ctx fr_ctx;
 typedef enum { FR_OK = 0, FR_EINVAL = 1, FR_ENOMEM = 2, FR_ECUDA = 3, FR_ESTATE = 4, FR_EUNSUPPORTED = 5 } fr_status;
 typedef enum { FR_F32 = 4, FR_F64 = 8 } fr_prec;                 /* P:23 "Precisions: Single, Double" */
 typedef enum { FR_EULER = 0, FR_NAVIER_STOKES = 1 } fr_system;   /* P:23 "Governing Systems" */
-typedef enum { FR_TET = 0, FR_PRI = 1, FR_HEX = 2 } fr_etype;    /* P:23; only FR_TET and FR_PRI are accepted by fr_setup */
+typedef enum { FR_TET = 0, FR_PRI = 1, FR_HEX = 2 } fr_etype;    /* P:23 (3-D element types of Table 1) */
 typedef enum { FR_RK4 = 0, FR_RK45_2R = 1, FR_EULER1 = 2 } fr_stepper;   /* P:23 "Time Steppers: Euler, RK4, RK45"; P:116 RK45[2R+] */
 typedef enum { FR_BC_NOSLIP_ISOTHERMAL_WALL = 0, FR_BC_CHAR_RIEMANN_INV = 1 } fr_bctype;
 typedef enum { FR_MODE_FUSED = 0, FR_MODE_UNFUSED = 1 } fr_mode; /* kernel chain: fused (default) or one kernel per step */

@@ -160,18 +160,20 @@ struct Ctx : CtxBase {
     long long utot = 0, gtot = 0;
     for (int t = 0; t < nt; ++t) {
       const fr_eles_desc &d = c->eles[t];
-      FR_REQUIRE(d.etype == FR_TET || d.etype == FR_PRI, "only tetrahedra and prisms are supported by fr_setup");
+      FR_REQUIRE(d.etype == FR_TET || d.etype == FR_PRI || d.etype == FR_HEX, "unknown element type");
       FR_REQUIRE(d.order >= 1 && d.nupts > 0 && d.nfpts > 0 && d.nfpts < 65536 && d.neles > 0 &&
-                     d.neles < (1ll << 31) - 64,
+                     d.neles < (1ll << 31) - 128,
                  "bad element counts");
       const int p = d.order;
-      const int nu = d.etype == FR_TET ? (p + 1) * (p + 2) * (p + 3) / 6 : (p + 1) * (p + 1) * (p + 2) / 2;
-      const int nf = d.etype == FR_TET ? 2 * (p + 1) * (p + 2) : (p + 1) * (p + 2) + 3 * (p + 1) * (p + 1);
+      const int nu = d.etype == FR_TET ? (p + 1) * (p + 2) * (p + 3) / 6
+                     : d.etype == FR_PRI ? (p + 1) * (p + 1) * (p + 2) / 2 : (p + 1) * (p + 1) * (p + 1);
+      const int nf = d.etype == FR_TET ? 2 * (p + 1) * (p + 2)
+                     : d.etype == FR_PRI ? (p + 1) * (p + 2) + 3 * (p + 1) * (p + 1) : 6 * (p + 1) * (p + 1);
       FR_REQUIRE(nu == d.nupts && nf == d.nfpts, "nupts / nfpts do not match the element type and order (Table 2)");
       FR_REQUIRE(d.M0 && d.M132 && d.M3 && d.smats && d.rcpdjac, "operator / metric pointers must be non-NULL");
       FR_REQUIRE(!ns || (d.M460 && d.M6), "M460 and M6 are required for Navier-Stokes");
       auto e = std::make_unique<EleData<T>>();
-      tname[t] = d.etype == FR_TET ? "tet" : "pri";
+      tname[t] = d.etype == FR_TET ? "tet" : (d.etype == FR_PRI ? "pri" : "hex");
       EleView<T> &v = e->view;
       v.nupts = nu;
       v.nfpts = nf;

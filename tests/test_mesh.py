@@ -14,6 +14,7 @@ MESHES = {
     "mixed4": lambda: M.box_mixed(4),
     "mixed4_random": lambda: M.box_mixed(4, numbering="random", seed=3),
     "cyl": lambda: M.cylinder_omesh(ntheta=16, nz=4, nlayers=5, nr=5, seed=11),
+    "hex3_warped": lambda: M.box_hex(3, numbering="random", seed=5, warp=0.12),
 }
 
 

@@ -27,6 +27,19 @@ def test_T1_freestream_and_T2_conservation_mixed(system, p):
     assert np.abs(conservation_defect(c, d)).max() < 1e-13
 
 
+@pytest.mark.parametrize("system", ["euler", "ns"])
+@pytest.mark.parametrize("p,warp", [(1, 0.0), (2, 0.0), (2, 0.12), (3, 0.12)])
+def test_T1_T2_hexahedra(system, p, warp):
+    """Hexahedra (NEXT-2): free-stream preservation and conservation, affine and warped (trilinear: the metric terms are of degree 2
+    per direction, inside Q_p for p >= 2)."""
+    c = cases.config_hex(3, p, system, mu=0.05, numbering="random", warp=warp)
+    fs = [state.freestream(e["xu"], v=(0.3, 0.2, -0.1)) for e in c["eles"]]
+    assert max(np.abs(x).max() for x in oracle_rhs(c, fs)) < 2e-11
+    d = oracle_rhs(c, state.perturb(fs, 0.05, 7, v=(0.3, 0.2, -0.1)))
+    assert max(np.abs(x).max() for x in d) > 1e-2
+    assert np.abs(conservation_defect(c, d)).max() < 1e-13
+
+
 def test_T1_T2_config1():
     c = cases.config1()
     d = oracle_rhs(c)
@@ -218,13 +231,17 @@ def _analytic_residual(mu, pr=0.72, gamma=1.4, length=1.0):
 
 @pytest.mark.parametrize("system,p,ns_,min_order", [("euler", 1, (8, 16), 0.75), ("euler", 2, (4, 8), 1.55),
                                                      ("euler", 3, (4, 8), 2.5), ("ns", 2, (4, 8), 0.6),
-                                                     ("ns", 3, (4, 8), 1.5)])
+                                                     ("ns", 3, (4, 8), 1.5), ("hex-euler", 2, (6, 12), 1.5),
+                                                     ("hex-ns", 3, (6, 12), 1.5)])
 def test_T3_T4_consistency_order(system, p, ns_, min_order):
+    hexes = system.startswith("hex-")
+    system = system.replace("hex-", "")
     mu = 0.05 if system == "ns" else 0.0
     res = _analytic_residual(mu)
     errs = []
     for n in ns_:
-        c = cases.config2(n, p, system, mu=mu, state_kind="smooth")
+        c = (cases.config_hex(n, p, system, mu=mu, state_kind="smooth", warp=0.1) if hexes
+             else cases.config2(n, p, system, mu=mu, state_kind="smooth"))
         d = oracle_rhs(c)
         num = np.zeros(5)
         for e, dd in zip(c["eles"], d):
