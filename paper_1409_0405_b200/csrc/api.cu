@@ -74,11 +74,55 @@ struct Timeline {
 };
 
 template <typename T>
+struct FusedPart {
+  PanelOp<T> op;
+  int r0 = 0, nr = 0;   // solution points r0 .. r0+nr-1
+};
+
+// Build a fused operator over `nrows` solution points as 1, 2, ... blocks (a multiple of 8 points each, as even as possible)
+// until every block fits the panel kernel.  build(op, r0, nr) -> bool.  Leaves `parts` empty if nothing fits.
+template <typename T, typename B>
+void build_split(std::vector<FusedPart<T>> &parts, int nrows, B build) {
+  for (auto &q : parts) panel_op_free(q.op);
+  parts.clear();
+  const int maxp = getenv("FRB_NO_ROWSPLIT") ? 1 : 32;
+  // FRB_FORCE_SPLIT=n: start at n blocks (parity tests of the row split on operators that would fit in one)
+  const int minp = getenv("FRB_FORCE_SPLIT") ? std::max(1, std::min(maxp, atoi(getenv("FRB_FORCE_SPLIT")))) : 1;
+  for (int np = minp; np <= maxp; ++np) {
+    const int per = np == 1 ? nrows : ((nrows + np - 1) / np + 7) / 8 * 8;
+    if (np > 1 && (long long)per * (np - 1) >= nrows) continue;
+    bool ok = true;
+    for (int r0 = 0; r0 < nrows && ok; r0 += per) {
+      FusedPart<T> q;
+      q.r0 = r0;
+      q.nr = std::min(per, nrows - r0);
+      ok = build(q.op, q.r0, q.nr);
+      if (ok) parts.push_back(q);
+    }
+    if (ok) return;
+    for (auto &q : parts) panel_op_free(q.op);
+    parts.clear();
+  }
+}
+
+template <typename T>
+double parts_density(const std::vector<FusedPart<T>> &parts) {
+  double a = 0, b = 0;
+  for (auto &q : parts) {
+    a += q.op.density * q.nr;
+    b += q.nr;
+  }
+  return b > 0 ? a / b : 1.0;
+}
+
+template <typename T>
 struct EleData {
   EleView<T> view;
   DevBuf<T> smats, rcpdjac;
   GemmPlan<T> pM0, pM132, pM3, pM460, pM6;
-  PanelOp<T> pDiv, pGrad;   // fused operators [M132 | M3] and [M460 | M6] (FR_MODE_FUSED)
+  // fused operators [M132 | M3] and [M460 | M6] (FR_MODE_FUSED); more than one entry = blocks of solution points, launched one
+  // after the other, for operators with more rows than one CTA's accumulators hold (e.g. hexahedra at p = 4)
+  std::vector<FusedPart<T>> pDiv, pGrad;
   DevBuf<T> X, Y, ACC;   // solution register, stage input, RK4 accumulator
   DevBuf<T> grad;        // [3][nupts][5][ld]: G~ -> G (-> F~ on the unfused path)
   DevBuf<T> ftil;        // [3][nupts][5][ld]: F~ written by the fused gradient kernel (NS, fused mode)
@@ -89,8 +133,8 @@ struct EleData {
     gemm_plan_free(pM3);
     gemm_plan_free(pM460);
     gemm_plan_free(pM6);
-    panel_op_free(pDiv);
-    panel_op_free(pGrad);
+    for (auto &q : pDiv) panel_op_free(q.op);
+    for (auto &q : pGrad) panel_op_free(q.op);
   }
 };
 
@@ -210,8 +254,10 @@ struct Ctx : CtxBase {
         gemm_plan_build(e->pM6, 3 * nu, nf, d.M6);
       }
       if (mode == FR_MODE_FUSED) {
-        fused_div_build(e->pDiv, nu, nf, d.M132, d.M3);
-        if (ns) fused_grad_build(e->pGrad, nu, nf, d.M460, d.M6, 0, d.M0);
+        build_split(e->pDiv, nu, [&](PanelOp<T> &op, int r0, int nr) { return fused_div_build(op, nu, nf, d.M132, d.M3, 0, r0, nr); });
+        if (ns)
+          build_split(e->pGrad, nu,
+                      [&](PanelOp<T> &op, int r0, int nr) { return fused_grad_build(op, nu, nf, d.M460, d.M6, 0, d.M0, r0, nr); });
       }
       const size_t nstate = (size_t)nu * 5 * ld;
       e->X.alloc(nstate);
@@ -222,7 +268,7 @@ struct Ctx : CtxBase {
       // parity-tested but measured slower than the stand-alone S6 kernel, which runs at the HBM roofline: the epilogue's metric and
       // state loads are latency-bound while the tensor pipe idles (profiles/r01_c_fusion_notes.md).  Off until the epilogue is
       // fed through shared memory.
-      if (kFuseFluxIntoGrad && e->pGrad.ok() && e->pDiv.ok()) e->ftil.alloc(3 * nstate);
+      if (kFuseFluxIntoGrad && !e->pGrad.empty() && !e->pDiv.empty()) e->ftil.alloc(3 * nstate);
       e->R.alloc(nstate);
       tt.ubase[t] = utot;
       tt.gbase[t] = gtot;
@@ -236,13 +282,17 @@ struct Ctx : CtxBase {
     if (mode == FR_MODE_FUSED && ns) {
       // the jump formulation of S2 needs every type on the fused gradient kernel; otherwise fall back to C itself
       bool all = true;
-      for (int t = 0; t < nt; ++t) all = all && el[t]->pGrad.ok();
+      for (int t = 0; t < nt; ++t) all = all && !el[t]->pGrad.empty();
       if (all) {
         jump = 1;
       } else {
         for (int t = 0; t < nt; ++t)
-          if (el[t]->pGrad.ok())
-            fused_grad_build(el[t]->pGrad, el[t]->view.nupts, el[t]->view.nfpts, c->eles[t].M460, c->eles[t].M6, 0, nullptr);
+          if (!el[t]->pGrad.empty()) {
+            const fr_eles_desc &d = c->eles[t];
+            build_split(el[t]->pGrad, d.nupts, [&](PanelOp<T> &op, int r0, int nr) {
+              return fused_grad_build(op, d.nupts, d.nfpts, d.M460, d.M6, 0, nullptr, r0, nr);
+            });
+          }
       }
     }
     uf.alloc(utot);
@@ -322,15 +372,18 @@ struct Ctx : CtxBase {
              [&](const PanelOp<T> &op) { panel_gemm_run(op, n5, T(1), (const T *)e.X.p, n5, 0, T(0), ufp, n5, 0, 1, stream); },
              (tag + ":M0").c_str());
       StageArgs<T> plain{nullptr, nullptr, nullptr, e.R.p, nullptr};
-      tune(e.pDiv, [&](PanelOp<T> &op, int k) { return fused_div_build(op, nu, nf, d.M132, d.M3, k); },
-           [&](const PanelOp<T> &op) { launch_fused_div(op, e.view, (const T *)e.grad.p, (const T *)ufp, plain, stream); },
-           (tag + ":[M132|M3]").c_str());
+      for (auto &q : e.pDiv)
+        tune(q.op, [&](PanelOp<T> &op, int k) { return fused_div_build(op, nu, nf, d.M132, d.M3, k, q.r0, q.nr); },
+             [&](const PanelOp<T> &op) { launch_fused_div(op, e.view, (const T *)e.grad.p, (const T *)ufp, plain, stream); },
+             (tag + ":[M132|M3]").c_str());
       if (ns)
-        tune(e.pGrad, [&](PanelOp<T> &op, int k) { return fused_grad_build(op, nu, nf, d.M460, d.M6, k, jump ? d.M0 : nullptr); },
-             [&](const PanelOp<T> &op) {
-               launch_fused_grad(op, e.view, (const T *)e.X.p, (const T *)(cf.p + tt.ubase[t]), e.grad.p, (T *)nullptr, ph, stream);
-             },
-             (tag + ":[M460|M6]").c_str());
+        for (auto &q : e.pGrad)
+          tune(q.op,
+               [&](PanelOp<T> &op, int k) { return fused_grad_build(op, nu, nf, d.M460, d.M6, k, jump ? d.M0 : nullptr, q.r0, q.nr); },
+               [&](const PanelOp<T> &op) {
+                 launch_fused_grad(op, e.view, (const T *)e.X.p, (const T *)(cf.p + tt.ubase[t]), e.grad.p, (T *)nullptr, ph, stream);
+               },
+               (tag + ":[M460|M6]").c_str());
     }
     FR_CUDA_TRY(cudaStreamSynchronize(stream));
   }
@@ -466,14 +519,14 @@ struct Ctx : CtxBase {
         const long long n5 = 5 * e.view.ld;
         const double n = (double)e.view.neles, nu = e.view.nupts, nf = e.view.nfpts;
         const double nmet = e.view.affine ? 1 : nu;
-        if (e.pGrad.ok()) {
+        if (!e.pGrad.empty()) {
           // S3 + S4 fused: G = (1/|J|) S^T ([M460 | M6] [U; C])
           // S3 + S4 (+S6) fused: G = (1/|J|) S^T ([M460 | M6] [U; C]);  F~ = S (f_inv(U) - f_visc(U, G))
-          nk += launch_fused_grad(e.pGrad, e.view, u[t], cf.p + tt.ubase[t], e.grad.p, e.ftil.p, ph, s);
+          for (auto &q : e.pGrad) nk += launch_fused_grad(q.op, e.view, u[t], cf.p + tt.ubase[t], e.grad.p, e.ftil.p, ph, s);
           const bool fl = e.ftil.p != nullptr;
           mark(CAT_GEMM, t, fl ? "S3_S4_S6_fused_grad_flux" : "S3_S4_fused_grad",
                (5 * nu + 5 * nf + 15 * nu + 10 * nmet + (fl ? 15 * nu : 0)) * n,
-               2 * e.pGrad.density * 3 * nu * (nu + nf) * 5 * n + 15 * 6 * nu * n + (fl ? 210 * nu * n : 0));
+               2 * parts_density(e.pGrad) * 3 * nu * (nu + nf) * 5 * n + 15 * 6 * nu * n + (fl ? 210 * nu * n : 0));
         } else {
           // S3: G~ = M460 U + M6 C
           nk += gemm_run(e.pM460, n5, T(1), u[t], n5, 0, T(0), e.grad.p, n5, 0, 1, s);
@@ -507,12 +560,12 @@ struct Ctx : CtxBase {
         mark(CAT_PW, t, "S6_tdisf", ((ns ? 35 : 20) * nu + 9 * nmet) * n, (ns ? 210 : 110) * nu * n);
         ft = e.grad.p;
       }
-      if (e.pDiv.ok()) {
+      if (!e.pDiv.empty()) {
         // S8 + S9 (+S10) fused: out = -(1/|J|) [M132 | M3] [F~; D], stage update in the epilogue
-        nk += launch_fused_div(e.pDiv, e.view, ft, uf.p + tt.ubase[t], sa[t], s);
+        for (auto &q : e.pDiv) nk += launch_fused_div(q.op, e.view, ft, uf.p + tt.ubase[t], sa[t], s);
         const double rk = sa[t].coef ? (sa[t].out2 ? 15 : 10) : 5;
         mark(CAT_GEMM, t, sa[t].coef ? "S8_S9_S10_fused_div_rk" : "S8_S9_fused_div", (15 * nu + 5 * nf + rk * nu + nmet) * n,
-             2 * e.pDiv.density * nu * (3 * nu + nf) * 5 * n + 5 * nu * n);
+             2 * parts_density(e.pDiv) * nu * (3 * nu + nf) * 5 * n + 5 * nu * n);
         continue;
       }
       // S8: R = M132 F~ + M3 D

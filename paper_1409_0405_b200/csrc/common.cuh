@@ -72,6 +72,12 @@ struct GemmPlan {
   size_t smem = 0;
   T *At = nullptr;               // device, [nrb][K][TY*MT], zero padded, transposed operator
   PanelOp<T> *pop = nullptr;     // non-null: the panel kernel serves this operator (At is then unused)
+  // operators with too many rows for one CTA: row blocks of A, each its own panel operator, launched one after the other
+  // (B is read once per block: these are the compute-bound shapes)
+  static constexpr int kMaxParts = 32;
+  int nparts = 0;
+  PanelOp<T> *part[kMaxParts] = {};
+  int part_row0[kMaxParts] = {};
 };
 
 template <typename T>

@@ -256,7 +256,8 @@ void gemm_plan_build(GemmPlan<T> &p, int M, int K, const double *A_host) {
   constexpr int CT = VecT<T>::CT;
   p.M = M;
   p.K = K;
-  {
+  const int force_split = getenv("FRB_FORCE_SPLIT") ? atoi(getenv("FRB_FORCE_SPLIT")) : 0;
+  if (force_split < 2 || M < 16) {
     // preferred path: operator resident in shared memory, all rows in one CTA (panel.cuh)
     auto *pop = new PanelOp<T>();
     bool ok = false;
@@ -271,6 +272,32 @@ void gemm_plan_build(GemmPlan<T> &p, int M, int K, const double *A_host) {
       return;
     }
     delete pop;
+  }
+  // row blocks of A on the panel kernel (rows per block a multiple of 8, as even as possible)
+  for (int np = std::max(2, force_split); np <= GemmPlan<T>::kMaxParts && getenv("FRB_NO_ROWSPLIT") == nullptr; ++np) {
+    const int per = ((M + np - 1) / np + 7) / 8 * 8;
+    if ((long long)per * (np - 1) >= M) continue;
+    bool ok = true;
+    int n = 0;
+    for (int r0 = 0; r0 < M && ok; r0 += per, ++n) {
+      auto *pop = new PanelOp<T>();
+      p.part[n] = pop;
+      p.part_row0[n] = r0;
+      try {
+        ok = panel_gemm_build(*pop, std::min(per, M - r0), K, A_host + (size_t)r0 * K);
+      } catch (...) {
+        ok = false;
+      }
+    }
+    if (ok) {
+      p.nparts = n;
+      return;
+    }
+    for (int i = 0; i < n; ++i) {
+      panel_op_free(*p.part[i]);
+      delete p.part[i];
+      p.part[i] = nullptr;
+    }
   }
   double best = 1e300;
   const int tys[3] = {4, 6, 8};
@@ -318,6 +345,12 @@ void gemm_plan_free(GemmPlan<T> &p) {
     delete p.pop;
     p.pop = nullptr;
   }
+  for (int i = 0; i < p.nparts; ++i) {
+    panel_op_free(*p.part[i]);
+    delete p.part[i];
+    p.part[i] = nullptr;
+  }
+  p.nparts = 0;
 }
 
 template <typename T>
@@ -332,6 +365,11 @@ int gemm_run(const GemmPlan<T> &p, long long N, T c1, const T *B, long long ldb,
   if (p.pop) {
     panel_gemm_run(*p.pop, N, c1, B, ldb, bstrideB, c2, C, ldc, bstrideC, nbatch, s);
     return 1;
+  }
+  if (p.nparts > 0) {
+    for (int i = 0; i < p.nparts; ++i)
+      panel_gemm_run(*p.part[i], N, c1, B, ldb, bstrideB, c2, C + (long long)p.part_row0[i] * ldc, ldc, bstrideC, nbatch, s);
+    return p.nparts;
   }
   GemmArgs<T> a;
   a.M = p.M;

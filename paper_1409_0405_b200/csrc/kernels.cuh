@@ -60,12 +60,13 @@ int launch_bc_comm_flux(const BndView<T> &bv, const TypeTab &tt, T *uf, const T 
 
 // Fused panel kernels (panel_fused.cu).  *_build return false if the operator does not fit the resident design.
 template <typename T>
-bool fused_div_build(PanelOp<T> &op, int nu, int nf, const double *M132, const double *M3, int cand = 0);
+bool fused_div_build(PanelOp<T> &op, int nu, int nf, const double *M132, const double *M3, int cand = 0, int r0 = 0, int nr = -1);
 template <typename T>
 int launch_fused_div(const PanelOp<T> &op, const EleView<T> &ev, const T *ftil, const T *d, const StageArgs<T> &sa,
                      cudaStream_t s);
 template <typename T>
-bool fused_grad_build(PanelOp<T> &op, int nu, int nf, const double *M460, const double *M6, int cand = 0, const double *M0_jump = nullptr);
+bool fused_grad_build(PanelOp<T> &op, int nu, int nf, const double *M460, const double *M6, int cand = 0, const double *M0_jump = nullptr,
+                      int r0 = 0, int nr = -1);
 template <typename T>
 int launch_fused_grad(const PanelOp<T> &op, const EleView<T> &ev, const T *u, const T *c, T *grad, T *ftil,
                       const PhysParams<T> &ph, cudaStream_t s);

@@ -212,6 +212,7 @@ struct PackOptions {
   int allow_sparse = 1;
   int curved = 0;          // flux sources: per-point metric terms
   int cand = 0;            // k-th best geometry by static score (autotuning)
+  const int *row_ids = nullptr;   // row split: the epilogue's row number of each row of A (nullptr = 0..M-1)
 };
 
 // Pack A (M x K, host FP64, row-major) for the panel kernels.  `srcs` stacks the K dimension.  Returns false if the
@@ -391,7 +392,10 @@ bool panel_op_build_kc(PanelOp<T> &p, int M, int K, const double *A, const std::
   std::vector<int> rowmap(NS * 8, -1);
   for (int s = 0; s < NS; ++s)
     if (slot_group[s] >= 0)
-      for (int r = 0; r < 8; ++r) rowmap[s * 8 + r] = order[8 * slot_group[s] + r];
+      for (int r = 0; r < 8; ++r) {
+        const int m = order[8 * slot_group[s] + r];
+        rowmap[s * 8 + r] = (m >= 0 && opt.row_ids) ? opt.row_ids[m] : m;
+      }
   long long macs = 0;
   int nblk = 0;
   if (!sparse) {

@@ -315,19 +315,28 @@ void launch_panel(K k, const A &a, int nthreads, size_t smem, long long ntot, in
 }  // namespace
 
 template <typename T>
-bool fused_div_build(PanelOp<T> &op, int nu, int nf, const double *M132, const double *M3, int cand) {
+bool fused_div_build(PanelOp<T> &op, int nu, int nf, const double *M132, const double *M3, int cand, int r0, int nr) {
+  // rows r0 .. r0+nr-1 of [M132 | M3] (nr < 0: all); the epilogue sees the solution-point numbers through the row map
+  if (nr < 0) {
+    r0 = 0;
+    nr = nu;
+  }
   const int K = 3 * nu + nf;
-  std::vector<double> A((size_t)nu * K);
-  for (int m = 0; m < nu; ++m) {
-    for (int k = 0; k < 3 * nu; ++k) A[(size_t)m * K + k] = M132[(size_t)m * 3 * nu + k];
-    for (int k = 0; k < nf; ++k) A[(size_t)m * K + 3 * nu + k] = M3[(size_t)m * nf + k];
+  std::vector<double> A((size_t)nr * K);
+  std::vector<int> ids(nr);
+  for (int j = 0; j < nr; ++j) {
+    const int m = r0 + j;
+    ids[j] = m;
+    for (int k = 0; k < 3 * nu; ++k) A[(size_t)j * K + k] = M132[(size_t)m * 3 * nu + k];
+    for (int k = 0; k < nf; ++k) A[(size_t)j * K + 3 * nu + k] = M3[(size_t)m * nf + k];
   }
   std::vector<KSource> srcs{KSource{3 * nu, KIND_PLAIN, 1}, KSource{nf, KIND_PLAIN, 1}};
   PackOptions opt;
   opt.min_ne = 16;
   opt.max_ne = sizeof(T) == 8 ? 64 : 128;
   opt.cand = cand;
-  return panel_op_build(op, nu, K, A.data(), srcs, opt, 150 * 1024);
+  opt.row_ids = ids.data();
+  return panel_op_build(op, nr, K, A.data(), srcs, opt, 150 * 1024);
 }
 
 template <typename T>
@@ -358,26 +367,37 @@ int launch_fused_div(const PanelOp<T> &op, const EleView<T> &ev, const T *ftil, 
 }
 
 template <typename T>
-bool fused_grad_build(PanelOp<T> &op, int nu, int nf, const double *M460, const double *M6, int cand, const double *M0_jump) {
-  const int K = nu + nf, M = 3 * nu;
-  std::vector<double> A((size_t)M * K);
-  for (int m = 0; m < M; ++m) {
-    for (int k = 0; k < nu; ++k) A[(size_t)m * K + k] = M460[(size_t)m * nu + k];
-    for (int k = 0; k < nf; ++k) A[(size_t)m * K + nu + k] = M6[(size_t)m * nf + k];
-    // jump formulation (k_con_u): the second operand is C - U_f, so the first block is M4 = M460 + M6 M0
-    if (M0_jump)
-      for (int k = 0; k < nu; ++k) {
-        double acc = 0;
-        for (int j = 0; j < nf; ++j) acc += M6[(size_t)m * nf + j] * M0_jump[(size_t)j * nu + k];
-        A[(size_t)m * K + k] += acc;
-      }
+bool fused_grad_build(PanelOp<T> &op, int nu, int nf, const double *M460, const double *M6, int cand, const double *M0_jump,
+                      int r0, int nr) {
+  // rows (alpha, rho), rho = r0 .. r0+nr-1, of [M460 | M6] (nr < 0: all rho), alpha-major as triple packing wants them
+  if (nr < 0) {
+    r0 = 0;
+    nr = nu;
   }
+  const int K = nu + nf, M = 3 * nr;
+  std::vector<double> A((size_t)M * K);
+  std::vector<int> ids(M);
+  for (int a = 0; a < 3; ++a)
+    for (int j = 0; j < nr; ++j) {
+      const int ml = a * nr + j, m = a * nu + r0 + j;
+      ids[ml] = m;
+      for (int k = 0; k < nu; ++k) A[(size_t)ml * K + k] = M460[(size_t)m * nu + k];
+      for (int k = 0; k < nf; ++k) A[(size_t)ml * K + nu + k] = M6[(size_t)m * nf + k];
+      // jump formulation (k_con_u): the second operand is C - U_f, so the first block is M4 = M460 + M6 M0
+      if (M0_jump)
+        for (int k = 0; k < nu; ++k) {
+          double acc = 0;
+          for (int i = 0; i < nf; ++i) acc += M6[(size_t)m * nf + i] * M0_jump[(size_t)i * nu + k];
+          A[(size_t)ml * K + k] += acc;
+        }
+    }
   std::vector<KSource> srcs{KSource{nu, KIND_PLAIN, 1}, KSource{nf, KIND_PLAIN, 1}};
   PackOptions opt;
   opt.min_ne = 16;
   opt.max_ne = sizeof(T) == 8 ? 64 : 128;
   opt.triple = 1;
   opt.cand = cand;
+  opt.row_ids = ids.data();
   return panel_op_build(op, M, K, A.data(), srcs, opt, 150 * 1024);
 }
 
@@ -410,10 +430,10 @@ int launch_fused_grad(const PanelOp<T> &op, const EleView<T> &ev, const T *u, co
 }
 
 #define FR_INST(T)                                                                                                          \
-  template bool fused_div_build<T>(PanelOp<T> &, int, int, const double *, const double *, int);                             \
+  template bool fused_div_build<T>(PanelOp<T> &, int, int, const double *, const double *, int, int, int);                             \
   template int launch_fused_div<T>(const PanelOp<T> &, const EleView<T> &, const T *, const T *, const StageArgs<T> &,     \
                                    cudaStream_t);                                                                          \
-  template bool fused_grad_build<T>(PanelOp<T> &, int, int, const double *, const double *, int, const double *);                             \
+  template bool fused_grad_build<T>(PanelOp<T> &, int, int, const double *, const double *, int, const double *, int, int);                             \
   template int launch_fused_grad<T>(const PanelOp<T> &, const EleView<T> &, const T *, const T *, T *, T *,                \
                                     const PhysParams<T> &, cudaStream_t);
 FR_INST(double)

@@ -43,7 +43,7 @@ def _check_rhs(case, prec, mode):
 # ---------------------------------------------------------------------------- T7: the operator product alone
 @pytest.mark.parametrize("prec", ["f64", "f32"])
 @pytest.mark.parametrize("M,K", [(24, 10), (10, 30), (4, 12), (60, 35), (35, 105), (105, 75), (225, 75), (75, 225),
-                                 (294, 343), (1, 1), (17, 3)])
+                                 (294, 343), (1, 1), (17, 3), (375, 125), (588, 196), (196, 588), (1029, 343)])
 def test_T7_gemm_vs_numpy(prec, M, K):
     import torch
     from paper_1409_0405_b200 import binding
@@ -250,6 +250,28 @@ def test_candidate_geometries_parity(cand, monkeypatch):
             _check_rhs(case, prec, "fused")
 
 
+# ---------------------------------------------------------------------------- row split of operators too tall for one CTA
+@pytest.mark.parametrize("nsplit", [2, 3, 5])
+def test_row_split_parity(nsplit, monkeypatch):
+    """FRB_FORCE_SPLIT=n makes every operator (plain, fused gradient, fused divergence + RK) run as n or more row blocks, the
+    path tall operators (hexahedra p >= 4, p >= 5 prisms) take.  Right-hand side and one RK45 step of the mixed config-2 mesh."""
+    from oracle import fr_oracle as O
+    monkeypatch.setenv("FRB_FORCE_SPLIT", str(nsplit))
+    case = cases.config2(6, 3, "ns", numbering="random")
+    for prec in ("f64", "f32"):
+        for mode in ("fused", "unfused"):
+            _check_rhs(case, prec, mode)
+    f = lambda us: O.rhs(case["cfg"], case["eles"], case["ifc"], case["bcs"], us)
+    ref = O.rk45_step(f, case["u0"], 1e-4)
+    ctx = _ctx(case, "f64", stepper="rk45")
+    ctx.set_state(case["u0"])
+    ctx.rk_step(1e-4)
+    got = ctx.get_state()
+    err, _ = field_errors([a - b for a, b in zip(got, case["u0"])], [a - b for a, b in zip(ref, case["u0"])])
+    assert np.all(err <= 1e-9), err
+    ctx.close()
+
+
 # ---------------------------------------------------------------------------- hexahedra (SURVEY 8(f) NEXT-2)
 @pytest.mark.parametrize("mode", ["unfused", "fused"])
 @pytest.mark.parametrize("prec", ["f64", "f32"])
@@ -258,7 +280,7 @@ def test_candidate_geometries_parity(cand, monkeypatch):
 def test_hex_rhs(p, system, prec, mode):
     """Periodic box of 5^3 hexahedra, warped (trilinear, per-point metrics) and randomly numbered; the Q_p operators are 4-25 %
     dense and take the k-list packing.  At p = 4 the gradient operator (375 rows) exceeds the accumulator budget of one CTA and
-    the library falls back to separate products."""
+    runs as blocks of solution points (row split, api.cu build_split)."""
     case = cases.config_hex(5, p, system, numbering="random", warp=0.12)
     _check_rhs(case, prec, mode)
 
