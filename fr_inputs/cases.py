@@ -18,7 +18,7 @@ def build_case(m, p, system="euler", gamma=state.GAMMA, mu=0.0, prandtl=0.72, ld
     eles, geo = [], {}
     for t in m["etypes"]:
         ops = refelem.operators(t, p)
-        g = _mesh.geometry(t, p, m["xv"][t])
+        g = _mesh.geometry(t, p, m["xq"][t] if "xq" in m else m["xv"][t])
         geo[t] = g
         e = dict(etype=t, order=p, nupts=ops["nupts"], nfpts=ops["nfpts"], neles=m["xv"][t].shape[0],
                  affine=g["affine"], smats=g["smats"], rcpdjac=g["rcpdjac"], djac=g["djac"], xu=g["xu"],
@@ -56,10 +56,11 @@ def config1(numbering="natural"):
     return case
 
 
-def config2(n=16, p=3, system="ns", mu=1e-3, numbering="natural", state_kind="vortex"):
+def config2(n=16, p=3, system="ns", mu=1e-3, numbering="natural", state_kind="vortex", curve=0.0):
     """BASELINE.json configs[1]: periodic unit box, n^3 cells, lower half prisms / upper half tets
-    (reading R18 for the counts), NS mu=1e-3 Pr=0.72, LDG beta=1/2 tau=0.1, isentropic vortex."""
-    m = _mesh.box_mixed(n, 1.0, numbering=numbering, seed=SEEDS["c2"])
+    (reading R18 for the counts), NS mu=1e-3 Pr=0.72, LDG beta=1/2 tau=0.1, isentropic vortex.
+    curve > 0: the same mesh with quadratically curved elements."""
+    m = _mesh.box_mixed(n, 1.0, numbering=numbering, seed=SEEDS["c2"], curve=curve)
     case = build_case(m, p, system=system, mu=mu if system == "ns" else 0.0)
     if state_kind == "vortex":
         case["u0"] = [state.isentropic_vortex(e["xu"]) for e in case["eles"]]
@@ -79,11 +80,11 @@ def config_hex(n=8, p=3, system="ns", mu=1e-3, numbering="natural", warp=0.0, st
     return case
 
 
-def config3(p=4, ntheta=100, nz=15, nlayers=40, nr=40, numbering="morton", system="ns", amp=0.005, seed=None):
+def config3(p=4, ntheta=100, nz=15, nlayers=40, nr=40, numbering="morton", system="ns", amp=0.005, seed=None, quadratic=False):
     """BASELINE.json configs[2] (and [4] when scaled): cylinder-like O-mesh, NS at Re=3900, M=0.2
     (PAPER.md:86-94,116), wall T_w = T_inf, far field = freestream, seeded 0.5 % perturbation."""
     seed = SEEDS["c3"] if seed is None else seed
-    m = _mesh.cylinder_omesh(ntheta, nz, nlayers, nr, numbering=numbering, seed=seed)
+    m = _mesh.cylinder_omesh(ntheta, nz, nlayers, nr, numbering=numbering, seed=seed, quadratic=quadratic)
     gamma, mach = state.GAMMA, 0.2
     fs = dict(rho=1.0, v=(1.0, 0.0, 0.0), p=1.0 / (gamma * mach * mach))
     e_w = fs["p"] / ((gamma - 1) * fs["rho"])

@@ -10,6 +10,7 @@ BASELINE.json configs[0..2] describe (recipe in DESIGN.md "Input recipe", SURVEY
 A mesh is a dict:
   etypes : list of element-type names; position = index into `eles[]` of the C ABI
   xv     : {etype: [N_e, n_vert, 3] float64 vertex coordinates (unwrapped across periodic seams)}
+  xq     : optional {etype: [N_e, n_quad, 3]} quadratic node coordinates (`quad_nodes` order; the first n_vert are xv)
   vid    : {etype: [N_e, n_vert] int64 global vertex ids, identical across periodic images}
   period : length-3 list, period length per direction or None
   bc_tag : callable(face centroid [n,3]) -> int tag array, or None if the mesh is fully periodic
@@ -51,6 +52,74 @@ def shape(etype, x):
     raise ValueError(etype)
 
 
+# quadratic (second-order, "quadratically curved") geometry: P2 tetrahedra (10 nodes), P2(tri) x P2(line) prisms
+# (18 nodes), Q2 hexahedra (27 nodes).  Node order: the vertices first (order of `shape`), then the remaining nodes.
+def _quad_exponents(etype):
+    rng3 = range(3)
+    if etype == "tet":
+        return [(a, b, c) for a in rng3 for b in rng3 for c in rng3 if a + b + c <= 2]
+    if etype == "pri":
+        return [(a, b, c) for a in rng3 for b in rng3 for c in rng3 if a + b <= 2]
+    if etype == "hex":
+        return [(a, b, c) for a in rng3 for b in rng3 for c in rng3]
+    raise ValueError(etype)
+
+
+def quad_nodes(etype):
+    """Reference coordinates [nq, 3] of the quadratic nodes: vertices, then edge midpoints (and, prism / hex, the face and
+    cell centres that the tensor-product spaces carry)."""
+    v = np.array(refelem._VERTS[etype], dtype=np.float64)
+    if etype == "tet":
+        rest = [(v[i] + v[j]) / 2 for i in range(4) for j in range(i + 1, 4)]
+    elif etype == "pri":
+        tri = v[:3, :2]
+        t6 = [tri[0], tri[1], tri[2], (tri[0] + tri[1]) / 2, (tri[1] + tri[2]) / 2, (tri[0] + tri[2]) / 2]
+        allp = [np.array([q[0], q[1], t]) for t in (-1.0, 1.0, 0.0) for q in t6]
+        rest = [q for q in allp if not any(np.allclose(q, w) for w in v)]
+    else:
+        allp = [np.array([a, b, c]) for c in (-1.0, 0.0, 1.0) for b in (-1.0, 0.0, 1.0) for a in (-1.0, 0.0, 1.0)]
+        rest = [q for q in allp if not any(np.allclose(q, w) for w in v)]
+    return np.concatenate([v, np.array(rest)], axis=0)
+
+
+def shape2(etype, x):
+    """Quadratic nodal shape functions N [npts, nq] on `quad_nodes(etype)` and reference gradients dN [npts, nq, 3]."""
+    x = np.asarray(x, dtype=np.float64)
+    ex = _quad_exponents(etype)
+
+    def mono(y):
+        return np.stack([y[:, 0] ** a * y[:, 1] ** b * y[:, 2] ** c for a, b, c in ex], axis=1)
+
+    def dmono(y):
+        cols = []
+        for a, b, c in ex:
+            d0 = a * y[:, 0] ** max(a - 1, 0) * y[:, 1] ** b * y[:, 2] ** c if a else np.zeros(len(y))
+            d1 = b * y[:, 0] ** a * y[:, 1] ** max(b - 1, 0) * y[:, 2] ** c if b else np.zeros(len(y))
+            d2 = c * y[:, 0] ** a * y[:, 1] ** b * y[:, 2] ** max(c - 1, 0) if c else np.zeros(len(y))
+            cols.append(np.stack([d0, d1, d2], axis=1))
+        return np.stack(cols, axis=1)           # [npts, nmono, 3]
+
+    Vinv = np.linalg.inv(mono(quad_nodes(etype)))
+    return mono(x) @ Vinv, np.einsum("pma,mq->pqa", dmono(x), Vinv)
+
+
+_NQUAD = {10: "tet", 18: "pri", 27: "hex"}
+
+
+def curve_nodes(etype, xv, lat, fn, wfn=None):
+    """Quadratic node coordinates [N_e, nq, 3] of elements that are straight in the parameter space `lat` ([N_e, nv, 3]) of a smooth
+    map `fn`:  x_q = fn(lat_q) + sum_v N_v(q) (xv_v - fn(lat_v)),  lat_q = sum_v N_v(q) lat_v  (N = linear vertex shape functions).
+    Vertices stay where they are; edge, face and cell nodes follow the map, so neighbours (which share the vertices, hence the
+    parameter-space positions, of their common face) stay conforming.  `wfn(lat_q)` in [0, 1] optionally scales the departure
+    from the straight element (1 = follow the map, 0 = stay straight), e.g. to curve only the elements near a wall."""
+    N, _ = shape(etype, quad_nodes(etype))
+    latq = np.einsum("qv,evi->eqi", N, lat)
+    bend = fn(latq) - np.einsum("qv,evi->eqi", N, fn(lat))
+    if wfn is not None:
+        bend = bend * wfn(latq)[..., None]
+    return np.einsum("qv,evi->eqi", N, xv) + bend
+
+
 def _adjugate(J):
     """J [..., 3(i), 3(alpha)] -> S [..., 3(alpha), 3(i)] = det(J) * inv(J), and det(J)."""
     a, b, c = J[..., :, 0], J[..., :, 1], J[..., :, 2]
@@ -67,8 +136,12 @@ def geometry(etype, p, xv):
     outward normals, fmag [N_f,N_e] = |S^T n_ref|, affine (bool: J constant in each element).
     """
     ops = refelem.operators(etype, p)
-    Nu, dNu = shape(etype, ops["upts"])
-    Nf, dNf = shape(etype, ops["fpts"])
+    quadratic = xv.shape[1] in _NQUAD
+    if quadratic and _NQUAD[xv.shape[1]] != etype:
+        raise ValueError("node count does not match the element type")
+    sh = shape2 if quadratic else shape
+    Nu, dNu = sh(etype, ops["upts"])
+    Nf, dNf = sh(etype, ops["fpts"])
     xu = np.einsum("pv,evi->pei", Nu, xv)
     xf = np.einsum("pv,evi->pei", Nf, xv)
     Ju = np.einsum("pva,evi->peia", dNu, xv)
@@ -79,7 +152,7 @@ def geometry(etype, p, xv):
     Sf, _ = _adjugate(Jf)
     m = np.einsum("peai,pa->pei", Sf, ops["fnorm"])
     mag = np.sqrt(np.einsum("pei,pei->pe", m, m))
-    affine = etype == "tet" or bool(np.allclose(Ju, Ju[:1], rtol=0, atol=1e-14 * np.abs(Ju).max()))
+    affine = (etype == "tet" and not quadratic) or bool(np.allclose(Ju, Ju[:1], rtol=0, atol=1e-14 * np.abs(Ju).max()))
     return dict(xu=xu, xf=xf, smats=np.ascontiguousarray(S.transpose(2, 3, 0, 1)), rcpdjac=1.0 / det, djac=det,
                 fnorm=np.ascontiguousarray((m / mag[..., None]).transpose(0, 2, 1)), fmag=mag, affine=affine)
 
@@ -106,9 +179,10 @@ for _perm in itertools.permutations(range(3)):
 _PRISM_TRIS = [np.array([[0, 0], [1, 0], [1, 1]]), np.array([[0, 0], [1, 1], [0, 1]])]
 
 
-def _fix_orientation(etype, xv, vid, xref=None):
+def _fix_orientation(etype, xv, vid, xref=None, lat=None):
     """Swap two vertices of negatively oriented elements (keeps the vertex set, hence the faces).
-    The orientation is read from `xref` (e.g. the unjittered coordinates) when given."""
+    The orientation is read from `xref` (e.g. the unjittered coordinates) when given.  `lat` (the lattice positions of the
+    vertices, wanted by `curve_nodes`) is permuted alongside and returned as a third value when given."""
     _, dN = shape(etype, np.zeros((1, 3)))
     J = np.einsum("va,evi->eia", dN[0], xv if xref is None else xref)
     neg = np.linalg.det(J) < 0
@@ -120,6 +194,10 @@ def _fix_orientation(etype, xv, vid, xref=None):
         sw = [0, 2, 1, 3, 5, 4]
     xv[neg] = xv[neg][:, sw]
     vid[neg] = vid[neg][:, sw]
+    if lat is not None:
+        lat = lat.astype(np.float64)
+        lat[neg] = lat[neg][:, sw]
+        return xv, vid, lat
     return xv, vid
 
 
@@ -128,10 +206,11 @@ def _cells(nx, ny, nz):
     return np.stack([i.ravel(), j.ravel(), k.ravel()], axis=1)
 
 
-def _kuhn_tets(cells, coord_fn, dims, periodic, orient_fn=None):
-    xs, ids, x0 = [], [], []
+def _kuhn_tets(cells, coord_fn, dims, periodic, orient_fn=None, want_lat=False):
+    xs, ids, x0, lats = [], [], [], []
     for offs in _KUHN:
         lat = cells[:, None, :] + offs[None, :, :]
+        lats.append(lat)
         xs.append(coord_fn(lat))
         if orient_fn is not None:
             x0.append(orient_fn(lat))
@@ -139,12 +218,12 @@ def _kuhn_tets(cells, coord_fn, dims, periodic, orient_fn=None):
     xv = np.stack(xs, axis=1).reshape(-1, 4, 3)
     vid = np.stack(ids, axis=1).reshape(-1, 4)
     xref = np.stack(x0, axis=1).reshape(-1, 4, 3) if orient_fn is not None else None
-    return _fix_orientation("tet", xv, vid, xref)
+    return _fix_orientation("tet", xv, vid, xref, np.stack(lats, axis=1).reshape(-1, 4, 3) if want_lat else None)
 
 
-def _prisms(cells, coord_fn, dims, periodic, tri_axes=(0, 1), ext_axis=2):
+def _prisms(cells, coord_fn, dims, periodic, tri_axes=(0, 1), ext_axis=2, want_lat=False):
     """Two prisms per lattice cell: triangles in the (tri_axes) plane, extruded along ext_axis."""
-    xs, ids = [], []
+    xs, ids, lats = [], [], []
     for tri in _PRISM_TRIS:
         offs = np.zeros((6, 3), dtype=np.int64)
         for lvl in range(2):
@@ -152,11 +231,12 @@ def _prisms(cells, coord_fn, dims, periodic, tri_axes=(0, 1), ext_axis=2):
             offs[3 * lvl:3 * lvl + 3, tri_axes[1]] = tri[:, 1]
             offs[3 * lvl:3 * lvl + 3, ext_axis] = lvl
         lat = cells[:, None, :] + offs[None, :, :]
+        lats.append(lat)
         xs.append(coord_fn(lat))
         ids.append(_grid_vid(lat, dims, periodic))
     xv = np.stack(xs, axis=1).reshape(-1, 6, 3)
     vid = np.stack(ids, axis=1).reshape(-1, 6)
-    return _fix_orientation("pri", xv, vid)
+    return _fix_orientation("pri", xv, vid, None, np.stack(lats, axis=1).reshape(-1, 6, 3) if want_lat else None)
 
 
 def _hexes(cells, coord_fn, dims, periodic):
@@ -188,6 +268,8 @@ def _renumber(mesh, numbering, seed):
             raise ValueError(numbering)
         mesh["xv"][t] = np.ascontiguousarray(mesh["xv"][t][perm])
         mesh["vid"][t] = np.ascontiguousarray(mesh["vid"][t][perm])
+        if "xq" in mesh:
+            mesh["xq"][t] = np.ascontiguousarray(mesh["xq"][t][perm])
     return mesh
 
 
@@ -220,8 +302,21 @@ def box_hex(n, length=1.0, numbering="natural", seed=0, warp=0.0):
     return _renumber(m, numbering, seed)
 
 
-def box_mixed(n, length=1.0, numbering="natural", seed=0):
-    """Config 2 (BASELINE.json configs[1]): periodic box, cells with k < n/2 -> 2 prisms (axis z), others -> 6 tets."""
+def _sine_bump(length, amp):
+    """x -> x + amp * (periodic sine field): the smooth map the box generators curve their elements with."""
+    k = 2 * np.pi / length
+
+    def fn(x):
+        d = np.stack([np.sin(k * x[..., 1]) * np.sin(k * x[..., 2]), np.sin(k * x[..., 0]) * np.sin(k * x[..., 2]),
+                      np.sin(k * x[..., 0]) * np.sin(k * x[..., 1])], axis=-1)
+        return x + amp * d
+    return fn
+
+
+def box_mixed(n, length=1.0, numbering="natural", seed=0, curve=0.0):
+    """Config 2 (BASELINE.json configs[1]): periodic box, cells with k < n/2 -> 2 prisms (axis z), others -> 6 tets.
+    curve > 0: quadratically curved elements -- the vertices stay, the edge / face / cell nodes of the
+    P2 tetrahedra and P2 x P2 prisms follow a smooth periodic displacement field of amplitude `curve` * length."""
     h = length / n
     dims, per = (n, n, n), (True, True, True)
     cells = _cells(n, n, n)
@@ -231,16 +326,26 @@ def box_mixed(n, length=1.0, numbering="natural", seed=0):
     xp, vp = _prisms(cells[low], coord, dims, per)
     m = dict(etypes=["tet", "pri"], xv={"tet": xt, "pri": xp}, vid={"tet": vt, "pri": vp},
              period=[length] * 3, bc_tag=None, n=n)
+    if curve > 0:
+        # a fixed smooth map of amplitude A = curve * length: an edge node leaves its chord by ~ (h^2 / 8) |d''| = A pi^2 / (2 n^2),
+        # i.e. by (curve pi^2 / (2 n)) h -- the relative curvature vanishes under refinement, as for any smooth geometry
+        fn = _sine_bump(length, curve * length)
+        m["xq"] = {"tet": curve_nodes("tet", xt, xt, fn), "pri": curve_nodes("pri", xp, xp, fn)}
     return _renumber(m, numbering, seed)
 
 
-def cylinder_omesh(ntheta=100, nz=15, nlayers=40, nr=40, ratio=1.1, h0=1e-3, jitter=0.15, numbering="natural", seed=0):
+def cylinder_omesh(ntheta=100, nz=15, nlayers=40, nr=40, ratio=1.1, h0=1e-3, jitter=0.15, numbering="natural", seed=0,
+                   quadratic=False):
     """Configs 3/5 (BASELINE.json configs[2], [4]): cylinder-like O-mesh, SURVEY D.3 / DESIGN.md reading R19.
 
     Unit-diameter cylinder at the origin, domain [-9,25]x[-9,9]x[0,pi] (PAPER.md:94), span-periodic;
     `nlayers` geometrically stretched prism layers on the wall, then `nr` layers of Kuhn-split tets
     out to the rectangle, seeded vertex jitter in the tet region.  2*ntheta*nz*nlayers prisms,
     6*ntheta*nz*nr tets.  bc tags: 0 = wall (no-slip isothermal), 1 = far field.
+    quadratic=True (the paper's cylinder meshes are quadratically curved): same vertices,
+    the edge / face nodes of the prisms follow the polar map of the lattice (`curve_nodes`), so the wall is a
+    piecewise-quadratic approximation of the circle instead of a polygon; the curvature is blended out linearly across the
+    first tetrahedral layer and the far field stays straight-sided.
     """
     rng = np.random.Generator(np.random.PCG64(seed))
     rw = 0.5
@@ -280,18 +385,27 @@ def cylinder_omesh(ntheta=100, nz=15, nlayers=40, nr=40, ratio=1.1, h0=1e-3, jit
             return x
         return coord
 
+    def smooth(lat):
+        """The unjittered map for real-valued lattice positions (the wall layers' radii in closed form)."""
+        i, J, k = lat[..., 0], lat[..., 1], lat[..., 2]
+        th = 2 * np.pi * i / ntheta
+        jj = np.clip(J - nlayers, 0, nr)
+        r_t = rtop + (rho_out(th) - rtop) * (ratio ** jj - 1) / (ratio ** nr - 1)
+        r = np.where(J <= nlayers, rw + h0 * (ratio ** np.minimum(J, nlayers) - 1) / (ratio - 1), r_t)
+        return np.stack([r * np.cos(th), r * np.sin(th), span * k / nz], axis=-1)
+
     cells_p = _cells(ntheta, nlayers, nz)
     cells_t = _cells(ntheta, nr, nz)
     cells_t[:, 1] += nlayers
     amp = jitter
     coord0 = make_coord(0.0)
-    xp, vp = _prisms(cells_p, coord0, dims, per, tri_axes=(0, 2), ext_axis=1)
+    xp, vp, lp = _prisms(cells_p, coord0, dims, per, tri_axes=(0, 2), ext_axis=1, want_lat=True)
     _, dN = shape("tet", np.zeros((1, 3)))
     x0, _v = _kuhn_tets(cells_t, coord0, dims, per)
     det0 = np.linalg.det(np.einsum("va,evi->eia", dN[0], x0))
     for _ in range(12):
         # orientation is fixed from the unjittered lattice; halve the jitter until no tet degenerates
-        xt, vt = _kuhn_tets(cells_t, make_coord(amp), dims, per, orient_fn=coord0)
+        xt, vt, lt = _kuhn_tets(cells_t, make_coord(amp), dims, per, orient_fn=coord0, want_lat=True)
         det = np.linalg.det(np.einsum("va,evi->eia", dN[0], xt))
         if np.all(det > 0.05 * det0):
             break
@@ -304,6 +418,9 @@ def cylinder_omesh(ntheta=100, nz=15, nlayers=40, nr=40, ratio=1.1, h0=1e-3, jit
 
     m = dict(etypes=["tet", "pri"], xv={"tet": xt, "pri": xp}, vid={"tet": vt, "pri": vp},
              period=[None, None, span], bc_tag=bc_tag, jitter_amp=amp)
+    if quadratic:
+        blend = lambda lat: np.clip(nlayers + 1.0 - lat[..., 1], 0.0, 1.0)
+        m["xq"] = {"tet": curve_nodes("tet", xt, lt, smooth, blend), "pri": curve_nodes("pri", xp, lp, smooth, blend)}
     return _renumber(m, numbering, seed)
 
 

@@ -272,6 +272,41 @@ def test_row_split_parity(nsplit, monkeypatch):
     ctx.close()
 
 
+# ---------------------------------------------------------------------------- quadratically curved elements
+@pytest.mark.parametrize("mode", ["unfused", "fused"])
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+@pytest.mark.parametrize("p", [2, 3, 4])
+def test_curved_mixed_rhs(p, prec, mode):
+    """Config-2 mesh with P2 tetrahedra and P2 x P2 prisms following a smooth map: every element type carries per-point metric
+    terms (the tetrahedra too), randomly numbered."""
+    case = cases.config2(6, p, "ns", numbering="random", curve=0.08)
+    assert not case["eles"][0]["affine"] and not case["eles"][1]["affine"]
+    _check_rhs(case, prec, mode)
+
+
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+def test_curved_cylinder_rhs(prec):
+    """Small cylinder O-mesh with a piecewise-quadratic wall (curved prism layers, curved first tetrahedral layer), wall and
+    far-field boundaries."""
+    case = cases.config3(p=3, ntheta=16, nz=3, nlayers=3, nr=4, numbering="random", quadratic=True)
+    assert not case["eles"][0]["affine"]
+    _check_rhs(case, prec, "fused")
+
+
+def test_curved_rk45_step():
+    from oracle import fr_oracle as O
+    case = cases.config2(4, 3, "ns", numbering="random", curve=0.08)
+    f = lambda us: O.rhs(case["cfg"], case["eles"], case["ifc"], case["bcs"], us)
+    ref = O.rk45_step(f, case["u0"], 1e-4)
+    ctx = _ctx(case, "f64", stepper="rk45")
+    ctx.set_state(case["u0"])
+    ctx.rk_step(1e-4)
+    got = ctx.get_state()
+    err, _ = field_errors([a - b for a, b in zip(got, case["u0"])], [a - b for a, b in zip(ref, case["u0"])])
+    assert np.all(err <= 1e-9), err
+    ctx.close()
+
+
 # ---------------------------------------------------------------------------- hexahedra (SURVEY 8(f) NEXT-2)
 @pytest.mark.parametrize("mode", ["unfused", "fused"])
 @pytest.mark.parametrize("prec", ["f64", "f32"])

@@ -6,7 +6,7 @@ from fr_inputs import cases, mesh as M, refelem as R
 
 
 def _geo(m, p):
-    return {t: M.geometry(t, p, m["xv"][t]) for t in m["etypes"]}
+    return {t: M.geometry(t, p, m["xq"][t] if "xq" in m else m["xv"][t]) for t in m["etypes"]}
 
 
 MESHES = {
@@ -15,6 +15,8 @@ MESHES = {
     "mixed4_random": lambda: M.box_mixed(4, numbering="random", seed=3),
     "cyl": lambda: M.cylinder_omesh(ntheta=16, nz=4, nlayers=5, nr=5, seed=11),
     "hex3_warped": lambda: M.box_hex(3, numbering="random", seed=5, warp=0.12),
+    "mixed4_curved": lambda: M.box_mixed(4, numbering="random", seed=3, curve=0.08),
+    "cyl_curved": lambda: M.cylinder_omesh(ntheta=16, nz=4, nlayers=5, nr=5, seed=11, quadratic=True),
 }
 
 
@@ -60,7 +62,7 @@ def test_pairs_cover_every_flux_point_once_and_coincide(name, p):
     assert np.all(np.diff(key) > 0)
 
 
-@pytest.mark.parametrize("name", ["tets4", "mixed4"])
+@pytest.mark.parametrize("name", ["tets4", "mixed4", "mixed4_curved"])
 def test_vertex_pairing_equals_coordinate_pairing(name):
     m = MESHES[name]()
     geo = _geo(m, 2)
@@ -123,3 +125,54 @@ def test_cylinder_bc_lists():
     assert np.all(np.einsum("in,ni->n", bf[0]["n"][:2], xw[:, :2]) < 0)
     xo = geo["tet"]["xf"][bf[1]["fpt"], bf[1]["ele"]]
     assert np.all(np.einsum("in,ni->n", bf[1]["n"][:2], xo[:, :2]) > 0)
+
+
+# ---------------------------------------------------------------------------- quadratic geometry
+@pytest.mark.parametrize("etype", ["tet", "pri", "hex"])
+def test_quadratic_shape_functions(etype):
+    """Nodal on `quad_nodes` (vertices first), partition of unity, exact on the element's quadratic space, and equal to the linear
+    shape functions' map when the nodes sit on a straight element."""
+    q = M.quad_nodes(etype)
+    nv = len(R._VERTS[etype])
+    assert q.shape == ({"tet": 10, "pri": 18, "hex": 27}[etype], 3)
+    assert np.array_equal(q[:nv], np.array(R._VERTS[etype], dtype=float))
+    N, dN = M.shape2(etype, q)
+    assert np.abs(N - np.eye(len(q))).max() < 1e-13
+    rng = np.random.Generator(np.random.PCG64(5))
+    x = rng.uniform(-0.9, -0.1, (7, 3))
+    N, dN = M.shape2(etype, x)
+    assert np.abs(N.sum(1) - 1).max() < 1e-13 and np.abs(dN.sum(1)).max() < 1e-12
+    f = lambda y: 0.3 + y[:, 0] - 2 * y[:, 2] + y[:, 0] * y[:, 1] - 0.5 * y[:, 2] ** 2 + 0.25 * y[:, 1] * y[:, 2]
+    df = lambda y: np.stack([1 + y[:, 1], y[:, 0] + 0.25 * y[:, 2], -2 - y[:, 2] + 0.25 * y[:, 1]], axis=1)
+    assert np.abs(N @ f(q) - f(x)).max() < 1e-13
+    assert np.abs(np.einsum("pqa,q->pa", dN, f(q)) - df(x)).max() < 1e-12
+    # straight element: quadratic nodes at the linear map of the reference nodes reproduce the linear geometry
+    xv = rng.uniform(-1, 1, (1, nv, 3)) * 0.2 + np.array(R._VERTS[etype], dtype=float)[None]
+    Nl, dNl = M.shape(etype, q)
+    xq = np.einsum("qv,evi->eqi", Nl, xv)
+    Nlx, dNlx = M.shape(etype, x)
+    assert np.abs(np.einsum("pq,eqi->epi", N, xq) - np.einsum("pv,evi->epi", Nlx, xv)).max() < 1e-13
+    assert np.abs(np.einsum("pqa,eqi->epia", dN, xq) - np.einsum("pva,evi->epia", dNlx, xv)).max() < 1e-12
+
+
+def test_curved_cylinder_converges_to_the_circle_at_fourth_order():
+    """The straight-sided O-mesh approximates the wall by a polygon (volume / area errors O(h^2)); with quadratic elements the
+    prism layer's volume and the wall's area converge at fourth order to pi (r_top^2 - r_w^2) * span and 2 pi r_w * span."""
+    nl = 3
+    rtop = 0.5 + 1e-3 * (1.1 ** nl - 1) / 0.1
+    vol_exact, area_exact = np.pi * (rtop ** 2 - 0.25) * np.pi, 2 * np.pi * 0.5 * np.pi
+    err = {}
+    for quad in (False, True):
+        for nth in (12, 24):
+            c = cases.config3(p=3, ntheta=nth, nz=3, nlayers=nl, nr=3, numbering="random", quadratic=quad)
+            e = [e for e in c["eles"] if e["etype"] == "pri"][0]
+            assert e["affine"] is False and c["eles"][0]["affine"] is (not quad)
+            vol = (e["wts"][:, None] * e["djac"]).sum()
+            wall = [b for b in c["bcs"] if b["type"] == "wall"][0]
+            area = sum((c["eles"][t]["fwts"][wall["fpt"][wall["et"] == t]] * wall["mag"][wall["et"] == t]).sum()
+                       for t in range(len(c["eles"])))
+            err[quad, nth] = (abs(vol / vol_exact - 1), abs(area / area_exact - 1))
+    for k in (0, 1):
+        assert 3.5 < err[False, 12][k] / err[False, 24][k] < 4.5          # second order
+        assert 13.0 < err[True, 12][k] / err[True, 24][k] < 19.0          # fourth order
+        assert err[True, 24][k] < 2e-5 and err[False, 24][k] > 2e-3
