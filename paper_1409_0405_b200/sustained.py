@@ -5,9 +5,12 @@ conserved quantities and the kinetic energy (quadrature-weighted, accumulated in
 point-wise work, stand-alone point-wise kernels, interface kernels).
 
   python -m paper_1409_0405_b200.sustained [--scale 2] [--p 3] [--prec f32] [--steps 1000] [--dt 4e-6] [--json out.json]
+                                           [--mesh cylinder|cylinder-quadratic|hex] [--n 40]
 
 `--scale s` multiplies the circumferential and spanwise cell counts of config 3 (100 x 15) by s: elements = 480 000 s^2.  Config 5
 itself is s = 6 (17.3 M elements, ~150 GB); the mesh generator is host-side numpy and its memory, not the library, bounds s.
+`--mesh cylinder-quadratic`: the same mesh with quadratically curved wall elements (every type then carries
+per-point metric terms); `--mesh hex`: periodic box of n^3 warped, randomly numbered hexahedra (NEXT-2), isentropic vortex.
 """
 import argparse
 import json
@@ -39,11 +42,17 @@ def main():
     ap.add_argument("--steps", type=int, default=1000)
     ap.add_argument("--dt", type=float, default=4e-6)
     ap.add_argument("--json", default=None)
+    ap.add_argument("--mesh", default="cylinder", choices=["cylinder", "cylinder-quadratic", "hex"])
+    ap.add_argument("--n", type=int, default=40, help="cells per direction of the hexahedral box")
     args = ap.parse_args()
     if not torch.cuda.is_available():
         raise SystemExit("sustained needs a CUDA device (no CPU fallback)")
     t0 = time.time()
-    case = cases.config3(p=args.p, ntheta=100 * args.scale, nz=15 * args.scale, seed=cases.SEEDS["c5"])
+    if args.mesh == "hex":
+        case = cases.config_hex(args.n, args.p, "ns", numbering="random", warp=0.1)
+    else:
+        case = cases.config3(p=args.p, ntheta=100 * args.scale, nz=15 * args.scale, seed=cases.SEEDS["c5"],
+                             quadratic=args.mesh == "cylinder-quadratic")
     ndof = cases.ndof(case)
     ne = {e["etype"]: e["neles"] for e in case["eles"]}
     print("mesh: %s elements, %d DOF, generated in %.0f s" % (ne, ndof, time.time() - t0), flush=True)
@@ -51,8 +60,10 @@ def main():
     ctx = Context(case, prec=args.prec, stepper="rk45", stream=stream.cuda_stream)
     ctx.set_state(case["u0"])
     marks = sorted(set(m for m in (0, 10, 100, 1000, args.steps) if m <= args.steps))
-    out = dict(workload="config3 generator x%d: %d pri + %d tet, p=%d, NS, RK45[2R+], %s" % (
-        args.scale, ne.get("pri", 0), ne.get("tet", 0), args.p, args.prec), dof=ndof, dt=args.dt, checkpoints=[])
+    what = ("hex box %d^3 warped: %d hex" % (args.n, ne.get("hex", 0)) if args.mesh == "hex" else
+            "config3 generator x%d%s: %d pri + %d tet" % (args.scale, " quadratic" if args.mesh != "cylinder" else "",
+                                                          ne.get("pri", 0), ne.get("tet", 0)))
+    out = dict(workload="%s, p=%d, NS, RK45[2R+], %s" % (what, args.p, args.prec), dof=ndof, dt=args.dt, checkpoints=[])
     done, gpu_s = 0, 0.0
     for m in marks:
         if m > done:
