@@ -274,3 +274,73 @@ def rk45_step(f, us, dt):
         if i < 4:
             Y = [x + dt * (RK45_A[i] - RK45_B[i]) * k for x, k in zip(X, K)]
     return X
+
+
+# Embedded third-order weights of RK4(3)5[2R+]C (PAPER.md:116 names the pair, not printed in the paper:
+# reading R12); pinned by the exact order-3 conditions in tests/test_rk.py.
+RK45_BHAT_FRAC = ((1016888040809, 7410784769900), (11231460423587, 58533540763752), (-1563879915014, 6823010717585),
+                  (606302364029, 971179775848), (1097981568119, 3980877426909))
+RK45_BHAT = tuple(n / d for n, d in RK45_BHAT_FRAC)
+
+
+def rk45_step_with_error(f, us, dt):
+    """One RK45[2R+] step and the embedded error estimate, from the definition: with the five stage derivatives K_i,
+    u+ = u + dt sum b_i K_i,  E = dt sum (b_i - bhat_i) K_i  (difference between the fourth- and the third-order solution)."""
+    X = [u.copy() for u in us]
+    Y = [u.copy() for u in us]
+    Ks = []
+    for i in range(5):
+        K = f(Y)
+        Ks.append(K)
+        X = [x + dt * RK45_B[i] * k for x, k in zip(X, K)]
+        if i < 4:
+            Y = [x + dt * (RK45_A[i] - RK45_B[i]) * k for x, k in zip(X, K)]
+    E = [np.zeros_like(u) for u in us]
+    for i in range(5):
+        E = [e + dt * (RK45_B[i] - RK45_BHAT[i]) * k for e, k in zip(E, Ks[i])]
+    return X, E
+
+
+def error_norm(E, u_old, u_new, atol, rtol):
+    """Reading R25: err = sqrt( mean over every solution point and variable of (E / (atol + rtol max(|u_n|, |u_n+1|)))^2 )."""
+    s, n = 0.0, 0
+    for e, a, b in zip(E, u_old, u_new):
+        s += float(np.sum((np.abs(e) / (atol + rtol * np.maximum(np.abs(a), np.abs(b)))) ** 2))
+        n += e.size
+    return float(np.sqrt(s / n))
+
+
+PI_ALPHA, PI_BETA, PI_SAFETY, PI_FMIN, PI_FMAX = 0.7 / 4, 0.4 / 4, 0.8, 0.3, 2.5
+
+
+def pi_factor(err, err_prev):
+    """Step-size factor of the PI controller (reading R25; Gustafsson's controller as in Hairer & Wanner II, IV.2, for a
+    local error of order 4): clip(safety * err^-alpha * err_prev^beta, fmin, fmax); a non-finite error gives fmin."""
+    if not np.isfinite(err):
+        return PI_FMIN
+    err = max(err, 1e-10)
+    return float(min(PI_FMAX, max(PI_FMIN, PI_SAFETY * err ** (-PI_ALPHA) * err_prev ** PI_BETA)))
+
+
+def rk45_adaptive(f, us, t0, t1, dt0, atol, rtol, max_attempts=10000):
+    """Adaptive RK45[2R+] from t0 to t1 (reading R25).  Each attempt uses dt = min(dt, t1 - t); it is
+    accepted iff err <= 1 (then t += dt, and t = t1 exactly when the step was cut to reach it); after every attempt
+    dt <- dt * pi_factor(err, err_prev), err_prev being the error of the last accepted step (1 initially).
+    Returns (state, history) with history = list of (dt tried, err, accepted)."""
+    t, dt, err_prev = t0, dt0, 1.0
+    hist = []
+    us = [u.copy() for u in us]
+    while t1 - t > 1e-12 * abs(t1 - t0) and len(hist) < max_attempts:
+        last = dt >= t1 - t
+        dtt = (t1 - t) if last else dt
+        new, E = rk45_step_with_error(f, us, dtt)
+        err = error_norm(E, us, new, atol, rtol)
+        ok = bool(np.isfinite(err) and err <= 1.0)
+        hist.append((dtt, err, ok))
+        if ok:
+            us = new
+            t = t1 if last else t + dtt
+        dt = dtt * pi_factor(err, err_prev)
+        if ok:
+            err_prev = max(err, 1e-10)
+    return us, hist
