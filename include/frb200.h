@@ -128,6 +128,25 @@ fr_status fr_get_state(fr_ctx *ctx, double *const *u_host);
 fr_status fr_rk_step(fr_ctx *ctx, double dt);
 fr_status fr_rk_run(fr_ctx *ctx, double dt, int64_t nsteps);
 
+/* Adaptive RK45[2R+] (the embedded pair P:116 names, reading R12 for b-hat, R25 for the norm and the
+ * controller): advance the internal state from t0 to t1 with step-size control.  FR_RK45_2R contexts only.
+ * Every attempt uses dt = min(dt, t1 - t) and evaluates
+ *   E = dt sum_i (b_i - bhat_i) K_i,   err = sqrt( mean over solution points and variables of (E / (atol + rtol max(|u_n|, |u_n+1|)))^2 );
+ * it is accepted iff err <= 1 (otherwise the state is restored); after every attempt
+ *   dt <- dt * clip(0.8 err^(-0.7/4) err_prev^(0.4/4), 0.3, 2.5),  err_prev = error of the last accepted step (1 initially),
+ * a non-finite err counting as a rejection with factor 0.3.  The five stages, the error accumulation (three extra registers: E,
+ * u_n, and the stage register kept after the last stage) and a deterministic two-pass reduction of the norm run as one CUDA
+ * graph per attempt; the accept / reject decision and the controller run on the host in FP64 after reading back one scalar.
+ * stats (HOST, may be NULL): accepted, rejected, t reached (== t1 unless max_attempts ran out: FR_ESTATE then), dt proposed for
+ * the next step.  dt_hist / err_hist (HOST, may be NULL, capacity hist_cap): dt tried and err of every attempt, in order.
+ * Synchronous. */
+typedef struct {
+  int64_t accepted, rejected;
+  double t, dt_next;
+} fr_adapt_stats;
+fr_status fr_rk_adaptive_run(fr_ctx *ctx, double t0, double t1, double dt_init, double atol, double rtol, int64_t max_attempts,
+                             fr_adapt_stats *stats, double *dt_hist, double *err_hist, int64_t hist_cap);
+
 /* Waits for the stream; returns FR_ECUDA if any asynchronous error occurred. */
 fr_status fr_sync(fr_ctx *ctx);
 

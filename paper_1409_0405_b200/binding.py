@@ -51,7 +51,12 @@ class fr_kernel_stat(C.Structure):
                 ("category", C.c_int32)]
 
 
+class fr_adapt_stats(C.Structure):
+    _fields_ = [("accepted", C.c_int64), ("rejected", C.c_int64), ("t", C.c_double), ("dt_next", C.c_double)]
+
+
 SYMBOLS = ["fr_profile_kernels", "fr_rk_step_host", "fr_setup", "fr_state_layout", "fr_rhs", "fr_set_state", "fr_get_state", "fr_rk_step", "fr_rk_run",
+           "fr_rk_adaptive_run",
            "fr_sync", "fr_launch_count", "fr_profile_rhs", "fr_last_error", "fr_global_error", "fr_destroy",
            "fr_gemm", "fr_gemm_plan_create", "fr_gemm_plan_run", "fr_gemm_plan_destroy", "fr_probe_peaks"]
 
@@ -75,6 +80,8 @@ def load():
     lib.fr_get_state.argtypes = [vp, C.POINTER(_dp)]
     lib.fr_rk_step.argtypes = [vp, C.c_double]
     lib.fr_rk_run.argtypes = [vp, C.c_double, C.c_int64]
+    lib.fr_rk_adaptive_run.argtypes = [vp, C.c_double, C.c_double, C.c_double, C.c_double, C.c_double, C.c_int64,
+                                       C.POINTER(fr_adapt_stats), _dp, _dp, C.c_int64]
     lib.fr_sync.argtypes = [vp]
     lib.fr_launch_count.argtypes = [vp]
     lib.fr_launch_count.restype = C.c_int64
@@ -217,6 +224,18 @@ class Context:
 
     def rk_run(self, dt, nsteps):
         self._check(self._lib.fr_rk_run(self._h, float(dt), int(nsteps)))
+
+    def rk_adaptive_run(self, t0, t1, dt_init, atol, rtol, max_attempts=10000):
+        """fr_rk_adaptive_run: returns (stats dict, history list of (dt tried, err, accepted))."""
+        st = fr_adapt_stats()
+        cap = int(max_attempts)
+        dts, errs = (C.c_double * cap)(), (C.c_double * cap)()
+        rc = self._lib.fr_rk_adaptive_run(self._h, float(t0), float(t1), float(dt_init), float(atol), float(rtol), cap,
+                                          C.byref(st), dts, errs, cap)
+        n = int(st.accepted + st.rejected)
+        hist = [(dts[i], errs[i], bool(errs[i] <= 1.0)) for i in range(n)]
+        self._check(rc)
+        return dict(accepted=int(st.accepted), rejected=int(st.rejected), t=float(st.t), dt_next=float(st.dt_next)), hist
 
     def sync(self):
         self._check(self._lib.fr_sync(self._h))

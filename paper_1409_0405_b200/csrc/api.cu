@@ -25,6 +25,8 @@ struct CtxBase {
   virtual void sync() = 0;
   virtual void profile(int reps, double ms[4], fr_kernel_stat *out, int cap, int *n) = 0;
   virtual void rk_step_host(double dt, void *const *u_host) = 0;
+  virtual void rk_adaptive(double t0, double t1, double dt0, double atol, double rtol, long long max_attempts, fr_adapt_stats *st,
+                           double *dt_hist, double *err_hist, long long hist_cap) = 0;
 };
 
 template <typename T>
@@ -124,6 +126,7 @@ struct EleData {
   // after the other, for operators with more rows than one CTA's accumulators hold (e.g. hexahedra at p = 4)
   std::vector<FusedPart<T>> pDiv, pGrad;
   DevBuf<T> X, Y, ACC;   // solution register, stage input, RK4 accumulator
+  DevBuf<T> E, U0;       // adaptive RK45: error register, state at the start of the attempt (allocated on first use)
   DevBuf<T> grad;        // [3][nupts][5][ld]: G~ -> G (-> F~ on the unfused path)
   DevBuf<T> ftil;        // [3][nupts][5][ld]: F~ written by the fused gradient kernel (NS, fused mode)
   DevBuf<T> R;           // [nupts][5][ld]
@@ -168,10 +171,17 @@ struct Ctx : CtxBase {
   int jump = 0;                     // S2 stores C - U_f and the fused gradient operator is [M4 | M6] (all types fused)
   cudaGraphExec_t graph = nullptr;
   int graph_kernels = 0;
+  cudaGraphExec_t graph_adapt = nullptr;   // one attempt of the adaptive stepper: save, 5 stages + error register, norm
+  int graph_adapt_kernels = 0;
+  DevBuf<double> err_partial, err_dev;      // [nt * rk_err_blocks()], [1 + 2]: sum of squares, then {atol, rtol}
+  double *err_host = nullptr;               // pinned: [0] sum of squares read back, [1..2] staging of {atol, rtol}
+  double tol_set[2] = {-1.0, -1.0};
 
   ~Ctx() override {
     if (graph) cudaGraphExecDestroy(graph);
+    if (graph_adapt) cudaGraphExecDestroy(graph_adapt);
     if (coef_host) cudaFreeHost(coef_host);
+    if (err_host) cudaFreeHost(err_host);
     if (own_stream && stream) cudaStreamDestroy(stream);
   }
 
@@ -636,16 +646,21 @@ struct Ctx : CtxBase {
       coef_host[0] = StageCoef{dt, 0.0};              // forward Euler: X <- X + dt K
     } else {
       // RK4(3)5[2R+]C (reading R12): X += dt b_i K ; Y = X_old + dt a_i K
-      static const double a[5] = {970286171893.0 / 4311952581923.0, 6584761158862.0 / 12103376702013.0,
-                                  2251764453980.0 / 15575788980749.0, 26877169314380.0 / 34165994151039.0, 0.0};
-      static const double b[5] = {1153189308089.0 / 22510343858157.0, 1772645290293.0 / 4653164025191.0,
-                                  -1672844663538.0 / 4480602732383.0, 2114624349019.0 / 3568978502595.0,
-                                  5198255086312.0 / 14908931495163.0};
-      for (int i = 0; i < 5; ++i) coef_host[i] = StageCoef{dt * b[i], dt * a[i]};
+      for (int i = 0; i < 5; ++i) coef_host[i] = StageCoef{dt * kB45[i], dt * kA45[i]};
     }
   }
 
-  int enqueue_step() {
+  // RK4(3)5[2R+]C (reading R12)
+  static constexpr double kA45[5] = {970286171893.0 / 4311952581923.0, 6584761158862.0 / 12103376702013.0,
+                                     2251764453980.0 / 15575788980749.0, 26877169314380.0 / 34165994151039.0, 0.0};
+  static constexpr double kB45[5] = {1153189308089.0 / 22510343858157.0, 1772645290293.0 / 4653164025191.0,
+                                     -1672844663538.0 / 4480602732383.0, 2114624349019.0 / 3568978502595.0,
+                                     5198255086312.0 / 14908931495163.0};
+  static constexpr double kBhat45[5] = {1016888040809.0 / 7410784769900.0, 11231460423587.0 / 58533540763752.0,
+                                        -1563879915014.0 / 6823010717585.0, 606302364029.0 / 971179775848.0,
+                                        1097981568119.0 / 3980877426909.0};
+
+  int enqueue_step(bool adaptive = false) {
     int nk = 0;
     const int S = nstages();
     std::vector<const T *> up(nt);
@@ -662,12 +677,124 @@ struct Ctx : CtxBase {
         } else if (stepper == FR_EULER1) {
           sa[t] = StageArgs<T>{c, e.X.p, nullptr, e.X.p, nullptr};
         } else {
-          sa[t] = StageArgs<T>{c, e.X.p, e.X.p, e.X.p, i < S - 1 ? e.Y.p : nullptr};
+          // adaptive: the last stage writes Y_5 = X_4 + dt a_5 K_5 = X_4 too, for the error estimate
+          sa[t] = StageArgs<T>{c, e.X.p, e.X.p, e.X.p, (i < S - 1 || adaptive) ? e.Y.p : nullptr};
         }
       }
       nk += run_rhs(up.data(), sa.data(), nullptr);
+      if (adaptive) {
+        // dt (b_i - bhat_i) K_i = g_i (Y_i - X_i)  (rk_adapt.cu)
+        const double g = (kB45[i] - kBhat45[i]) / (kA45[i] - kB45[i]);
+        const int nb = rk_err_blocks();
+        for (int t = 0; t < nt; ++t) {
+          EleData<T> &e = *el[t];
+          const long long n = (long long)e.view.nupts * 5 * e.view.ld;
+          if (i < S - 1)
+            nk += launch_rk_err_accum(e.E.p, (const T *)e.Y.p, (const T *)e.X.p, g, i == 0, n, stream);
+          else
+            nk += launch_rk_err_norm((const T *)e.E.p, (const T *)e.Y.p, (const T *)e.X.p, (const T *)e.U0.p, g, err_dev.p + 1, n,
+                                     err_partial.p + (size_t)t * nb, stream);
+        }
+        if (i == S - 1) nk += launch_rk_err_final(err_partial.p, nt * nb, err_dev.p, stream);
+      }
     }
     return nk;
+  }
+
+  void rk_adaptive(double t0, double t1, double dt0, double atol, double rtol, long long max_attempts, fr_adapt_stats *st,
+                   double *dt_hist, double *err_hist, long long hist_cap) override {
+    FR_REQUIRE(stepper == FR_RK45_2R, "adaptive stepping needs an FR_RK45_2R context");
+    FR_REQUIRE(std::isfinite(t0) && std::isfinite(t1) && t1 >= t0, "need finite t0 <= t1");
+    FR_REQUIRE(dt0 > 0 && std::isfinite(dt0), "dt_init must be positive and finite");
+    FR_REQUIRE(atol > 0 && rtol >= 0 && std::isfinite(atol) && std::isfinite(rtol), "need atol > 0 and rtol >= 0");
+    FR_REQUIRE(max_attempts > 0, "max_attempts must be positive");
+    FR_REQUIRE(hist_cap == 0 || (dt_hist && err_hist), "history buffers must be non-NULL when hist_cap > 0");
+    const int nb = rk_err_blocks();
+    if (!err_host) {
+      for (int t = 0; t < nt; ++t) {
+        const size_t n = (size_t)el[t]->view.nupts * 5 * el[t]->view.ld;
+        if (!el[t]->E.p) el[t]->E.alloc(n);
+        if (!el[t]->U0.p) el[t]->U0.alloc(n);
+      }
+      if (!err_partial.p) err_partial.alloc((size_t)nt * nb);
+      if (!err_dev.p) err_dev.alloc(3);
+      FR_CUDA_TRY(cudaMallocHost(&err_host, 3 * sizeof(double)));
+    }
+    FR_CUDA_TRY(cudaStreamSynchronize(stream));
+    if (tol_set[0] != atol || tol_set[1] != rtol) {
+      err_host[1] = atol;
+      err_host[2] = rtol;
+      FR_CUDA_TRY(cudaMemcpyAsync(err_dev.p + 1, err_host + 1, 2 * sizeof(double), cudaMemcpyHostToDevice, stream));
+      tol_set[0] = atol;
+      tol_set[1] = rtol;
+    }
+    if (!graph_adapt) {
+      cudaGraph_t g = nullptr;
+      FR_CUDA_TRY(cudaStreamBeginCapture(stream, cudaStreamCaptureModeThreadLocal));
+      int nk = 0;
+      try {
+        for (int t = 0; t < nt; ++t) {
+          const size_t nbytes = (size_t)el[t]->view.nupts * 5 * el[t]->view.ld * sizeof(T);
+          FR_CUDA_TRY(cudaMemcpyAsync(el[t]->U0.p, el[t]->X.p, nbytes, cudaMemcpyDeviceToDevice, stream));
+        }
+        nk = enqueue_step(true);
+        FR_CUDA_TRY(cudaMemcpyAsync(err_host, err_dev.p, sizeof(double), cudaMemcpyDeviceToHost, stream));
+      } catch (...) {
+        cudaStreamEndCapture(stream, &g);
+        if (g) cudaGraphDestroy(g);
+        throw;
+      }
+      FR_CUDA_TRY(cudaStreamEndCapture(stream, &g));
+      cudaError_t e = cudaGraphInstantiate(&graph_adapt, g, 0);
+      cudaGraphDestroy(g);
+      FR_CUDA_TRY(e);
+      graph_adapt_kernels = nk;
+    }
+    double ndof = 0;
+    for (int t = 0; t < nt; ++t) ndof += (double)el[t]->view.nupts * 5.0 * (double)el[t]->view.neles;
+    // the controller (reading R25), in FP64 on the host
+    const double alpha = 0.7 / 4, beta = 0.4 / 4, safety = 0.8, fmin = 0.3, fmax = 2.5;
+    double t = t0, dt = dt0, err_prev = 1.0;
+    long long nacc = 0, nrej = 0, natt = 0;
+    while (t1 - t > 1e-12 * std::fabs(t1 - t0) && natt < max_attempts) {
+      const bool last = dt >= t1 - t;
+      const double dtt = last ? t1 - t : dt;
+      fill_coefs(dtt);
+      FR_CUDA_TRY(cudaMemcpyAsync(coef.p, coef_host, 8 * sizeof(StageCoef), cudaMemcpyHostToDevice, stream));
+      coef_dt = dtt;
+      FR_CUDA_TRY(cudaGraphLaunch(graph_adapt, stream));
+      launches += graph_adapt_kernels;
+      FR_CUDA_TRY(cudaStreamSynchronize(stream));
+      const double err = std::sqrt(err_host[0] / ndof);
+      const bool ok = std::isfinite(err) && err <= 1.0;
+      if (natt < hist_cap) {
+        dt_hist[natt] = dtt;
+        err_hist[natt] = err;
+      }
+      ++natt;
+      if (ok) {
+        ++nacc;
+        t = last ? t1 : t + dtt;
+      } else {
+        ++nrej;
+        for (int tt_ = 0; tt_ < nt; ++tt_) {
+          const size_t nbytes = (size_t)el[tt_]->view.nupts * 5 * el[tt_]->view.ld * sizeof(T);
+          FR_CUDA_TRY(cudaMemcpyAsync(el[tt_]->X.p, el[tt_]->U0.p, nbytes, cudaMemcpyDeviceToDevice, stream));
+        }
+      }
+      double fac = fmin;
+      if (std::isfinite(err)) fac = std::min(fmax, std::max(fmin, safety * std::pow(std::max(err, 1e-10), -alpha) * std::pow(err_prev, beta)));
+      dt = dtt * fac;
+      if (ok) err_prev = std::max(err, 1e-10);
+    }
+    FR_CUDA_TRY(cudaStreamSynchronize(stream));
+    if (st) {
+      st->accepted = nacc;
+      st->rejected = nrej;
+      st->t = t;
+      st->dt_next = dt;
+    }
+    if (t1 - t > 1e-12 * std::fabs(t1 - t0)) throw Error{FR_ESTATE, "fr_rk_adaptive_run: max_attempts reached before t1"};
   }
 
   void rk_step(double dt, long long nsteps) override {
@@ -846,6 +973,10 @@ fr_status fr_set_state(fr_ctx *ctx, const double *const *u_host) { FR_CTX_CALL(c
 fr_status fr_get_state(fr_ctx *ctx, double *const *u_host) { FR_CTX_CALL(ctx, ctx->impl->get_state(u_host)); }
 fr_status fr_rk_step(fr_ctx *ctx, double dt) { FR_CTX_CALL(ctx, ctx->impl->rk_step(dt, 1)); }
 fr_status fr_rk_run(fr_ctx *ctx, double dt, int64_t nsteps) { FR_CTX_CALL(ctx, ctx->impl->rk_step(dt, nsteps)); }
+fr_status fr_rk_adaptive_run(fr_ctx *ctx, double t0, double t1, double dt_init, double atol, double rtol, int64_t max_attempts,
+                             fr_adapt_stats *stats, double *dt_hist, double *err_hist, int64_t hist_cap) {
+  FR_CTX_CALL(ctx, ctx->impl->rk_adaptive(t0, t1, dt_init, atol, rtol, max_attempts, stats, dt_hist, err_hist, hist_cap));
+}
 fr_status fr_sync(fr_ctx *ctx) { FR_CTX_CALL(ctx, ctx->impl->sync()); }
 fr_status fr_profile_rhs(fr_ctx *ctx, int32_t reps, double ms[4]) {
   FR_CTX_CALL(ctx, {

@@ -58,6 +58,15 @@ template <typename T>
 int launch_bc_comm_flux(const BndView<T> &bv, const TypeTab &tt, T *uf, const T *gf, const PhysParams<T> &ph,
                         cudaStream_t s);
 
+// Embedded error estimate of RK45[2R+] and its norm (rk_adapt.cu)
+int rk_err_blocks();
+template <typename T>
+int launch_rk_err_accum(T *E, const T *Y, const T *X, double g, int first, long long n, cudaStream_t s);
+template <typename T>
+int launch_rk_err_norm(const T *E, const T *Y, const T *X, const T *U0, double g, const double *tol_dev, long long n,
+                       double *partial, cudaStream_t s);
+int launch_rk_err_final(const double *partial, int n, double *out, cudaStream_t s);
+
 // Fused panel kernels (panel_fused.cu).  *_build return false if the operator does not fit the resident design.
 template <typename T>
 bool fused_div_build(PanelOp<T> &op, int nu, int nf, const double *M132, const double *M3, int cand = 0, int r0 = 0, int nr = -1);

@@ -31,6 +31,29 @@ def totals(case, us):
     return tot
 
 
+def adaptive(args, case, ctx, stream, ndof):
+    import torch
+    t1 = args.steps * args.dt
+    ctx.rk_adaptive_run(0.0, 2 * args.dt, args.dt, args.adaptive, args.adaptive)    # warm-up: graph capture, registers
+    ctx.set_state(case["u0"])
+    tot0 = totals(case, ctx.get_state())
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(stream)
+    st, hist = ctx.rk_adaptive_run(0.0, t1, args.dt, args.adaptive, args.adaptive)
+    e1.record(stream)
+    e1.synchronize()
+    sec = e0.elapsed_time(e1) * 1e-3
+    natt = st["accepted"] + st["rejected"]
+    tot1 = totals(case, ctx.get_state())
+    acc = [h[0] for h in hist if h[2]]
+    out = dict(mode="adaptive", tol=args.adaptive, t1=t1, dof=ndof, accepted=st["accepted"], rejected=st["rejected"],
+               dt_min=min(acc), dt_max=max(acc), dt_next=st["dt_next"], ms_per_attempt=1e3 * sec / natt,
+               gdof_rhs_per_s=ndof * 5 * natt / sec / 1e9, mass_drift=(tot1[0] - tot0[0]) / abs(tot0[0]),
+               energy_drift=(tot1[4] - tot0[4]) / abs(tot0[4]))
+    print(json.dumps(out))
+    ctx.close()
+
+
 def main():
     import torch
     from fr_inputs import cases
@@ -44,6 +67,8 @@ def main():
     ap.add_argument("--json", default=None)
     ap.add_argument("--mesh", default="cylinder", choices=["cylinder", "cylinder-quadratic", "hex"])
     ap.add_argument("--n", type=int, default=40, help="cells per direction of the hexahedral box")
+    ap.add_argument("--adaptive", type=float, default=None, metavar="TOL",
+                    help="step-size control (fr_rk_adaptive_run, atol = rtol = TOL) from t = 0 to steps * dt, starting at dt")
     args = ap.parse_args()
     if not torch.cuda.is_available():
         raise SystemExit("sustained needs a CUDA device (no CPU fallback)")
@@ -59,6 +84,8 @@ def main():
     stream = torch.cuda.Stream()
     ctx = Context(case, prec=args.prec, stepper="rk45", stream=stream.cuda_stream)
     ctx.set_state(case["u0"])
+    if args.adaptive is not None:
+        return adaptive(args, case, ctx, stream, ndof)
     marks = sorted(set(m for m in (0, 10, 100, 1000, args.steps) if m <= args.steps))
     what = ("hex box %d^3 warped: %d hex" % (args.n, ne.get("hex", 0)) if args.mesh == "hex" else
             "config3 generator x%d%s: %d pri + %d tet" % (args.scale, " quadratic" if args.mesh != "cylinder" else "",

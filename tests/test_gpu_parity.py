@@ -272,6 +272,68 @@ def test_row_split_parity(nsplit, monkeypatch):
     ctx.close()
 
 
+# ---------------------------------------------------------------------------- adaptive RK45[2R+]
+@pytest.mark.parametrize("mode", ["fused", "unfused"])
+def test_adaptive_rk45_matches_oracle(mode):
+    """fr_rk_adaptive_run against the oracle's controller loop on the mixed mesh: dt0 is far too large, so the run starts with
+    rejections, then settles; the same attempts are taken (accept / reject flags identical -- both sides decide in FP64 on an
+    error norm they agree on to ~1e-9), with the same step sizes and errors, and the final states agree."""
+    from oracle import fr_oracle as O
+    case = cases.config2(4, 2, "ns", numbering="random")
+    f = lambda us: O.rhs(case["cfg"], case["eles"], case["ifc"], case["bcs"], us)
+    t1, dt0, atol, rtol = 5e-3, 1e-2, 1e-8, 1e-8
+    ref, hist = O.rk45_adaptive(f, case["u0"], 0.0, t1, dt0, atol, rtol)
+    # the scenario: three rejections (errors 2e3, 21, 1.07), then a dozen accepted steps limited by stability, the last one cut to t1
+    assert [h[2] for h in hist[:4]] == [False, False, False, True] and sum(h[2] for h in hist) >= 10
+    ctx = _ctx(case, "f64", mode=mode, stepper="rk45")
+    ctx.set_state(case["u0"])
+    st, got_hist = ctx.rk_adaptive_run(0.0, t1, dt0, atol, rtol)
+    assert st["t"] == t1 and st["accepted"] == sum(h[2] for h in hist) and st["rejected"] == sum(not h[2] for h in hist)
+    assert [h[2] for h in got_hist] == [h[2] for h in hist]
+    for (d0, e0, _), (d1, e1, _) in zip(got_hist, hist):
+        assert abs(d0 - d1) <= 1e-8 * d1 and (abs(e0 - e1) <= 1e-6 * e1 or not np.isfinite(e1))
+    got = ctx.get_state()
+    err, _ = field_errors([a - b for a, b in zip(got, case["u0"])], [a - b for a, b in zip(ref, case["u0"])])
+    assert np.all(err <= 1e-8), err
+    # a fixed-step run afterwards still works (the two graphs share the coefficient buffer)
+    ctx.set_state(case["u0"])
+    ctx.rk_step(1e-4)
+    ref1 = O.rk45_step(f, case["u0"], 1e-4)
+    err, _ = field_errors([a - b for a, b in zip(ctx.get_state(), case["u0"])], [a - b for a, b in zip(ref1, case["u0"])])
+    assert np.all(err <= 1e-9), err
+    ctx.close()
+
+
+def test_adaptive_rk45_fp32_and_errors():
+    """FP32: the error register is FP32, the norm is summed in FP64; the run reaches t1 with step sizes close to the FP64
+    oracle's.  Argument checks: wrong stepper, non-positive atol, max_attempts exhausted."""
+    from oracle import fr_oracle as O
+    from paper_1409_0405_b200 import binding
+    case = round_case_to_f32(cases.config2(4, 2, "ns", numbering="random"))
+    f = lambda us: O.rhs(case["cfg"], case["eles"], case["ifc"], case["bcs"], us)
+    t1, dt0, atol, rtol = 5e-3, 8e-3, 1e-5, 1e-5
+    ref, hist = O.rk45_adaptive(f, case["u0"], 0.0, t1, dt0, atol, rtol)
+    assert [(round(h[1], 1), h[2]) for h in hist[:2]] == [(2.2, False), (0.6, True)]      # errors well away from 1
+    ctx = _ctx(case, "f32", stepper="rk45")
+    ctx.set_state(case["u0"])
+    st, got_hist = ctx.rk_adaptive_run(0.0, t1, dt0, atol, rtol)
+    assert st["t"] == t1 and [h[2] for h in got_hist] == [h[2] for h in hist]
+    for (d0, e0, _), (d1, e1, _) in zip(got_hist[:2], hist[:2]):
+        assert abs(e0 - e1) <= 0.05 * e1 and abs(d0 - d1) <= 0.02 * d1
+    got = ctx.get_state()
+    err, _ = field_errors([a - b for a, b in zip(got, case["u0"])], [a - b for a, b in zip(ref, case["u0"])])
+    assert np.all(err <= 2e-3), err
+    with pytest.raises(binding.FrError):
+        ctx.rk_adaptive_run(0.0, t1, dt0, 0.0, rtol)
+    with pytest.raises(binding.FrError):
+        ctx.rk_adaptive_run(0.0, 1.0, 1e-6, atol, rtol, max_attempts=3)
+    ctx.close()
+    ctx4 = _ctx(case, "f32", stepper="rk4")
+    with pytest.raises(binding.FrError):
+        ctx4.rk_adaptive_run(0.0, t1, dt0, atol, rtol)
+    ctx4.close()
+
+
 # ---------------------------------------------------------------------------- quadratically curved elements (SURVEY 8(f) NEXT-1)
 @pytest.mark.parametrize("mode", ["unfused", "fused"])
 @pytest.mark.parametrize("prec", ["f64", "f32"])
