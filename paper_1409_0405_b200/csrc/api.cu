@@ -719,6 +719,8 @@ struct Ctx : CtxBase {
       if (!err_partial.p) err_partial.alloc((size_t)nt * nb);
       if (!err_dev.p) err_dev.alloc(3);
       FR_CUDA_TRY(cudaMallocHost(&err_host, 3 * sizeof(double)));
+      // the allocations zero-fill on the legacy stream, which a non-blocking user stream does not wait for
+      FR_CUDA_TRY(cudaDeviceSynchronize());
     }
     FR_CUDA_TRY(cudaStreamSynchronize(stream));
     if (tol_set[0] != atol || tol_set[1] != rtol) {

@@ -285,7 +285,11 @@ def test_adaptive_rk45_matches_oracle(mode):
     ref, hist = O.rk45_adaptive(f, case["u0"], 0.0, t1, dt0, atol, rtol)
     # the scenario: three rejections (errors 2e3, 21, 1.07), then a dozen accepted steps limited by stability, the last one cut to t1
     assert [h[2] for h in hist[:4]] == [False, False, False, True] and sum(h[2] for h in hist) >= 10
-    ctx = _ctx(case, "f64", mode=mode, stepper="rk45")
+    # on a non-blocking user stream (the first call allocates and zero-fills its registers, which must be ordered with that stream)
+    import torch
+    from paper_1409_0405_b200 import Context
+    stream = torch.cuda.Stream()
+    ctx = Context(case, prec="f64", mode=mode, stepper="rk45", stream=stream.cuda_stream)
     ctx.set_state(case["u0"])
     st, got_hist = ctx.rk_adaptive_run(0.0, t1, dt0, atol, rtol)
     assert st["t"] == t1 and st["accepted"] == sum(h[2] for h in hist) and st["rejected"] == sum(not h[2] for h in hist)
