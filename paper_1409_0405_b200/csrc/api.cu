@@ -346,8 +346,9 @@ struct Ctx : CtxBase {
     const bool verbose = getenv("FRB_PANEL_VERBOSE") != nullptr;
     if (verbose) fprintf(stderr, "autotune %s cand 0: %.3f ms\n", what, bt);
     const bool both = cur.density > 0.25 && cur.density < 0.95;   // intermediate density: also time the other packing
+    const int ncand = getenv("FRB_TUNE_CANDS") ? std::max(1, atoi(getenv("FRB_TUNE_CANDS"))) : kTuneCands;
     for (int pass = 0; pass < (both ? 2 : 1); ++pass)
-      for (int k = pass ? 1000 : 1; k < (pass ? 1000 + kTuneCands / 2 : kTuneCands); ++k) {
+      for (int k = pass ? 1000 : 1; k < (pass ? 1000 + ncand / 2 : ncand); ++k) {
         PanelOp<T> op;
         if (!build(op, k)) break;
         const float t = time_op(op);
