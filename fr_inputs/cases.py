@@ -95,3 +95,67 @@ def config3(p=4, ntheta=100, nz=15, nlayers=40, nr=40, numbering="morton", syste
     case["u0"] = state.perturb(u0, amp, seed, **fs) if amp > 0 else u0
     case["freestream"] = fs
     return case
+
+
+def replicate(case, copies, amp=None, seed=None, compact=False):
+    """`copies` disjoint copies of a case as one case: copy k's elements of a type follow copy k-1's, its flux-point pairs and
+    boundary lists follow copy k-1's with the element numbers shifted.  The copies do not touch; each keeps its own periodic
+    span, wall and far field.  This is how the sustained run (BASELINE.json configs[4]) reaches sizes the host-side mesh
+    generator cannot (ntheta x nz grows with the square of the scale): same element mix, operators, metric terms and
+    connectivity structure per copy.  `amp`/`seed`: copy k > 0 gets its own seeded perturbation of the free stream
+    (`case['freestream']` must be there); otherwise the initial state is tiled.  `compact=True` keeps one point of the
+    metric terms of affine types (what fr_setup reads) and drops the coordinates, for very large cases."""
+    K = int(copies)
+    if K < 1:
+        raise ValueError("copies must be >= 1")
+    ne = [e["neles"] for e in case["eles"]]
+    out = dict(cfg=dict(case["cfg"]), etypes=list(case["etypes"]), order=case["order"], copies=K)
+    if "freestream" in case:
+        out["freestream"] = case["freestream"]
+    eles = []
+    for e in case["eles"]:
+        d = dict(e)
+        d["neles"] = e["neles"] * K
+        cut = slice(0, 1) if (compact and e["affine"]) else slice(None)
+        d["smats"] = np.tile(e["smats"][:, :, cut, :], (1, 1, 1, K))
+        d["rcpdjac"] = np.tile(e["rcpdjac"][cut, :], (1, K))
+        d["djac"] = np.tile(e["djac"][cut, :], (1, K))
+        d["xu"] = None if compact else np.tile(e["xu"], (1, K, 1))
+        eles.append(d)
+    out["eles"] = eles
+    nea = np.asarray(ne, dtype=np.int64)
+
+    def shifted(et, ele):
+        return (ele[None, :] + np.arange(K, dtype=np.int64)[:, None] * nea[et][None, :]).reshape(-1)
+
+    ifc = case["ifc"]
+    o = {}
+    for side in ("l", "r"):
+        o[side + "_et"] = np.tile(ifc[side + "_et"], K)
+        o[side + "_fpt"] = np.tile(ifc[side + "_fpt"], K)
+        o[side + "_ele"] = shifted(ifc[side + "_et"], ifc[side + "_ele"])
+    o["nl"] = np.tile(ifc["nl"], (1, K))
+    o["magl"] = np.tile(ifc["magl"], K)
+    o["magr"] = np.tile(ifc["magr"], K)
+    out["ifc"] = o
+    bcs = []
+    for b in case["bcs"]:
+        d = dict(b)
+        d["et"] = np.tile(b["et"], K)
+        d["fpt"] = np.tile(b["fpt"], K)
+        d["ele"] = shifted(b["et"], b["ele"])
+        d["n"] = np.tile(b["n"], (1, K))
+        d["mag"] = np.tile(b["mag"], K)
+        bcs.append(d)
+    out["bcs"] = bcs
+    if "u0" in case:
+        u0 = [np.tile(u, (1, 1, K)) for u in case["u0"]]
+        if amp is not None and K > 1:
+            fs = case["freestream"]
+            for k in range(1, K):
+                base = [state.freestream(e["xu"], **fs) for e in case["eles"]]
+                pk = state.perturb(base, amp, (SEEDS["c5"] if seed is None else seed) + k, **fs)
+                for u, p_, n in zip(u0, pk, ne):
+                    u[:, :, k * n:(k + 1) * n] = p_
+        out["u0"] = u0
+    return out

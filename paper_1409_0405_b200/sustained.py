@@ -4,11 +4,13 @@ conserved quantities and the kinetic energy (quadrature-weighted, accumulated in
 0 / 10 / 100 / 1000, and the per-kernel-group time breakdown of one right-hand side (`fr_profile_rhs`: operator products incl. fused
 point-wise work, stand-alone point-wise kernels, interface kernels).
 
-  python -m paper_1409_0405_b200.sustained [--scale 2] [--p 3] [--prec f32] [--steps 1000] [--dt 4e-6] [--json out.json]
-                                           [--mesh cylinder|cylinder-quadratic|hex] [--n 40]
+  python -m paper_1409_0405_b200.sustained [--scale 2] [--copies 1] [--p 3] [--prec f32] [--steps 1000] [--dt 4e-6]
+                                           [--json out.json] [--mesh cylinder|cylinder-quadratic|hex] [--n 40]
 
 `--scale s` multiplies the circumferential and spanwise cell counts of config 3 (100 x 15) by s: elements = 480 000 s^2.  Config 5
-itself is s = 6 (17.3 M elements, ~150 GB); the mesh generator is host-side numpy and its memory, not the library, bounds s.
+itself is s = 6 (17.3 M elements, ~150 GB); the mesh generator is host-side numpy and its memory and time, not the library,
+bound s.  `--copies K` reaches that size another way (`fr_inputs.cases.replicate`): K disjoint copies of the scale-s mesh as one
+case, each with its own seeded perturbation -- s = 2, K = 9 has config 5's 4.32 M prisms + 12.96 M tetrahedra.
 `--mesh cylinder-quadratic`: the same mesh with quadratically curved wall elements (every type then carries
 per-point metric terms); `--mesh hex`: periodic box of n^3 warped, randomly numbered hexahedra (NEXT-2), isentropic vortex.
 """
@@ -60,6 +62,7 @@ def main():
     from . import Context
     ap = argparse.ArgumentParser()
     ap.add_argument("--scale", type=int, default=2)
+    ap.add_argument("--copies", type=int, default=1, help="disjoint copies of the mesh held as one case")
     ap.add_argument("--p", type=int, default=3)
     ap.add_argument("--prec", default="f32", choices=["f32", "f64"])
     ap.add_argument("--steps", type=int, default=1000)
@@ -78,19 +81,26 @@ def main():
     else:
         case = cases.config3(p=args.p, ntheta=100 * args.scale, nz=15 * args.scale, seed=cases.SEEDS["c5"],
                              quadratic=args.mesh == "cylinder-quadratic")
+    if args.copies > 1:
+        case = cases.replicate(case, args.copies, amp=0.005, seed=cases.SEEDS["c5"], compact=True)
     ndof = cases.ndof(case)
     ne = {e["etype"]: e["neles"] for e in case["eles"]}
     print("mesh: %s elements, %d DOF, generated in %.0f s" % (ne, ndof, time.time() - t0), flush=True)
     stream = torch.cuda.Stream()
     ctx = Context(case, prec=args.prec, stepper="rk45", stream=stream.cuda_stream)
     ctx.set_state(case["u0"])
+    free_b, total_b = torch.cuda.mem_get_info()
+    hbm_gb = (total_b - free_b) / 1e9
+    print("set-up done at %.0f s, device memory in use %.1f GB of %.1f" % (time.time() - t0, hbm_gb, total_b / 1e9), flush=True)
     if args.adaptive is not None:
         return adaptive(args, case, ctx, stream, ndof)
     marks = sorted(set(m for m in (0, 10, 100, 1000, args.steps) if m <= args.steps))
     what = ("hex box %d^3 warped: %d hex" % (args.n, ne.get("hex", 0)) if args.mesh == "hex" else
-            "config3 generator x%d%s: %d pri + %d tet" % (args.scale, " quadratic" if args.mesh != "cylinder" else "",
-                                                          ne.get("pri", 0), ne.get("tet", 0)))
-    out = dict(workload="%s, p=%d, NS, RK45[2R+], %s" % (what, args.p, args.prec), dof=ndof, dt=args.dt, checkpoints=[])
+            "config3 generator x%d%s%s: %d pri + %d tet" % (args.scale, " quadratic" if args.mesh != "cylinder" else "",
+                                                            ", %d disjoint copies" % args.copies if args.copies > 1 else "",
+                                                            ne.get("pri", 0), ne.get("tet", 0)))
+    out = dict(workload="%s, p=%d, NS, RK45[2R+], %s" % (what, args.p, args.prec), dof=ndof, dt=args.dt, hbm_in_use_gb=hbm_gb,
+               checkpoints=[])
     done, gpu_s = 0, 0.0
     for m in marks:
         if m > done:
