@@ -176,8 +176,16 @@ struct Ctx : CtxBase {
   DevBuf<double> err_partial, err_dev;      // [nt * rk_err_blocks()], [1 + 2]: sum of squares, then {atol, rtol}
   double *err_host = nullptr;               // pinned: [0] sum of squares read back, [1..2] staging of {atol, rtol}
   double tol_set[2] = {-1.0, -1.0};
+  int cmask = 0;                            // phases that run one branch per element type (run_rhs; FRB_CONCURRENT=mask, 0: one stream)
+  std::vector<cudaStream_t> aux;
+  std::vector<cudaEvent_t> ev_type;
+  cudaEvent_t ev_main[3] = {nullptr, nullptr, nullptr};
 
   ~Ctx() override {
+    for (auto q : aux) cudaStreamDestroy(q);
+    for (auto e : ev_type) cudaEventDestroy(e);
+    for (auto e : ev_main)
+      if (e) cudaEventDestroy(e);
     if (graph) cudaGraphExecDestroy(graph);
     if (graph_adapt) cudaGraphExecDestroy(graph_adapt);
     if (coef_host) cudaFreeHost(coef_host);
@@ -192,6 +200,7 @@ struct Ctx : CtxBase {
     stepper = c->stepper;
     mode = c->mode;
     stream = (cudaStream_t)c->cuda_stream;
+    if (getenv("FRB_CONCURRENT")) cmask = atoi(getenv("FRB_CONCURRENT")) & 15;
     if (!stream) {
       // the legacy default stream cannot be captured into a graph: use an own *blocking* stream, which keeps the
       // implicit ordering with work the caller enqueues on the default stream
@@ -512,83 +521,155 @@ struct Ctx : CtxBase {
     double nbnd = 0;
     for (auto &b : bnd) nbnd += (double)b->view.n;
     const double npr = (double)iv.npairs;
-    for (int t = 0; t < nt; ++t) {   // S1: U_f = M0 U
+    auto do_S1 = [&](int t, cudaStream_t q) {   // S1: U_f = M0 U
       EleData<T> &e = *el[t];
       const double n = (double)e.view.neles, nu = e.view.nupts, nf = e.view.nfpts;
-      nk += gemm_run(e.pM0, 5 * e.view.ld, T(1), u[t], 5 * e.view.ld, 0, T(0), uf.p + tt.ubase[t], 5 * e.view.ld, 0, 1, s);
+      nk += gemm_run(e.pM0, 5 * e.view.ld, T(1), u[t], 5 * e.view.ld, 0, T(0), uf.p + tt.ubase[t], 5 * e.view.ld, 0, 1, q);
       mark(CAT_GEMM, t, "S1_M0", (nu + nf) * 5 * n, 2 * (e.pM0.pop ? e.pM0.pop->density : 1.0) * nf * nu * 5 * n);
-    }
-    if (ns) {
+    };
+    auto do_S2 = [&]() {
       nk += launch_con_u(iv, tt, uf.p, cf.p, ph.beta, jump, s);   // S2
       for (auto &b : bnd) nk += launch_bc_con_u(b->view, tt, uf.p, cf.p, ph.gamma, jump, s);
-      {
-        const double words = jump ? (ph.beta == T(0.5) ? 15 : 20) : 20;
-        mark(CAT_IFACE, -1, jump ? "S2_con_u_jump" : "S2_con_u", npr * (words + 16 / w) + nbnd * (10 + 3 + 8 / w), npr * 15 + nbnd * 60);
-      }
-      for (int t = 0; t < nt; ++t) {
-        EleData<T> &e = *el[t];
-        const long long n5 = 5 * e.view.ld;
-        const double n = (double)e.view.neles, nu = e.view.nupts, nf = e.view.nfpts;
-        const double nmet = e.view.affine ? 1 : nu;
-        if (!e.pGrad.empty()) {
-          // S3 + S4 fused: G = (1/|J|) S^T ([M460 | M6] [U; C])
-          // S3 + S4 (+S6) fused: G = (1/|J|) S^T ([M460 | M6] [U; C]);  F~ = S (f_inv(U) - f_visc(U, G))
-          for (auto &q : e.pGrad) nk += launch_fused_grad(q.op, e.view, u[t], cf.p + tt.ubase[t], e.grad.p, e.ftil.p, ph, s);
-          const bool fl = e.ftil.p != nullptr;
-          mark(CAT_GEMM, t, fl ? "S3_S4_S6_fused_grad_flux" : "S3_S4_fused_grad",
-               (5 * nu + 5 * nf + 15 * nu + 10 * nmet + (fl ? 15 * nu : 0)) * n,
-               2 * parts_density(e.pGrad) * 3 * nu * (nu + nf) * 5 * n + 15 * 6 * nu * n + (fl ? 210 * nu * n : 0));
-        } else {
-          // S3: G~ = M460 U + M6 C
-          nk += gemm_run(e.pM460, n5, T(1), u[t], n5, 0, T(0), e.grad.p, n5, 0, 1, s);
-          mark(CAT_GEMM, t, "S3a_M460", (nu + 3 * nu) * 5 * n, 2 * 3 * nu * nu * 5 * n);
-          nk += gemm_run(e.pM6, n5, T(1), cf.p + tt.ubase[t], n5, 0, T(1), e.grad.p, n5, 0, 1, s);
-          mark(CAT_GEMM, t, "S3b_M6", (nf + 6 * nu) * 5 * n, 2 * 3 * nu * nf * 5 * n);
-          nk += launch_gradcoru(e.view, e.grad.p, s);   // S4
-          mark(CAT_PW, t, "S4_gradcoru", (30 * nu + 10 * nmet) * n, 15 * 6 * nu * n);
-        }
-        // S5: G_f,i = M0 G_i, i = 0..2 (batched)
-        nk += gemm_run(e.pM0, n5, T(1), e.grad.p, n5, (long long)e.view.nupts * n5, T(0), gf.p + tt.gbase[t], n5,
-                       tt.gcomp[t], 3, s);
-        mark(CAT_GEMM, t, "S5_M0grad", (nu + nf) * 15 * n, 2 * (e.pM0.pop ? e.pM0.pop->density : 1.0) * nf * nu * 15 * n);
-      }
-    }
-    nk += launch_comm_flux(iv, tt, uf.p, gf.p, ph, s);   // S7 (D overwrites U_f)
-    for (auto &b : bnd) nk += launch_bc_comm_flux(b->view, tt, uf.p, gf.p, ph, s);
-    {
-      const double sides = ns ? ((ph.beta == T(0.5) || ph.beta == T(-0.5)) ? 1 : 2) : 0;
-      mark(CAT_IFACE, -1, "S7_comm_flux", npr * (20 + 15 * sides + 5 + 16 / w) + nbnd * (10 + (ns ? 15 : 0) + 4 + 8 / w),
-           npr * (ns ? 420 : 160) + nbnd * (ns ? 420 : 200));
-    }
-    for (int t = 0; t < nt; ++t) {
+      const double words = jump ? (ph.beta == T(0.5) ? 15 : 20) : 20;
+      mark(CAT_IFACE, -1, jump ? "S2_con_u_jump" : "S2_con_u", npr * (words + 16 / w) + nbnd * (10 + 3 + 8 / w), npr * 15 + nbnd * 60);
+    };
+    auto do_grad = [&](int t, cudaStream_t q) {   // S3, S4, S5
       EleData<T> &e = *el[t];
       const long long n5 = 5 * e.view.ld;
       const double n = (double)e.view.neles, nu = e.view.nupts, nf = e.view.nfpts;
       const double nmet = e.view.affine ? 1 : nu;
-      const T *ft = e.ftil.p;
-      if (!ft) {
-        nk += launch_tdisf(e.view, u[t], e.grad.p, ph, s);   // S6 (Euler, or unfused): F~ in place over G
-        mark(CAT_PW, t, "S6_tdisf", ((ns ? 35 : 20) * nu + 9 * nmet) * n, (ns ? 210 : 110) * nu * n);
-        ft = e.grad.p;
+      if (!e.pGrad.empty()) {
+        // S3 + S4 (+S6) fused: G = (1/|J|) S^T ([M460 | M6] [U; C]);  F~ = S (f_inv(U) - f_visc(U, G))
+        for (auto &g : e.pGrad) nk += launch_fused_grad(g.op, e.view, u[t], cf.p + tt.ubase[t], e.grad.p, e.ftil.p, ph, q);
+        const bool fl = e.ftil.p != nullptr;
+        mark(CAT_GEMM, t, fl ? "S3_S4_S6_fused_grad_flux" : "S3_S4_fused_grad",
+             (5 * nu + 5 * nf + 15 * nu + 10 * nmet + (fl ? 15 * nu : 0)) * n,
+             2 * parts_density(e.pGrad) * 3 * nu * (nu + nf) * 5 * n + 15 * 6 * nu * n + (fl ? 210 * nu * n : 0));
+      } else {
+        // S3: G~ = M460 U + M6 C
+        nk += gemm_run(e.pM460, n5, T(1), u[t], n5, 0, T(0), e.grad.p, n5, 0, 1, q);
+        mark(CAT_GEMM, t, "S3a_M460", (nu + 3 * nu) * 5 * n, 2 * 3 * nu * nu * 5 * n);
+        nk += gemm_run(e.pM6, n5, T(1), cf.p + tt.ubase[t], n5, 0, T(1), e.grad.p, n5, 0, 1, q);
+        mark(CAT_GEMM, t, "S3b_M6", (nf + 6 * nu) * 5 * n, 2 * 3 * nu * nf * 5 * n);
+        nk += launch_gradcoru(e.view, e.grad.p, q);   // S4
+        mark(CAT_PW, t, "S4_gradcoru", (30 * nu + 10 * nmet) * n, 15 * 6 * nu * n);
       }
+      // S5: G_f,i = M0 G_i, i = 0..2 (batched)
+      nk += gemm_run(e.pM0, n5, T(1), e.grad.p, n5, (long long)e.view.nupts * n5, T(0), gf.p + tt.gbase[t], n5,
+                     tt.gcomp[t], 3, q);
+      mark(CAT_GEMM, t, "S5_M0grad", (nu + nf) * 15 * n, 2 * (e.pM0.pop ? e.pM0.pop->density : 1.0) * nf * nu * 15 * n);
+    };
+    auto do_S7 = [&]() {
+      nk += launch_comm_flux(iv, tt, uf.p, gf.p, ph, s);   // S7 (D overwrites U_f)
+      for (auto &b : bnd) nk += launch_bc_comm_flux(b->view, tt, uf.p, gf.p, ph, s);
+      const double sides = ns ? ((ph.beta == T(0.5) || ph.beta == T(-0.5)) ? 1 : 2) : 0;
+      mark(CAT_IFACE, -1, "S7_comm_flux", npr * (20 + 15 * sides + 5 + 16 / w) + nbnd * (10 + (ns ? 15 : 0) + 4 + 8 / w),
+           npr * (ns ? 420 : 160) + nbnd * (ns ? 420 : 200));
+    };
+    auto do_S6 = [&](int t, cudaStream_t q) {
+      EleData<T> &e = *el[t];
+      if (e.ftil.p) return;
+      const double n = (double)e.view.neles, nu = e.view.nupts;
+      const double nmet = e.view.affine ? 1 : nu;
+      nk += launch_tdisf(e.view, u[t], e.grad.p, ph, q);   // S6 (Euler, or unfused): F~ in place over G
+      mark(CAT_PW, t, "S6_tdisf", ((ns ? 35 : 20) * nu + 9 * nmet) * n, (ns ? 210 : 110) * nu * n);
+    };
+    auto do_div = [&](int t, cudaStream_t q) {   // S8, S9, S10
+      EleData<T> &e = *el[t];
+      const long long n5 = 5 * e.view.ld;
+      const double n = (double)e.view.neles, nu = e.view.nupts, nf = e.view.nfpts;
+      const double nmet = e.view.affine ? 1 : nu;
+      const T *ft = e.ftil.p ? e.ftil.p : e.grad.p;
       if (!e.pDiv.empty()) {
         // S8 + S9 (+S10) fused: out = -(1/|J|) [M132 | M3] [F~; D], stage update in the epilogue
-        for (auto &q : e.pDiv) nk += launch_fused_div(q.op, e.view, ft, uf.p + tt.ubase[t], sa[t], s);
+        for (auto &g : e.pDiv) nk += launch_fused_div(g.op, e.view, ft, uf.p + tt.ubase[t], sa[t], q);
         const double rk = sa[t].coef ? (sa[t].out2 ? 15 : 10) : 5;
         mark(CAT_GEMM, t, sa[t].coef ? "S8_S9_S10_fused_div_rk" : "S8_S9_fused_div", (15 * nu + 5 * nf + rk * nu + nmet) * n,
              2 * parts_density(e.pDiv) * nu * (3 * nu + nf) * 5 * n + 5 * nu * n);
-        continue;
+        return;
       }
       // S8: R = M132 F~ + M3 D
-      nk += gemm_run(e.pM132, n5, T(1), e.grad.p, n5, 0, T(0), e.R.p, n5, 0, 1, s);
+      nk += gemm_run(e.pM132, n5, T(1), e.grad.p, n5, 0, T(0), e.R.p, n5, 0, 1, q);
       mark(CAT_GEMM, t, "S8a_M132", (3 * nu + nu) * 5 * n, 2 * nu * 3 * nu * 5 * n);
-      nk += gemm_run(e.pM3, n5, T(1), uf.p + tt.ubase[t], n5, 0, T(1), e.R.p, n5, 0, 1, s);
+      nk += gemm_run(e.pM3, n5, T(1), uf.p + tt.ubase[t], n5, 0, T(1), e.R.p, n5, 0, 1, q);
       mark(CAT_GEMM, t, "S8b_M3", (nf + 2 * nu) * 5 * n, 2 * nu * nf * 5 * n);
-      nk += launch_negdivconf(e.view, e.R.p, sa[t], s);   // S9 / S10
+      nk += launch_negdivconf(e.view, e.R.p, sa[t], q);   // S9 / S10
       const double extra = sa[t].coef ? (sa[t].out2 ? 20 : 10) : 5;
       mark(CAT_PW, t, sa[t].coef ? "S9_S10_negdiv_rk" : "S9_negdivconf", ((5 + extra) * nu + nmet) * n, 5 * nu * n * (sa[t].coef ? 5 : 1));
+    };
+    if (!tl && cmask && nt > 1) {
+      // The element types' chains are independent between the interface kernels (which read and write every type's flux
+      // points): a phase whose bit is set in cmask runs one branch per type (1: S1, 2: S3..S5, 4: S6 beside S7, 8: S8..S10),
+      // the interface kernels stay on the caller's stream.  Under capture the events become the edges of the step's graph.
+      ensure_branches();
+      auto rec = [&](cudaEvent_t e, cudaStream_t q) { FR_CUDA_TRY(cudaEventRecord(e, q)); };
+      auto wait = [&](cudaStream_t q, cudaEvent_t e) { FR_CUDA_TRY(cudaStreamWaitEvent(q, e, 0)); };
+      auto branch = [&](int t, int bit) { return (cmask & bit) ? aux[t] : s; };
+      auto fork_join = [&](int bit, cudaEvent_t start, auto &&body) {
+        if (cmask & bit) rec(start, s);
+        for (int t = 0; t < nt; ++t) {
+          cudaStream_t q = branch(t, bit);
+          if (q != s) wait(q, start);
+          body(t, q);
+          if (q != s) rec(ev_type[t], q);
+        }
+        if (cmask & bit)
+          for (int t = 0; t < nt; ++t) wait(s, ev_type[t]);
+      };
+      fork_join(1, ev_main[0], do_S1);
+      if (ns) {
+        do_S2();
+        fork_join(2, ev_main[1], do_grad);
+      }
+      if (cmask & 4) {                       // S6 needs only this evaluation's S5 to have read G: beside S7
+        rec(ev_main[1], s);
+        for (int t = 0; t < nt; ++t) {
+          wait(aux[t], ev_main[1]);
+          do_S6(t, aux[t]);
+          rec(ev_type[t], aux[t]);
+        }
+      }
+      do_S7();
+      if (!(cmask & 4))
+        for (int t = 0; t < nt; ++t) do_S6(t, s);
+      if (cmask & 8) rec(ev_main[2], s);
+      for (int t = 0; t < nt; ++t) {
+        cudaStream_t q = branch(t, 8);
+        if (q != s) wait(q, ev_main[2]);     // S7 (and S6 where it ran on s); S6 on aux[t] precedes in stream order
+        else if (cmask & 4) wait(s, ev_type[t]);
+        do_div(t, q);
+        if (q != s) rec(ev_type[t], q);
+      }
+      if (cmask & 8)
+        for (int t = 0; t < nt; ++t) wait(s, ev_type[t]);
+      return nk;
+    }
+    for (int t = 0; t < nt; ++t) do_S1(t, s);
+    if (ns) {
+      do_S2();
+      for (int t = 0; t < nt; ++t) do_grad(t, s);
+    }
+    do_S7();
+    for (int t = 0; t < nt; ++t) {
+      do_S6(t, s);
+      do_div(t, s);
     }
     return nk;
+  }
+
+  // per-type branch streams and the events that fork from / join into the caller's stream (run_rhs)
+  void ensure_branches() {
+    if ((int)aux.size() == nt) return;
+    for (int t = (int)aux.size(); t < nt; ++t) {
+      cudaStream_t q;
+      cudaEvent_t e;
+      FR_CUDA_TRY(cudaStreamCreateWithFlags(&q, cudaStreamNonBlocking));
+      aux.push_back(q);
+      FR_CUDA_TRY(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
+      ev_type.push_back(e);
+    }
+    for (int i = 0; i < 3; ++i)
+      if (!ev_main[i]) FR_CUDA_TRY(cudaEventCreateWithFlags(&ev_main[i], cudaEventDisableTiming));
   }
 
   void state_layout(int et, int64_t *ld, int64_t *nbytes) const override {

@@ -272,6 +272,38 @@ def test_row_split_parity(nsplit, monkeypatch):
     ctx.close()
 
 
+# ---------------------------------------------------------------------------- per-type branches of the step's graph
+@pytest.mark.parametrize("system", ["ns", "euler"])
+@pytest.mark.parametrize("mode", ["fused", "unfused"])
+def test_type_branches_bitwise_equal_single_stream(system, mode, monkeypatch):
+    """The element types' kernel chains may run as parallel branches between the interface kernels (api.cu run_rhs;
+    FRB_CONCURRENT = mask of the phases that branch, 0 keeps everything on one stream).  Same kernels, same operands: the
+    right-hand side and three RK45 steps (graph replay) must agree bit for bit for every mask -- a missing edge between the
+    branches shows up as a difference."""
+    case = cases.config2(6, 3, system, numbering="random")
+    res = {}
+    masks = ("0", "15", "5", "10", "4", "8")
+    for conc in masks:
+        monkeypatch.setenv("FRB_CONCURRENT", conc)
+        ctx = _ctx(case, "f64", mode, stepper="rk45")
+        _, raw = gpu_rhs(ctx, case["u0"])
+        for _ in range(3):                                   # eager launches race differently from replays: repeat
+            _, raw2 = gpu_rhs(ctx, case["u0"])
+            assert all(np.array_equal(a, b) for a, b in zip(raw, raw2))
+        ctx.set_state(case["u0"])
+        ctx.rk_run(1e-4, 3)
+        ctx.sync()
+        res[conc] = (raw, ctx.get_state())
+        ctx.close()
+    for m in masks[1:]:
+        for k in (0, 1):
+            for a, b in zip(res[m][k], res["0"][k]):
+                assert np.array_equal(a, b), (m, k)
+    ref = oracle_rhs(case)
+    err, _ = field_errors([r[:, :, :u.shape[2]] for r, u in zip(res["15"][0], case["u0"])], ref)
+    assert np.all(err <= 1e-11), err
+
+
 # ---------------------------------------------------------------------------- adaptive RK45[2R+] (SURVEY 8(f) NEXT-3)
 @pytest.mark.parametrize("mode", ["fused", "unfused"])
 def test_adaptive_rk45_matches_oracle(mode):
