@@ -75,3 +75,51 @@ def test_gpu_replica_matches_oracle(prec, tol):
         num = np.maximum(num, np.abs(g - r).max(axis=(0, 2)))
         den = np.maximum(den, np.abs(r).max(axis=(0, 2)))
     assert (num / den).max() < tol
+
+
+def _totals(case, us):
+    """quadrature-weighted sums of the five conserved variables over all elements (omega_j |J| u), FP64"""
+    tot = np.zeros(5)
+    for e, u in zip(case["eles"], us):
+        w = e["wts"][:, None] * e["djac"]
+        tot += (w[:, None, :] * u).sum(axis=(0, 2))
+    return tot
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+def test_gpu_ten_step_prefix_drift_matches_oracle(prec):
+    """BASELINE.json configs[4]: "energy/conservation drift against the oracle on a 10-step prefix".  The sustained run's
+    recipe (config-3 generator, p = 3, replicated copies with their own perturbations, compact metric terms, RK45[2R+] graph
+    replay with fixed dt) at a size the oracle steps in seconds: the change of the conserved totals over 10 steps and the
+    state itself against the oracle's ten rk45_step calls."""
+    from gpu_util import round_case_to_f32
+    from oracle import fr_oracle as O
+    from paper_1409_0405_b200 import Context
+    case = cases.config3(p=3, ntheta=12, nz=3, nlayers=3, nr=3, numbering="random")
+    rep = cases.replicate(case, 2, amp=0.005, seed=cases.SEEDS["c5"])
+    comp = cases.replicate(case, 2, amp=0.005, seed=cases.SEEDS["c5"], compact=True)
+    c = round_case_to_f32(rep) if prec == "f32" else rep
+    f = lambda us: O.rhs(c["cfg"], c["eles"], c["ifc"], c["bcs"], us)
+    dt, nsteps = 4e-6, 10                         # the sustained run's dt (the wall layers do not allow 2e-5 at p = 3)
+    ref = c["u0"]
+    for _ in range(nsteps):
+        ref = O.rk45_step(f, ref, dt)
+    ctx = Context(comp, prec=prec, stepper="rk45")
+    ctx.set_state(rep["u0"])
+    ctx.rk_run(dt, nsteps)
+    ctx.sync()
+    got = ctx.get_state()
+    ctx.close()
+    assert all(np.isfinite(g).all() for g in got)
+    t0, tr, tg = _totals(rep, c["u0"]), _totals(rep, ref), _totals(rep, got)
+    scale = np.abs(t0).max()
+    drift_ref, drift_got = (tr - t0) / scale, (tg - t0) / scale
+    assert np.abs(drift_ref).max() > 2e-8          # open boundaries: the totals do move, so the comparison is not 0 = 0
+    # FP64: the drift itself agrees to 1e-9 of its size.  FP32: 50 stage updates of an FP32 state round the totals by a few
+    # 2^-24 relative (the sums are taken in FP64 on the host from the FP32 state)
+    tol = 1e-9 * np.abs(drift_ref).max() if prec == "f64" else 5e-7
+    assert np.abs(drift_got - drift_ref).max() <= tol, (drift_got, drift_ref)
+    num = max(np.abs(a - b).max() for a, b in zip(got, ref))
+    den = max(np.abs(b).max() for b in ref)
+    assert num / den <= (1e-11 if prec == "f64" else 2e-6)
