@@ -10,8 +10,7 @@ SOURCES = ["api.cu", "gemm.cu", "panel_gemm.cu", "panel_fused.cu", "pointwise.cu
 HEADERS = ["common.cuh", "kernels.cuh", "physics.cuh", "panel.cuh", "panel_kernel.cuh", os.path.join("..", "..", "include", "frb200.h")]
 NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
               "-Xcompiler", "-fPIC", "--expt-relaxed-constexpr"] + (
-                  ["-DFRB_NSTAGE=" + os.environ["FRB_NSTAGE"]] if os.environ.get("FRB_NSTAGE") else []) + (
-                  ["-DFRB_DENSE_SKIP=" + os.environ["FRB_DENSE_SKIP"]] if os.environ.get("FRB_DENSE_SKIP") else [])
+                  ["-DFRB_NSTAGE=" + os.environ["FRB_NSTAGE"]] if os.environ.get("FRB_NSTAGE") else [])
 
 
 def _nvcc():

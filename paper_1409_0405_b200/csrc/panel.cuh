@@ -17,9 +17,6 @@
 //   * producers (how a B chunk comes to be) and epilogues (what happens to the accumulators) are policies, which is how the
 //     point-wise flux, gradient transform, -1/|J| scaling and Runge-Kutta stage update are fused into the products.
 #pragma once
-#ifndef FRB_DENSE_SKIP
-#define FRB_DENSE_SKIP 0
-#endif
 #include <algorithm>
 #include <cmath>
 #include <cstdlib>
@@ -679,19 +676,6 @@ struct Acc<double, NIT, CX> {
     for (int b = 0; b < nb; ++b) {
       const int row = min(4 * b + kl, last);           // padded rows of the last block: operator is zero, data must be finite
       const char *bp = bcol + (uint32_t)row * rs;
-      const char *ap = av + (uint32_t)b * as;
-#if FRB_DENSE_SKIP
-      // (row group, k-block) tiles that are entirely zero are skipped (warp-uniform vote on the A fragment); a k-block whose
-      // tiles are zero for every row group of the warp is not even loaded.  Adding an exact zero is what is skipped.
-      double aa[NIT];
-      unsigned live = 0;
-#pragma unroll
-      for (int i = 0; i < NIT; ++i) {
-        aa[i] = *reinterpret_cast<const double *>(ap + i * 256);
-        live |= __any_sync(0xffffffffu, aa[i] != 0.0) ? (1u << i) : 0u;
-      }
-      if (!live) continue;
-#endif
       double bf[PV][CX];
 #pragma unroll
       for (int v = 0; v < PV; ++v) {
@@ -699,14 +683,10 @@ struct Acc<double, NIT, CX> {
         for (int cb = 0; cb < CX; ++cb) bf[v][cb] = *reinterpret_cast<const double *>(bp + cb * 64);
         bp += vs;
       }
+      const char *ap = av + (uint32_t)b * as;
 #pragma unroll
       for (int i = 0; i < NIT; ++i) {
-#if FRB_DENSE_SKIP
-        if (!(live & (1u << i))) continue;
-        const double a = aa[i];
-#else
         const double a = *reinterpret_cast<const double *>(ap + i * 256);
-#endif
 #pragma unroll
         for (int v = 0; v < PV; ++v)
 #pragma unroll
@@ -826,11 +806,6 @@ struct Acc<float, NIT, CX> {
         const float4 a0 = *reinterpret_cast<const float4 *>(ap + i * 32);
         const float4 a1 = *reinterpret_cast<const float4 *>(ap + i * 32 + 16);
         const float av[8] = {a0.x, a0.y, a0.z, a0.w, a1.x, a1.y, a1.z, a1.w};
-#if FRB_DENSE_SKIP
-        // the operator values are broadcast loads, so this branch is warp-uniform: an all-zero (row group, k) costs no FFMA
-        if (a0.x == 0.f && a0.y == 0.f && a0.z == 0.f && a0.w == 0.f && a1.x == 0.f && a1.y == 0.f && a1.z == 0.f && a1.w == 0.f)
-          continue;
-#endif
 #pragma unroll
         for (int r = 0; r < 8; ++r)
 #pragma unroll
