@@ -124,6 +124,8 @@ inline std::vector<PanelGeom> list_geoms(int G, int min_ne, int max_ne, int trip
   // two groups help some FP64 kernels and hurt most FP32 ones (profiles/r01_c_fusion_notes.md): both are candidates, the static
   // score favours them in FP64 only, and the autotuner decides on large meshes
   const int ngmax = getenv("FRB_PANEL_NG") ? atoi(getenv("FRB_PANEL_NG")) : 2;
+  // FRB_MIN_EFF: row-warps without rows still issue copies, which can pay (profiles/r01_j_panel_source_level.md)
+  const double min_eff = getenv("FRB_MIN_EFF") ? atof(getenv("FRB_MIN_EFF")) : 0.7;
   for (int NG = 1; NG <= ngmax; ++NG)
     for (int WR = 1; WR <= PANEL_MAXW; ++WR) {
       const int nit = ((GU + WR - 1) / WR) * gu;
@@ -135,7 +137,7 @@ inline std::vector<PanelGeom> list_geoms(int G, int min_ne, int max_ne, int trip
           const int NE = (f64 ? 8 : 32) * CX * WC;
           if (NE < min_ne || NE > max_ne) continue;
           double eff = (double)G / (WR * nit);
-          if (eff < 0.7) continue;                       // more than 30 % of the row slots empty: never worth timing
+          if (eff < min_eff) continue;                   // more than 30 % of the row slots empty: not timed by default
           // prefer many warps, then wider panels, then fewer accumulators
           double score = eff * (0.4 + 0.6 * std::min(W, 14) / 14.0) * (1.0 + 0.02 * std::log2((double)NE)) * (1.0 - 0.005 * nit * CX);
           // dense operators: the B fragments of a k-block are shared by the NIT row groups of the warp; shared-memory
