@@ -216,6 +216,7 @@ struct GradEpilogue {
   template <typename ACC>
   __device__ __forceinline__ void prefetch(ACC &acc, const int *rowmap, int slot0, long long, long long pl, int wc, int lane) const {
     const long long e0 = pl * NE;
+    if (!curved && slot0 != 0) return;      // per-element metric terms: the first row-warp's prefetch covers the panel
     acc.foreach_coord(wc, lane, [&](int i, int rr, int e) {
       if (i % 3 != 0) return;
       const int rho = rowmap[(slot0 + i) * 8 + (ACC::ROWS == 1 ? (lane >> 2) : rr)];
