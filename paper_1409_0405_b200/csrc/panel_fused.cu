@@ -407,6 +407,11 @@ int launch_fused_grad(const PanelOp<T> &op, const EleView<T> &ev, const T *u, co
                       const PhysParams<T> &ph, cudaStream_t s) {
   GradArgs<T> a;
   a.op = op;
+  // The L2 prefetch of the epilogue's metric terms pays only in FP64 with per-element terms (tet S3+S4 1.54 -> 1.46 ms); with
+  // per-point terms (20 lines per thread) and in FP32 it costs more issue slots than the latency it hides (pri S3+S4 FP64
+  // 1.07 -> 1.00 ms without, tet S3+S4 FP32 1.27 -> 1.18 ms; profiles/r01_j_panel_source_level.md item 7).  Bit 2 of dbg makes
+  // panel_mainloop skip it -- decided here so that the kernels' code is untouched (an in-kernel test cost FP64 tets 12 %).
+  if (!ev.affine || sizeof(T) == 4) a.op.dbg |= 4;
   ColMap cm{op.NE, ev.ld, 0, ev.ld};
   a.prod = PlainProducer<T>();
   a.prod.src[0] = MatRef<T>{u, 5 * ev.ld, 0};
