@@ -56,12 +56,12 @@ def config1(numbering="natural"):
     return case
 
 
-def config2(n=16, p=3, system="ns", mu=1e-3, numbering="natural", state_kind="vortex", curve=0.0):
+def config2(n=16, p=3, system="ns", mu=1e-3, numbering="natural", state_kind="vortex", curve=0.0, ldg_beta=0.5, ldg_tau=0.1):
     """BASELINE.json configs[1]: periodic unit box, n^3 cells, lower half prisms / upper half tets
     (reading R18 for the counts), NS mu=1e-3 Pr=0.72, LDG beta=1/2 tau=0.1, isentropic vortex.
     curve > 0: the same mesh with quadratically curved elements."""
     m = _mesh.box_mixed(n, 1.0, numbering=numbering, seed=SEEDS["c2"], curve=curve)
-    case = build_case(m, p, system=system, mu=mu if system == "ns" else 0.0)
+    case = build_case(m, p, system=system, mu=mu if system == "ns" else 0.0, ldg_beta=ldg_beta, ldg_tau=ldg_tau)
     if state_kind == "vortex":
         case["u0"] = [state.isentropic_vortex(e["xu"]) for e in case["eles"]]
     else:
@@ -80,15 +80,17 @@ def config_hex(n=8, p=3, system="ns", mu=1e-3, numbering="natural", warp=0.0, st
     return case
 
 
-def config3(p=4, ntheta=100, nz=15, nlayers=40, nr=40, numbering="morton", system="ns", amp=0.005, seed=None, quadratic=False):
+def config3(p=4, ntheta=100, nz=15, nlayers=40, nr=40, numbering="morton", system="ns", amp=0.005, seed=None, quadratic=False,
+            mach=0.2, ldg_beta=0.5, ldg_tau=0.1):
     """BASELINE.json configs[2] (and [4] when scaled): cylinder-like O-mesh, NS at Re=3900, M=0.2
-    (PAPER.md:86-94,116), wall T_w = T_inf, far field = freestream, seeded 0.5 % perturbation."""
+    (PAPER.md:86-94,116), wall T_w = T_inf, far field = freestream, seeded 0.5 % perturbation.
+    `mach` > 1 drives the far-field boundary through its supersonic in- and outflow branches (test input only)."""
     seed = SEEDS["c3"] if seed is None else seed
     m = _mesh.cylinder_omesh(ntheta, nz, nlayers, nr, numbering=numbering, seed=seed, quadratic=quadratic)
-    gamma, mach = state.GAMMA, 0.2
+    gamma = state.GAMMA
     fs = dict(rho=1.0, v=(1.0, 0.0, 0.0), p=1.0 / (gamma * mach * mach))
     e_w = fs["p"] / ((gamma - 1) * fs["rho"])
-    case = build_case(m, p, system=system, mu=1.0 / 3900.0 if system == "ns" else 0.0,
+    case = build_case(m, p, system=system, mu=1.0 / 3900.0 if system == "ns" else 0.0, ldg_beta=ldg_beta, ldg_tau=ldg_tau,
                       bc_types={0: "wall", 1: "farfield"},
                       bc_params={0: [e_w], 1: [fs["rho"], *fs["v"], fs["p"]]})
     u0 = [state.freestream(e["xu"], **fs) for e in case["eles"]]

@@ -7,10 +7,11 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libfrb200.so")
 SOURCES = ["api.cu", "gemm.cu", "panel_gemm.cu", "panel_fused.cu", "pointwise.cu", "rk_adapt.cu", "peaks.cu"]
-HEADERS = ["common.cuh", "kernels.cuh", "physics.cuh", "panel.cuh", "panel_kernel.cuh", os.path.join("..", "..", "include", "frb200.h")]
+HEADERS = ["common.cuh", "kernels.cuh", "physics.cuh", "panel.cuh", "panel_kernel.cuh", "tma.cuh", os.path.join("..", "..", "include", "frb200.h")]
 NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
               "-Xcompiler", "-fPIC", "--expt-relaxed-constexpr"] + (
-                  ["-DFRB_NSTAGE=" + os.environ["FRB_NSTAGE"]] if os.environ.get("FRB_NSTAGE") else [])
+                  # measurement aids (skip-multiply / skip-epilogue switches, plan printing): never in the default build
+                  ["-DFRB_DEBUG_KNOBS"] if os.environ.get("FRB_DEBUG_KNOBS") else [])
 
 
 def _nvcc():

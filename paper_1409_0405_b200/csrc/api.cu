@@ -53,7 +53,6 @@ struct DevBuf {
 };
 
 enum { CAT_GEMM = 0, CAT_PW = 1, CAT_IFACE = 2 };
-constexpr bool kFuseFluxIntoGrad = false;
 constexpr long long kIfaceBlock = 256;  // elements per locality block of the interface pair order
 
 // Per-kernel CUDA-event timeline of one RHS evaluation (measurement aid; never active on the normal path).
@@ -127,8 +126,7 @@ struct EleData {
   std::vector<FusedPart<T>> pDiv, pGrad;
   DevBuf<T> X, Y, ACC;   // solution register, stage input, RK4 accumulator
   DevBuf<T> E, U0;       // adaptive RK45: error register, state at the start of the attempt (allocated on first use)
-  DevBuf<T> grad;        // [3][nupts][5][ld]: G~ -> G (-> F~ on the unfused path)
-  DevBuf<T> ftil;        // [3][nupts][5][ld]: F~ written by the fused gradient kernel (NS, fused mode)
+  DevBuf<T> grad;        // [3][nupts][5][ld]: G~ -> G -> F~ (S6 in place)
   DevBuf<T> R;           // [nupts][5][ld]
   ~EleData() {
     gemm_plan_free(pM0);
@@ -283,11 +281,6 @@ struct Ctx : CtxBase {
       e->Y.alloc(nstate);
       if (stepper == FR_RK4) e->ACC.alloc(nstate);
       e->grad.alloc(3 * nstate);
-      // Forming F~ in the epilogue of the fused gradient kernel (S6 fused, GradEpilogue with ftil != nullptr) is implemented and
-      // parity-tested but measured slower than the stand-alone S6 kernel, which runs at the HBM roofline: the epilogue's metric and
-      // state loads are latency-bound while the tensor pipe idles (profiles/r01_c_fusion_notes.md).  Off until the epilogue is
-      // fed through shared memory.
-      if (kFuseFluxIntoGrad && !e->pGrad.empty() && !e->pDiv.empty()) e->ftil.alloc(3 * nstate);
       e->R.alloc(nstate);
       tt.ubase[t] = utot;
       tt.gbase[t] = gtot;
@@ -330,7 +323,7 @@ struct Ctx : CtxBase {
   // The static score of choose_geom ranks the (warps x row groups x column blocks x warp groups) candidates of an operator;
   // which one is fastest depends on things it does not model (register allocation, barrier skew, epilogue latency).  For
   // meshes large enough to time reliably, fr_setup launches the first kTuneCands candidates on the context's own arrays and
-  // keeps the fastest.  Results do not depend on the choice (the summation order over k is the same for every geometry).
+  // keeps the fastest.  Results do not depend on the choice: bit-identical for every geometry (tests/test_gpu_parity.py).
   static constexpr int kTuneCands = 14;
   static constexpr long long kTuneMinEles = 16384;
   template <typename B, typename L>
@@ -357,24 +350,31 @@ struct Ctx : CtxBase {
     };
     PanelOp<T> best = cur;
     float bt = time_op(best);
+#ifdef FRB_DEBUG_KNOBS
     const bool verbose = getenv("FRB_PANEL_VERBOSE") != nullptr;
+#else
+    const bool verbose = false;
+#endif
     if (verbose) fprintf(stderr, "autotune %s cand 0: %.3f ms\n", what, bt);
-    const bool both = cur.density > 0.25 && cur.density < 0.95;   // intermediate density: also time the other packing
+    // only the launch geometry varies between candidates: the packing (k-lists or dense k-blocks) and the composition of every
+    // k-block depend on the operator alone (panel.cuh), so every candidate gives bit-identical results
     const int ncand = getenv("FRB_TUNE_CANDS") ? std::max(1, atoi(getenv("FRB_TUNE_CANDS"))) : kTuneCands;
-    for (int pass = 0; pass < (both ? 2 : 1); ++pass)
-      for (int k = pass ? 1000 : 1; k < (pass ? 1000 + ncand / 2 : ncand); ++k) {
-        PanelOp<T> op;
-        if (!build(op, k)) break;
-        const float t = time_op(op);
-        if (verbose) fprintf(stderr, "autotune %s cand %d: %.3f ms\n", what, k, t);
-        if (t < bt) {
-          panel_op_free(best);
-          best = op;
-          bt = t;
-        } else {
-          panel_op_free(op);
-        }
+    for (int k = 1, miss = 0; k < ncand + miss && miss < 64; ++k) {
+      PanelOp<T> op;
+      if (!build(op, k)) {
+        ++miss;                  // the candidate does not fit shared memory (or does not exist): try the next
+        continue;
       }
+      const float t = time_op(op);
+      if (verbose) fprintf(stderr, "autotune %s cand %d: %.3f ms\n", what, k, t);
+      if (t < bt) {
+        panel_op_free(best);
+        best = op;
+        bt = t;
+      } else {
+        panel_op_free(op);
+      }
+    }
     cur = best;
     cudaEventDestroy(e0);
     cudaEventDestroy(e1);
@@ -406,7 +406,7 @@ struct Ctx : CtxBase {
           tune(q.op,
                [&](PanelOp<T> &op, int k) { return fused_grad_build(op, nu, nf, d.M460, d.M6, k, jump ? d.M0 : nullptr, q.r0, q.nr); },
                [&](const PanelOp<T> &op) {
-                 launch_fused_grad(op, e.view, (const T *)e.X.p, (const T *)(cf.p + tt.ubase[t]), e.grad.p, (T *)nullptr, ph, stream);
+                 launch_fused_grad(op, e.view, (const T *)e.X.p, (const T *)(cf.p + tt.ubase[t]), e.grad.p, stream);
                },
                (tag + ":[M460|M6]").c_str());
     }
@@ -544,12 +544,10 @@ struct Ctx : CtxBase {
       const double n = (double)e.view.neles, nu = e.view.nupts, nf = e.view.nfpts;
       const double nmet = e.view.affine ? 1 : nu;
       if (!e.pGrad.empty()) {
-        // S3 + S4 (+S6) fused: G = (1/|J|) S^T ([M460 | M6] [U; C]);  F~ = S (f_inv(U) - f_visc(U, G))
-        for (auto &g : e.pGrad) nk += launch_fused_grad(g.op, e.view, u[t], cf.p + tt.ubase[t], e.grad.p, e.ftil.p, ph, q);
-        const bool fl = e.ftil.p != nullptr;
-        mark(CAT_GEMM, t, fl ? "S3_S4_S6_fused_grad_flux" : "S3_S4_fused_grad",
-             (5 * nu + 5 * nf + 15 * nu + 10 * nmet + (fl ? 15 * nu : 0)) * n,
-             2 * parts_density(e.pGrad) * 3 * nu * (nu + nf) * 5 * n + 15 * 6 * nu * n + (fl ? 210 * nu * n : 0));
+        // S3 + S4 fused: G = (1/|J|) S^T ([M460 | M6] [U; C])
+        for (auto &g : e.pGrad) nk += launch_fused_grad(g.op, e.view, u[t], cf.p + tt.ubase[t], e.grad.p, q);
+        mark(CAT_GEMM, t, "S3_S4_fused_grad", (5 * nu + 5 * nf + 15 * nu + 10 * nmet) * n,
+             2 * parts_density(e.pGrad) * 3 * nu * (nu + nf) * 5 * n + 15 * 6 * nu * n);
       } else {
         // S3: G~ = M460 U + M6 C
         nk += gemm_run(e.pM460, n5, T(1), u[t], n5, 0, T(0), e.grad.p, n5, 0, 1, q);
@@ -573,7 +571,6 @@ struct Ctx : CtxBase {
     };
     auto do_S6 = [&](int t, cudaStream_t q) {
       EleData<T> &e = *el[t];
-      if (e.ftil.p) return;
       const double n = (double)e.view.neles, nu = e.view.nupts;
       const double nmet = e.view.affine ? 1 : nu;
       nk += launch_tdisf(e.view, u[t], e.grad.p, ph, q);   // S6 (Euler, or unfused): F~ in place over G
@@ -584,7 +581,7 @@ struct Ctx : CtxBase {
       const long long n5 = 5 * e.view.ld;
       const double n = (double)e.view.neles, nu = e.view.nupts, nf = e.view.nfpts;
       const double nmet = e.view.affine ? 1 : nu;
-      const T *ft = e.ftil.p ? e.ftil.p : e.grad.p;
+      const T *ft = e.grad.p;
       if (!e.pDiv.empty()) {
         // S8 + S9 (+S10) fused: out = -(1/|J|) [M132 | M3] [F~; D], stage update in the epilogue
         for (auto &g : e.pDiv) nk += launch_fused_div(g.op, e.view, ft, uf.p + tt.ubase[t], sa[t], q);
@@ -1099,8 +1096,8 @@ fr_status fr_gemm_plan_create(int32_t M, int32_t K, const double *A_host, fr_pre
     require_device();
     auto p = std::make_unique<fr_gemm_plan>();
     p->prec = prec;
-    if (prec == FR_F64) frb::gemm_plan_build(p->pd, M, K, A_host);
-    else frb::gemm_plan_build(p->pf, M, K, A_host);
+    if (prec == FR_F64) frb::gemm_plan_build(p->pd, M, K, A_host, 0.0);
+    else frb::gemm_plan_build(p->pf, M, K, A_host, 0.0);
     *out = p.release();
   });
 }

@@ -80,8 +80,10 @@ struct GemmPlan {
   int part_row0[kMaxParts] = {};
 };
 
+// drop_rel: entries with |a| <= drop_rel * max|A| are treated as structural zeros when the operator is packed (reading R24: the FR
+// operators handed to fr_setup); the public fr_gemm passes 0 (only exact zeros are skipped)
 template <typename T>
-void gemm_plan_build(GemmPlan<T> &p, int M, int K, const double *A_host);
+void gemm_plan_build(GemmPlan<T> &p, int M, int K, const double *A_host, double drop_rel = 1.4210854715202004e-14);
 template <typename T>
 void gemm_plan_free(GemmPlan<T> &p);
 // C[b] <- c1 * A * B[b] + c2 * C[b], b < nbatch; returns the number of kernels launched

@@ -19,7 +19,7 @@
 namespace frb {
 
 template <typename T>
-bool panel_gemm_build(PanelOp<T> &op, int M, int K, const double *A, int cand = 0);
+bool panel_gemm_build(PanelOp<T> &op, int M, int K, const double *A, int cand = 0, double drop_rel = 1.4210854715202004e-14);
 template <typename T>
 void panel_gemm_run(const PanelOp<T> &op, long long N, T c1, const T *B, long long ldb, long long bsB, T c2, T *C,
                     long long ldc, long long bsC, int nbatch, cudaStream_t s);
@@ -240,18 +240,15 @@ void launch_ty(const GemmPlan<T> &p, const GemmArgs<T> &a, int grid, cudaStream_
 }  // namespace
 
 int device_sm_count() {
-  static int n = 0;
-  if (n == 0) {
-    int dev = 0;
-    cudaGetDevice(&dev);
-    cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev);
-    if (n <= 0) n = 148;
-  }
-  return n;
+  // per device: a process may drive several (one context per host thread, include/frb200.h)
+  int dev = 0, n = 0;
+  cudaGetDevice(&dev);
+  cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev);
+  return n > 0 ? n : 148;
 }
 
 template <typename T>
-void gemm_plan_build(GemmPlan<T> &p, int M, int K, const double *A_host) {
+void gemm_plan_build(GemmPlan<T> &p, int M, int K, const double *A_host, double drop_rel) {
   FR_REQUIRE(M > 0 && K > 0 && A_host, "gemm: M, K must be positive and A non-NULL");
   constexpr int CT = VecT<T>::CT;
   p.M = M;
@@ -262,7 +259,7 @@ void gemm_plan_build(GemmPlan<T> &p, int M, int K, const double *A_host) {
     auto *pop = new PanelOp<T>();
     bool ok = false;
     try {
-      ok = panel_gemm_build(*pop, M, K, A_host);
+      ok = panel_gemm_build(*pop, M, K, A_host, 0, drop_rel);
     } catch (...) {
       delete pop;
       throw;
@@ -284,7 +281,7 @@ void gemm_plan_build(GemmPlan<T> &p, int M, int K, const double *A_host) {
       p.part[n] = pop;
       p.part_row0[n] = r0;
       try {
-        ok = panel_gemm_build(*pop, std::min(per, M - r0), K, A_host + (size_t)r0 * K);
+        ok = panel_gemm_build(*pop, std::min(per, M - r0), K, A_host + (size_t)r0 * K, 0, drop_rel);
       } catch (...) {
         ok = false;
       }
@@ -398,8 +395,8 @@ int gemm_run(const GemmPlan<T> &p, long long N, T c1, const T *B, long long ldb,
   return 1;
 }
 
-template void gemm_plan_build<double>(GemmPlan<double> &, int, int, const double *);
-template void gemm_plan_build<float>(GemmPlan<float> &, int, int, const double *);
+template void gemm_plan_build<double>(GemmPlan<double> &, int, int, const double *, double);
+template void gemm_plan_build<float>(GemmPlan<float> &, int, int, const double *, double);
 template void gemm_plan_free<double>(GemmPlan<double> &);
 template void gemm_plan_free<float>(GemmPlan<float> &);
 template int gemm_run<double>(const GemmPlan<double> &, long long, double, const double *, long long, long long, double,

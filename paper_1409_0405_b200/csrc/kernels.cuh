@@ -77,12 +77,12 @@ template <typename T>
 bool fused_grad_build(PanelOp<T> &op, int nu, int nf, const double *M460, const double *M6, int cand = 0, const double *M0_jump = nullptr,
                       int r0 = 0, int nr = -1);
 template <typename T>
-int launch_fused_grad(const PanelOp<T> &op, const EleView<T> &ev, const T *u, const T *c, T *grad, T *ftil,
-                      const PhysParams<T> &ph, cudaStream_t s);
+int launch_fused_grad(const PanelOp<T> &op, const EleView<T> &ev, const T *u, const T *c, T *grad, cudaStream_t s);
 
 // Plain operator product on the panel kernels (panel_gemm.cu); `cand` as above.
+// drop_rel: entries with |a| <= drop_rel * max|A| count as structural zeros (reading R24; 0 = exact zeros only)
 template <typename T>
-bool panel_gemm_build(PanelOp<T> &op, int M, int K, const double *A, int cand = 0);
+bool panel_gemm_build(PanelOp<T> &op, int M, int K, const double *A, int cand = 0, double drop_rel = 1.4210854715202004e-14);
 template <typename T>
 void panel_gemm_run(const PanelOp<T> &op, long long N, T c1, const T *B, long long ldb, long long bsB, T c2, T *C,
                     long long ldc, long long bsC, int nbatch, cudaStream_t s);

@@ -5,17 +5,20 @@
 // -- while B streams through shared memory in K-chunks and the accumulators stay in registers.
 //
 // B200 design:
-//   * the operator is packed once at fr_setup into 8-row groups with a compact list of the k indices that are non-zero
-//     in the group (dense operators: all k; prism operators are 15-45 % dense and skip the rest) and stays resident in
-//     shared memory for the life of the persistent CTA;
-//   * FP64 multiplies on the FP64 tensor pipe, mma.sync.m8n8k4.f64 (DMMA: measured 37.1 TFLOP/s on B200 against 33.7
-//     for a DFMA chain, with 1/8 of the issue slots and a fraction of the shared-memory operand traffic);
+//   * the operator is packed once at fr_setup into 8-row groups (dense operators: every k of a chunk, in k-blocks shared by
+//     all groups; sparse operators: per group a compact list of the k that are non-zero in it) and stays resident in shared
+//     memory for the life of the persistent CTA;
+//   * B chunks are moved by the TMA unit (cp.async.bulk.tensor from tensor maps over the state matrices, tma.cuh): a producer
+//     warp per warp group issues the copies into a ring of stages, each stage guarded by a full and an empty mbarrier; the
+//     consumer warps never issue a copy and never meet at a CTA-wide barrier;
+//   * FP64 multiplies on the FP64 tensor pipe, mma.sync.m8n8k4.f64 (DMMA), reading its B fragments from the 128-byte-swizzled
+//     stage; the four rows of a k-block are chosen at set-up so that these loads are bank-conflict free;
 //     FP32 multiplies with FFMA on register tiles of 8 rows x 5 variables x (1|2) elements (no TF32: the 2e-5 parity
 //     bound excludes it, and tcgen05 has no FP32/FP64 kind);
-//   * B chunks arrive through a multi-stage cp.async ring that runs across panel boundaries; rows are padded so that the
-//     DMMA fragment loads are bank-conflict free;
-//   * producers (how a B chunk comes to be) and epilogues (what happens to the accumulators) are policies, which is how the
-//     point-wise flux, gradient transform, -1/|J| scaling and Runge-Kutta stage update are fused into the products.
+//   * the chunking of K and the composition of every k-block depend on the operator alone, never on the launch geometry, so
+//     every geometry the autotuner may pick gives bit-identical results;
+//   * epilogues (what happens to the accumulators) are policies, which is how the gradient transform, the -1/|J| scaling and
+//     the Runge-Kutta stage update are fused into the products.
 #pragma once
 #include <algorithm>
 #include <cmath>
@@ -28,17 +31,16 @@
 namespace frb {
 
 constexpr int PV = FR_NVAR;          // variable segments per panel
-constexpr int PANEL_MAXW = 16;       // warps per CTA (upper bound; 8 when the accumulators need > 128 registers)
+constexpr int PANEL_MAXW = 20;       // warps per CTA, producers included (fewer when the accumulators need more registers)
 constexpr int PANEL_MAXCHUNKS = 64;
-#ifndef FRB_NSTAGE
-#define FRB_NSTAGE 2
-#endif
-constexpr int PANEL_NSTAGE = FRB_NSTAGE;   // cp.async ring depth: 2 beats 3 and 4 on config 3 (taller chunks, fewer barriers; profiles/r01_c_fusion_notes.md)
+constexpr int PANEL_KCMAX = 40;      // rows per chunk (upper bound; a multiple of 8)
+constexpr int PANEL_MAXSTAGE = 8;    // ring depth (upper bound)
+constexpr int PANEL_MAXSRC = 2;      // matrices stacked along K
 
-// One K-chunk of the stacked right-hand operand: rows [row0, row0+nrows) of source `src`.
+// One K-chunk of the stacked right-hand operand: rows [row0, row0+nrows) of source `src`, copied as a box of `step` rows.
 struct ChunkDesc {
-  int src, row0, nrows, kind;
-  int base, pad0, pad1, pad2;   // dense operators: first packed block (FP64: 4 rows) / row (FP32) of this chunk
+  int src, row0, nrows, step;
+  int base, nblk, pad0, pad1;   // dense operators: first packed block of this chunk and their number (FP64: k-blocks of 4 rows; FP32: rows)
 };
 
 // Device image of a packed operator + its launch geometry (all pointers device).
@@ -49,21 +51,28 @@ struct PanelOp {
   int NE = 0;                            // elements per panel (of one warp group)
   int NG = 1;                            // independent warp groups per CTA, each streaming its own panels (staggered)
   int occ = 1;                           // CTAs per SM the plan was sized for (shared memory and registers)
-  int KC = 0, nchunks = 0, NS = 0;       // rows per chunk (max), chunks, slots = WR*NIT
-  int stage_elems = 0;                   // elements of one ring stage
-  int curved = 0;                        // flux chunks: metric terms per point (1) or per element (0)
+  int nchunks = 0, NS = 0;               // chunks, slots = WR*NIT
+  int nstage = 0;                        // ring depth
+  int stage_bytes = 0;                   // bytes of one ring stage (multiple of 1024)
   int nblk = 0;                          // packed blocks (FP64: 8x4 tiles; FP32: 8x1 columns)
   int nidx = 0;                          // entries of idx
+  int pf_epi = 0;                        // the epilogue's global operands are pulled into L2 before the last chunk (set by the launcher)
+#ifdef FRB_DEBUG_KNOBS
   int dbg = 0;                           // measurement aid (env FRB_PANEL_DBG): 1 skip multiply, 2 skip epilogue
-  int sparse = 0;                        // 1: per-group k-lists (idx/off); 0: dense, all slots share the chunk's rows
+#endif
+  int sparse = 0;                        // 1: per-group k-lists (idx/off); 0: dense, all slots share the chunk's k-blocks
+  int nsrc = 0;
+  int src_rows[PANEL_MAXSRC] = {0, 0};   // rows of each stacked source
+  int src_step[PANEL_MAXSRC] = {0, 0};   // rows per chunk (TMA box height) of each source
   double macs_per_col = 0;               // executed multiply-adds per column (dense: M*K)
   double density = 1;                    // fraction of non-zero entries of the operator
   T *vals = nullptr;                     // FP64 [nblk][32]; FP32 [nblk][8]
-  uint32_t *idx = nullptr;               // byte offset of the B row in the stage: FP64 [nblk][4], FP32 [nblk]
-  int *off = nullptr;                    // [nchunks*NS + 1]
+  uint32_t *idx = nullptr;               // byte offset of the B row in a stage plane: FP64 [..][4] (swizzle term included), FP32 [..]
+  int *off = nullptr;                    // sparse: [nchunks*NS + 1]
   int *rowmap = nullptr;                 // [NS*8] actual row of (slot, r) or -1
   ChunkDesc *chunks = nullptr;           // [nchunks]
   size_t smem_op = 0;                    // bytes of the operator image in shared memory
+  size_t bytes_vals = 0, bytes_idx = 0, bytes_off = 0, bytes_rowmap = 0, bytes_chunks = 0;   // each a multiple of 16
   bool ok() const { return vals != nullptr; }
 };
 
@@ -77,23 +86,10 @@ void panel_op_free(PanelOp<T> &p) {
   p = PanelOp<T>();
 }
 
-// How the K dimension of the operator is fed: a list of sources stacked along K, each cut into chunks of at most KC rows.
-// kind 0: `rows` plain rows of a global matrix <-> `rows` columns of A.
-// kind 1 (kept for producers that transform a chunk in shared memory -- kTransform in panel_kernel.cuh; not used by the kernels of
-//         this round, see panel_fused.cu for why): transformed flux at `rows` solution points <-> 3*rows columns of A (alpha-major: column alpha*rows + nu); a chunk
-//         of n points occupies stage rows [0,3n) (alpha-major within the chunk: row alpha*n + j) for G -> F~, rows [3n,4n)
-//         for U, followed by the metric terms (flux_stage_elems).
+// How the K dimension of the operator is fed: a list of matrices stacked along K, `rows` plain rows each <-> `rows` columns of A.
 struct KSource {
   int rows;
-  int kind;
-  int unit;      // unused (kept for aggregate initialisation)
 };
-constexpr int KIND_PLAIN = 0, KIND_FLUX = 1;
-
-// shared-memory elements of one stage holding a flux chunk of n points
-inline __host__ __device__ size_t flux_stage_elems(int n, int NE, int LDB, int curved) {
-  return (size_t)4 * n * LDB + (size_t)9 * (curved ? n : 1) * NE;
-}
 
 struct PanelGeom {
   int WR, WC, NIT, CX, NE;
@@ -102,66 +98,57 @@ struct PanelGeom {
   int occ;
 };
 
-// Warps per CTA a given accumulator shape allows: registers per thread ~ accumulators + 70 must fit the 64K register file.
-// FP64: NIT*CX*10 doubles per thread; FP32: NIT*CX*40 floats.
+// Warps per CTA (consumers + one producer per group) a given accumulator shape allows: a multiple of four (ptxas sizes the
+// register budget for whole quads of warps, one per SM sub-partition), the largest whose register share still leaves the
+// accumulators 48 registers of head-room.  FP64: NIT*CX*10 doubles per thread; FP32: NIT*CX*40 floats.
 template <typename T>
 constexpr int panel_maxw(int nit, int cx) {
-  // FP32 tiles also keep 8 operator values and 5*CX state values live per k and index more arrays: with only +70 registers of
-  // head-room the CX = 2 shapes spilled inside the multiply loop (8x slower), so FP32 with CX = 2 budgets +110.
-  const int acc_regs = sizeof(T) == 8 ? nit * cx * 20 : nit * cx * 40;
-  const int w = 2048 / (acc_regs + ((sizeof(T) == 4 && cx == 2) ? 110 : 70));
-  return w > 16 ? 16 : (w < 1 ? 1 : w);
+  // FP32 tiles also keep 8 operator values and 5*CX state values live per k and index more arrays: the CX = 2 shapes spill
+  // inside the multiply loop with little head-room (8x slower), so FP32 with CX = 2 budgets +110.
+  const int need = (sizeof(T) == 8 ? nit * cx * 20 : nit * cx * 40) + ((sizeof(T) == 4 && cx == 2) ? 110 : 48);
+  int w = PANEL_MAXW / 4 * 4;
+  while (w > 8 && 2048 / w < need) w -= 4;
+  return w;
 }
 
-// Choose the warp grid for G row groups.  The FP64 tensor pipe takes one DMMA per warp every ~32 cycles, so two warps per
-// scheduler saturate it only if they do nothing else: prefer 12-16 warps per SM.
+// Candidate launch geometries for G row groups, best static score first.  The FP64 tensor pipe is per SM sub-partition: the
+// multiplying warps should spread evenly over the four of them.
 template <typename T>
 inline std::vector<PanelGeom> list_geoms(int G, int min_ne, int max_ne, int triple, bool dense) {
   std::vector<PanelGeom> all;
   const bool f64 = sizeof(T) == 8;
   const int gu = triple ? 3 : 1;            // groups come in units of `gu` that must stay on one row-warp
   const int GU = (G + gu - 1) / gu;
-  // two groups help some FP64 kernels and hurt most FP32 ones (profiles/r01_c_fusion_notes.md): both are candidates, the static
-  // score favours them in FP64 only, and the autotuner decides on large meshes
   const int ngmax = getenv("FRB_PANEL_NG") ? atoi(getenv("FRB_PANEL_NG")) : 2;
-  // FRB_MIN_EFF: row-warps without rows still issue copies, which can pay (profiles/r01_j_panel_source_level.md)
-  const double min_eff = getenv("FRB_MIN_EFF") ? atof(getenv("FRB_MIN_EFF")) : 0.7;
   for (int NG = 1; NG <= ngmax; ++NG)
     for (int WR = 1; WR <= PANEL_MAXW; ++WR) {
       const int nit = ((GU + WR - 1) / WR) * gu;
-      for (int WC = 1; NG * WR * WC <= PANEL_MAXW; WC *= 2) {
+      if (WR > 1 && ((GU + WR - 2) / (WR - 1)) * gu == nit) continue;   // same accumulators with fewer row-warps exist: skip the idle ones
+      for (int WC = 1; NG * WR * WC + NG <= PANEL_MAXW; ++WC) {
         for (int CX = 2; CX >= 1; --CX) {
           if (f64 ? nit * CX > 8 : nit * CX > 4) continue;
-          const int W = NG * WR * WC;
-          if (W > panel_maxw<T>(nit, CX)) continue;
+          const int W = NG * WR * WC;                          // consumer warps
+          if (W + NG > panel_maxw<T>(nit, CX)) continue;
           const int NE = (f64 ? 8 : 32) * CX * WC;
-          if (NE < min_ne || NE > max_ne) continue;
-          double eff = (double)G / (WR * nit);
-          if (eff < min_eff) continue;                   // more than 30 % of the row slots empty: not timed by default
-          // prefer many warps, then wider panels, then fewer accumulators
-          double score = eff * (0.4 + 0.6 * std::min(W, 14) / 14.0) * (1.0 + 0.02 * std::log2((double)NE)) * (1.0 - 0.005 * nit * CX);
-          // dense operators: the B fragments of a k-block are shared by the NIT row groups of the warp; shared-memory
-          // wavefronts per multiply ~ 2/NIT + 0.4/CX
+          // panels tile the padded leading dimension (a multiple of 128) exactly; FP64 stages are made of 16-element blocks
+          if (NE < min_ne || NE > max_ne || 128 % NE != 0 || (f64 && NE % 16)) continue;
+          const double eff = (double)G / (WR * nit);
+          // spread over the sub-partitions: the busiest of the four bounds the multiply rate
+          const double bal = (double)W / (4.0 * ((W + 3) / 4));
+          double score = eff * bal * (0.4 + 0.6 * std::min(W, 12) / 12.0) * (1.0 + 0.02 * std::log2((double)NE)) * (1.0 - 0.005 * nit * CX);
+          // dense operators: the B fragments of a k-block are shared by the NIT row groups of the warp
           if (dense) score /= 1.0 + 0.4 * (2.0 / nit + 0.4 / CX);
-          // two staggered warp groups hide one group's epilogue and load waits behind the other's multiplies
-          if (NG == 2) score *= f64 ? 1.25 : 0.85;
+          // two staggered warp groups hide one group's epilogue behind the other's multiplies
+          if (NG == 2) score *= f64 ? 1.15 : 0.9;
           all.push_back(PanelGeom{WR, WC, nit, CX, NE, score, NG, 1});
-          // two CTAs per SM (half the shared memory and registers each): another way to overlap one panel's epilogue and
-          // load waits with another's multiplies; only timing (fr_setup autotuning) tells which wins
-          if (NG == 1 && 2 * W <= panel_maxw<T>(nit, CX)) all.push_back(PanelGeom{WR, WC, nit, CX, NE, score * 0.9, NG, 2});
+          // two CTAs per SM (half the shared memory and registers each): the other way to overlap one panel's epilogue with
+          // another's multiplies; only timing (fr_setup autotuning) tells which wins
+          if (NG == 1 && 2 * (W + 1) <= panel_maxw<T>(nit, CX)) all.push_back(PanelGeom{WR, WC, nit, CX, NE, score * 0.9, NG, 2});
         }
       }
     }
   std::stable_sort(all.begin(), all.end(), [](const PanelGeom &x, const PanelGeom &y) { return x.eff > y.eff; });
   return all;
-}
-
-// Best geometry by the static score; fr_setup may instead time the first few candidates on the real arrays (PackOptions::cand).
-template <typename T>
-inline PanelGeom choose_geom(int G, int min_ne, int max_ne, int triple, bool dense, int cand = 0) {
-  const std::vector<PanelGeom> all = list_geoms<T>(G, min_ne, max_ne, triple, dense);
-  if (cand < 0 || cand >= (int)all.size()) return PanelGeom{0, 0, 0, 0, 0, -1.0, 1, 1};
-  return all[cand];
 }
 
 // Greedy clustering of rows into groups of 8 with similar column support (sparse operators only).
@@ -210,55 +197,104 @@ inline std::vector<int> cluster_rows(const std::vector<std::vector<uint8_t>> &su
 struct PackOptions {
   int min_ne = 16, max_ne = 64;
   int triple = 0;          // rows come as (alpha, rho) with alpha-major blocks of M/3: keep the three alpha of a rho in one thread
-  int kc = 0;              // rows per chunk (0 = default)
   int allow_sparse = 1;
-  int curved = 0;          // flux sources: per-point metric terms
   int cand = 0;            // k-th best geometry by static score (autotuning)
   const int *row_ids = nullptr;   // row split: the epilogue's row number of each row of A (nullptr = 0..M-1)
+  // entries with |a| <= drop_rel * max|A| are treated as structural zeros (reading R24); 0: only exact zeros
+  double drop_rel = 1.4210854715202004e-14;
 };
 
-// Pack A (M x K, host FP64, row-major) for the panel kernels.  `srcs` stacks the K dimension.  Returns false if the
-// operator does not fit the resident-in-shared-memory design (caller falls back to the streaming kernel).
-template <typename T>
-bool panel_op_build_kc(PanelOp<T> &p, int M, int K, const double *A, const std::vector<KSource> &srcs, const PackOptions &opt,
-                       size_t smem_budget, size_t smem_total, int kc_try, int *kc_fit);
+// Rows per chunk of a source with `rows` rows: the multiple of 8 (<= PANEL_KCMAX) with the fewest chunks, counting a fixed
+// per-chunk overhead worth six rows.  A function of `rows` alone (see the determinism note at the top).
+inline int panel_chunk_step(int rows) {
+  int best = 8;
+  long bestc = 1l << 60;
+  for (int step = 8; step <= PANEL_KCMAX; step += 8) {
+    const long nch = (rows + step - 1) / step;
+    const long c = nch * (step + 6);
+    if (c <= bestc) {
+      bestc = c;
+      best = step;
+    }
+  }
+  return best;
+}
 
-// Chunk height: as tall as the B ring allows (few, large cp.async stages keep enough bytes in flight to cover HBM latency
-// with one persistent CTA per SM); first try whole sources, then the height that makes three stages fit `smem_total`.
+// The four stage rows of each k-block of a chunk with n rows (FP64).  Inside a group of eight consecutive rows the even and
+// the odd rows form one block each: with the 128-byte swizzle the rows of a block then differ in (row & 7) >> 1, which makes
+// the DMMA B-fragment loads bank-conflict free.  A tail of at most four rows is one block.
+inline std::vector<std::vector<int>> dense_blocks_f64(int n) {
+  std::vector<std::vector<int>> out;
+  for (int g = 0; g < n; g += 8) {
+    const int t = std::min(8, n - g);
+    if (t <= 4) {
+      std::vector<int> b;
+      for (int j = 0; j < t; ++j) b.push_back(g + j);
+      out.push_back(b);
+    } else {
+      std::vector<int> ev, od;
+      for (int j = 0; j < t; ++j) (j & 1 ? od : ev).push_back(g + j);
+      out.push_back(ev);
+      out.push_back(od);
+    }
+  }
+  return out;
+}
+
+// Blocks of four from a list of stage rows, rows of a block from different bank classes ((row & 7) >> 1) where possible.
+inline std::vector<std::vector<int>> sparse_blocks_f64(const std::vector<int> &rows) {
+  std::vector<std::vector<int>> bucket(4), out;
+  for (int r : rows) bucket[(r & 7) >> 1].push_back(r);
+  size_t pos[4] = {0, 0, 0, 0};
+  size_t left = rows.size();
+  while (left > 0) {
+    std::vector<int> b;
+    bool took[4] = {false, false, false, false};
+    while (b.size() < 4 && left > 0) {
+      // the fullest class not yet in this block; when every class with rows left is in it already, the fullest one again
+      int q = -1;
+      for (int pass = 0; pass < 2 && q < 0; ++pass)
+        for (int c = 0; c < 4; ++c) {
+          const size_t rem = bucket[c].size() - pos[c];
+          if (rem == 0 || (pass == 0 && took[c])) continue;
+          if (q < 0 || rem > bucket[q].size() - pos[q]) q = c;
+        }
+      b.push_back(bucket[q][pos[q]++]);
+      took[q] = true;
+      --left;
+    }
+    out.push_back(b);
+  }
+  return out;
+}
+
+// byte offset of stage row r inside a plane, with the swizzle term of its 128-byte line in bits 4..6
+inline uint32_t swz_row_offset(int r) { return (uint32_t)r * 128u + (uint32_t)(r & 7) * 16u; }
+
+// Pack A (M x K, host FP64, row-major) for the panel kernels.  `srcs` stacks the K dimension.  Returns false if the
+// operator does not fit the resident-in-shared-memory design with geometry candidate opt.cand (or the candidate does not exist).
 template <typename T>
-bool panel_op_build(PanelOp<T> &p, int M, int K, const double *A, const std::vector<KSource> &srcs, const PackOptions &opt,
-                    size_t smem_budget, size_t smem_total = 220 * 1024) {
-  // FRB_FORCE_CAND=k: build candidate k (geometry + 1000 * opposite packing) where the caller asked for the default; falls back
-  // to the default if k does not exist for this operator.  Lets the parity tests cover every candidate the autotuner may pick.
+bool panel_op_build(PanelOp<T> &p, int M, int K, const double *A, const std::vector<KSource> &srcs, const PackOptions &opt_in,
+                    size_t smem_budget, size_t smem_total = 226 * 1024) {
+  PackOptions opt = opt_in;
+  // FRB_FORCE_CAND=k: build geometry candidate k where the caller asked for the default; falls back to the default if k does
+  // not exist for this operator.  Lets the parity tests cover every candidate the autotuner may pick.
   if (opt.cand == 0 && getenv("FRB_FORCE_CAND")) {
     PackOptions o2 = opt;
     o2.cand = atoi(getenv("FRB_FORCE_CAND"));
-    if (o2.cand != 0 && panel_op_build(p, M, K, A, srcs, o2, smem_budget, smem_total)) return true;
+    if (o2.cand > 0 && panel_op_build(p, M, K, A, srcs, o2, smem_budget, smem_total)) return true;
   }
-  int kc = opt.kc > 0 ? opt.kc : 252;
-  for (int attempt = 0; attempt < 6 && kc >= 4; ++attempt) {
-    int fit = 0;
-    if (panel_op_build_kc(p, M, K, A, srcs, opt, smem_budget, smem_total, kc, &fit)) return true;
-    if (fit <= 0) return false;
-    kc = std::min(fit, kc - 4);
-  }
-  return false;
-}
-
-template <typename T>
-bool panel_op_build_kc(PanelOp<T> &p, int M, int K, const double *A, const std::vector<KSource> &srcs, const PackOptions &opt,
-                       size_t smem_budget, size_t smem_total, int kc_try, int *kc_fit) {
   const bool f64 = sizeof(T) == 8;
+  FR_REQUIRE((int)srcs.size() >= 1 && (int)srcs.size() <= PANEL_MAXSRC, "panel_op_build: one or two stacked sources");
   int ktot = 0;
-  for (auto &s : srcs) ktot += s.kind == KIND_FLUX ? 3 * s.rows : s.rows;
+  for (auto &s : srcs) ktot += s.rows;
   FR_REQUIRE(ktot == K, "panel_op_build: sources do not add up to K");
   double amax = 0;
   for (size_t i = 0; i < (size_t)M * K; ++i) {
     FR_REQUIRE(A[i] == A[i] && A[i] - A[i] == 0.0, "operator contains non-finite entries");
     amax = std::max(amax, std::fabs(A[i]));
   }
-  // structural zeros: entries below 2^-46 of the largest entry are dropped (reading R24)
-  const double thr = amax * 1.4210854715202004e-14;
+  const double thr = amax * opt.drop_rel;
   std::vector<std::vector<uint8_t>> sup(M, std::vector<uint8_t>(K, 0));
   size_t nnz = 0;
   for (int m = 0; m < M; ++m)
@@ -268,103 +304,105 @@ bool panel_op_build_kc(PanelOp<T> &p, int M, int K, const double *A, const std::
         ++nnz;
       }
   const double density = (double)nnz / ((double)M * K);
-  // automatic choice: k-lists below 60 % density; cand >= 1000 asks for the opposite packing (the autotuner times both for
-  // operators of intermediate density, e.g. [M4 | M6] of tetrahedra, 66 % dense, whose M6 half is zero for two faces per alpha)
-  const bool flip = opt.cand >= 1000 && density < 0.95;
-  const bool sparse = (opt.allow_sparse && density < 0.6) != flip;
-  // ---- rows -> groups of 8
-  std::vector<int> order;   // virtual row -> actual row or -1
-  if (opt.triple) {
-    FR_REQUIRE(M % 3 == 0, "triple packing needs M divisible by 3");
-    const int nu = M / 3;
-    std::vector<int> rho_order;
-    if (sparse) {
-      std::vector<std::vector<uint8_t>> s3(nu, std::vector<uint8_t>(K, 0));
-      for (int r = 0; r < nu; ++r)
-        for (int a = 0; a < 3; ++a)
-          for (int k = 0; k < K; ++k) s3[r][k] |= sup[a * nu + r][k];
-      rho_order = cluster_rows(s3, nu, K);
-    } else {
-      for (int r = 0; r < nu; ++r) rho_order.push_back(r);
-      while (rho_order.size() % 8) rho_order.push_back(-1);
-    }
-    // group 3g+a holds rows (a, rho_order[8g .. 8g+7])
-    for (size_t g = 0; g < rho_order.size() / 8; ++g)
-      for (int a = 0; a < 3; ++a)
-        for (int r = 0; r < 8; ++r) {
-          const int rho = rho_order[8 * g + r];
-          order.push_back(rho < 0 ? -1 : a * nu + rho);
-        }
-  } else if (sparse) {
-    order = cluster_rows(sup, M, K);
-  } else {
-    for (int m = 0; m < M; ++m) order.push_back(m);
-    while (order.size() % 8) order.push_back(-1);
-  }
-  const int G = (int)order.size() / 8;
-  // ---- chunks
-  const int KC = kc_try;
+  // ---- chunks: a function of the sources' row counts alone
   std::vector<ChunkDesc> chunks;
-  std::vector<std::vector<int>> chunk_cols;   // column of A behind each MAC row of the chunk's stage
+  std::vector<int> chunk_k0;   // column of A behind stage row 0 of the chunk
+  int src_step[PANEL_MAXSRC] = {0, 0};
   {
     int k0 = 0, si = 0;
     for (auto &s : srcs) {
-      if (s.kind == KIND_PLAIN) {
-        // equal chunks of at most KC rows, a multiple of 4 so that dense k-lists need no padding
-        const int nch = std::max(1, (s.rows + KC - 1) / KC);
-        int step = ((s.rows + nch - 1) / nch + 3) / 4 * 4;
-        if (step > KC) step = std::max(4, KC / 4 * 4);
-        for (int r = 0; r < s.rows; r += step) {
-          const int n = std::min(step, s.rows - r);
-          chunks.push_back(ChunkDesc{si, r, n, s.kind, 0, 0, 0, 0});
-          std::vector<int> cols(n);
-          for (int j = 0; j < n; ++j) cols[j] = k0 + r + j;
-          chunk_cols.push_back(cols);
-        }
-        k0 += s.rows;
-      } else {
-        const int nlim = std::max(1, KC / 3);
-        const int nch = std::max(1, (s.rows + nlim - 1) / nlim);
-        int step = (s.rows + nch - 1) / nch;
-        if ((step + 3) / 4 * 4 <= nlim) step = (step + 3) / 4 * 4;
-        for (int r = 0; r < s.rows; r += step) {
-          const int n = std::min(step, s.rows - r);
-          chunks.push_back(ChunkDesc{si, r, n, s.kind, 0, 0, 0, 0});
-          std::vector<int> cols(3 * n);
-          for (int a = 0; a < 3; ++a)
-            for (int j = 0; j < n; ++j) cols[a * n + j] = k0 + a * s.rows + r + j;
-          chunk_cols.push_back(cols);
-        }
-        k0 += 3 * s.rows;
+      const int step = panel_chunk_step(s.rows);
+      src_step[si] = step;
+      for (int r = 0; r < s.rows; r += step) {
+        chunks.push_back(ChunkDesc{si, r, std::min(step, s.rows - r), step, 0, 0, 0, 0});
+        chunk_k0.push_back(k0 + r);
       }
+      k0 += s.rows;
       ++si;
     }
   }
   const int nchunks = (int)chunks.size();
   if (nchunks > PANEL_MAXCHUNKS) return false;
-  int kcmax = 0;
-  for (auto &c : chunk_cols) kcmax = std::max(kcmax, (int)c.size());
-  if (kcmax > 8000) return false;
-  // ---- cost of each group (number of listed k) and its assignment to row-warps
-  std::vector<std::vector<std::vector<int>>> lists(G, std::vector<std::vector<int>>(nchunks));
+
+  // ---- rows -> groups of 8, for a given packing
+  auto make_order = [&](bool sparse) {
+    std::vector<int> order;   // virtual row -> actual row or -1
+    if (opt.triple) {
+      const int nu = M / 3;
+      std::vector<int> rho_order;
+      if (sparse) {
+        std::vector<std::vector<uint8_t>> s3(nu, std::vector<uint8_t>(K, 0));
+        for (int r = 0; r < nu; ++r)
+          for (int a = 0; a < 3; ++a)
+            for (int k = 0; k < K; ++k) s3[r][k] |= sup[a * nu + r][k];
+        rho_order = cluster_rows(s3, nu, K);
+      } else {
+        for (int r = 0; r < nu; ++r) rho_order.push_back(r);
+        while (rho_order.size() % 8) rho_order.push_back(-1);
+      }
+      // group 3g+a holds rows (a, rho_order[8g .. 8g+7])
+      for (size_t g = 0; g < rho_order.size() / 8; ++g)
+        for (int a = 0; a < 3; ++a)
+          for (int r = 0; r < 8; ++r) {
+            const int rho = rho_order[8 * g + r];
+            order.push_back(rho < 0 ? -1 : a * nu + rho);
+          }
+    } else if (sparse) {
+      order = cluster_rows(sup, M, K);
+    } else {
+      for (int m = 0; m < M; ++m) order.push_back(m);
+      while (order.size() % 8) order.push_back(-1);
+    }
+    return order;
+  };
+  if (opt.triple) FR_REQUIRE(M % 3 == 0, "triple packing needs M divisible by 3");
+  // per (group, chunk): the stage rows with a non-zero in the group
+  auto make_lists = [&](const std::vector<int> &order) {
+    const int G = (int)order.size() / 8;
+    std::vector<std::vector<std::vector<int>>> lists(G, std::vector<std::vector<int>>(nchunks));
+    for (int g = 0; g < G; ++g)
+      for (int c = 0; c < nchunks; ++c)
+        for (int kk = 0; kk < chunks[c].nrows; ++kk) {
+          bool any = false;
+          for (int r = 0; r < 8 && !any; ++r) {
+            const int m = order[8 * g + r];
+            if (m >= 0 && sup[m][chunk_k0[c] + kk]) any = true;
+          }
+          if (any) lists[g][c].push_back(kk);
+        }
+    return lists;
+  };
+  // ---- packing: k-lists when they save at least 15 % of the multiplies of the dense packing (a function of the operator alone)
+  bool sparse = false;
+  std::vector<int> order = make_order(false);
+  std::vector<std::vector<std::vector<int>>> lists;
+  if (opt.allow_sparse && density < 0.95) {
+    std::vector<int> so = make_order(true);
+    auto sl = make_lists(so);
+    double ds = 0, dd = 0;
+    for (auto &g : sl)
+      for (auto &l : g) ds += f64 ? (double)((l.size() + 3) / 4) : (double)l.size();
+    for (int c = 0; c < nchunks; ++c) dd += (f64 ? (double)dense_blocks_f64(chunks[c].nrows).size() : (double)chunks[c].nrows) * (order.size() / 8);
+    if (ds < 0.85 * dd) {
+      sparse = true;
+      order = so;
+      lists = sl;
+    }
+  }
+  const int G = (int)order.size() / 8;
+
+  // ---- geometry
+  const std::vector<PanelGeom> geoms = list_geoms<T>(G, opt.min_ne, opt.max_ne, opt.triple, !sparse);
+  if (opt.cand < 0 || opt.cand >= (int)geoms.size()) return false;
+  const PanelGeom geo = geoms[opt.cand];
+  const int WR = geo.WR, NIT = geo.NIT, NS = WR * NIT;
+  // cost of each group (blocks it executes) and LPT assignment of group units (1 or 3 groups) to row-warps
   std::vector<long long> gcost(G, 0);
   for (int g = 0; g < G; ++g)
     for (int c = 0; c < nchunks; ++c) {
-      for (int kk = 0; kk < (int)chunk_cols[c].size(); ++kk) {
-        bool any = !sparse;
-        for (int r = 0; r < 8 && !any; ++r) {
-          const int m = order[8 * g + r];
-          if (m >= 0 && sup[m][chunk_cols[c][kk]]) any = true;
-        }
-        if (any) lists[g][c].push_back(kk);
-      }
-      const int n = (int)lists[g][c].size();
+      const int n = sparse ? (int)lists[g][c].size() : chunks[c].nrows;
       gcost[g] += f64 ? (n + 3) / 4 * 4 : n;
     }
-  PanelGeom geo = choose_geom<T>(G, opt.min_ne, opt.max_ne, opt.triple, !sparse, opt.cand % 1000);
-  if (geo.eff < 0) return false;
-  const int WR = geo.WR, NIT = geo.NIT, NS = WR * NIT;
-  // LPT assignment of group units (1 or 3 groups) to row-warps, at most NIT groups per row-warp
   const int gu = opt.triple ? 3 : 1;
   const int GU = G / gu;
   std::vector<int> uorder(GU);
@@ -390,7 +428,7 @@ bool panel_op_build_kc(PanelOp<T> &p, int M, int K, const double *A, const std::
   // ---- pack
   std::vector<T> vals;
   std::vector<uint32_t> idx;
-  std::vector<int> off(nchunks * NS + 1, 0);
+  std::vector<int> off(sparse ? nchunks * NS + 1 : 1, 0);
   std::vector<int> rowmap(NS * 8, -1);
   for (int s = 0; s < NS; ++s)
     if (slot_group[s] >= 0)
@@ -398,96 +436,99 @@ bool panel_op_build_kc(PanelOp<T> &p, int M, int K, const double *A, const std::
         const int m = order[8 * slot_group[s] + r];
         rowmap[s * 8 + r] = (m >= 0 && opt.row_ids) ? opt.row_ids[m] : m;
       }
+  auto aval = [&](int m, int col) {
+    if (m < 0) return 0.0;
+    const double v = A[(size_t)m * K + col];
+    return std::fabs(v) > thr ? v : 0.0;
+  };
+  const uint32_t rs32 = (uint32_t)geo.NE * 4u;   // FP32: bytes between stage rows
   long long macs = 0;
   int nblk = 0;
   if (!sparse) {
-    // dense: blocks ordered (chunk, k-block, slot); rows of a block are the consecutive stage rows 4b..4b+3 (FP64) / row b (FP32)
+    // dense: blocks ordered (chunk, k-block, slot); the rows of a k-block come from the row table idx[block][4] (FP64)
     for (int c = 0; c < nchunks; ++c) {
       chunks[c].base = nblk / NS;
-      const int n = (int)chunk_cols[c].size();
-      const int nb = f64 ? (n + 3) / 4 : n;
-      for (int b = 0; b < nb; ++b)
-        for (int s = 0; s < NS; ++s) {
-          const int g = slot_group[s];
-          if (f64) {
+      if (f64) {
+        const auto blocks = dense_blocks_f64(chunks[c].nrows);
+        chunks[c].nblk = (int)blocks.size();
+        for (auto &b : blocks) {
+          for (int j = 0; j < 4; ++j) idx.push_back(swz_row_offset(j < (int)b.size() ? b[j] : b[0]));
+          for (int s = 0; s < NS; ++s) {
+            const int g = slot_group[s];
             for (int lane = 0; lane < 32; ++lane) {
               const int r = lane >> 2, j = lane & 3;
               const int m = g >= 0 ? order[8 * g + r] : -1;
-              vals.push_back((T)((m >= 0 && 4 * b + j < n) ? A[(size_t)m * K + chunk_cols[c][4 * b + j]] : 0.0));
+              vals.push_back((T)(j < (int)b.size() ? aval(m, chunk_k0[c] + b[j]) : 0.0));
             }
             if (g >= 0) macs += 32;
-          } else {
-            for (int r = 0; r < 8; ++r) {
-              const int m = g >= 0 ? order[8 * g + r] : -1;
-              vals.push_back((T)(m >= 0 ? A[(size_t)m * K + chunk_cols[c][b]] : 0.0));
-            }
-            if (g >= 0) macs += 8;
+            ++nblk;
           }
-          ++nblk;
-        }
-    }
-  }
-  for (int c = 0; c < nchunks && sparse; ++c)
-    for (int s = 0; s < NS; ++s) {
-      off[c * NS + s] = nblk;
-      const int g = slot_group[s];
-      if (g < 0) continue;
-      const std::vector<int> &L = lists[g][c];
-      const int n = (int)L.size();
-      if (f64) {
-        for (int b = 0; b < (n + 3) / 4; ++b) {
-          for (int j = 0; j < 4; ++j) {
-            const int kk = 4 * b + j < n ? L[4 * b + j] : 0;
-            idx.push_back((uint32_t)kk * (uint32_t)(PV * geo.NE + 4) * (uint32_t)sizeof(T));
-          }
-          for (int lane = 0; lane < 32; ++lane) {
-            const int r = lane >> 2, j = lane & 3;
-            const int m = order[8 * g + r];
-            double v = 0;
-            if (m >= 0 && 4 * b + j < n) v = A[(size_t)m * K + chunk_cols[c][L[4 * b + j]]];
-            if (sparse && std::fabs(v) <= thr) v = 0;
-            vals.push_back((T)v);
-          }
-          ++nblk;
-          macs += 32;
         }
       } else {
-        for (int b = 0; b < n; ++b) {
-          idx.push_back((uint32_t)L[b] * (uint32_t)(PV * geo.NE + 4) * (uint32_t)sizeof(T));
-          for (int r = 0; r < 8; ++r) {
-            const int m = order[8 * g + r];
-            double v = m >= 0 ? A[(size_t)m * K + chunk_cols[c][L[b]]] : 0.0;
-            if (sparse && std::fabs(v) <= thr) v = 0;
-            vals.push_back((T)v);
+        chunks[c].nblk = chunks[c].nrows;
+        for (int k = 0; k < chunks[c].nrows; ++k)
+          for (int s = 0; s < NS; ++s) {
+            const int g = slot_group[s];
+            for (int r = 0; r < 8; ++r) vals.push_back((T)aval(g >= 0 ? order[8 * g + r] : -1, chunk_k0[c] + k));
+            if (g >= 0) macs += 8;
+            ++nblk;
           }
-          ++nblk;
-          macs += 8;
-        }
       }
     }
-  if (sparse) off[nchunks * NS] = nblk;
-  // the multiply loop prefetches two blocks ahead: two all-zero blocks close the arrays (not counted in nblk)
+  } else {
+    for (int c = 0; c < nchunks; ++c)
+      for (int s = 0; s < NS; ++s) {
+        off[c * NS + s] = nblk;
+        const int g = slot_group[s];
+        if (g < 0) continue;
+        const std::vector<int> &L = lists[g][c];
+        if (f64) {
+          for (auto &b : sparse_blocks_f64(L)) {
+            for (int j = 0; j < 4; ++j) idx.push_back(swz_row_offset(j < (int)b.size() ? b[j] : b[0]));
+            for (int lane = 0; lane < 32; ++lane) {
+              const int r = lane >> 2, j = lane & 3;
+              vals.push_back((T)(j < (int)b.size() ? aval(order[8 * g + r], chunk_k0[c] + b[j]) : 0.0));
+            }
+            ++nblk;
+            macs += 32;
+          }
+        } else {
+          for (int kk : L) {
+            idx.push_back((uint32_t)kk * rs32);
+            for (int r = 0; r < 8; ++r) vals.push_back((T)aval(order[8 * g + r], chunk_k0[c] + kk));
+            ++nblk;
+            macs += 8;
+          }
+        }
+      }
+    off[nchunks * NS] = nblk;
+  }
+  // the sparse multiply loop prefetches two blocks ahead: two all-zero blocks close the arrays (not counted in nblk)
   for (int d = 0; d < 2; ++d) {
     for (int j = 0; j < (f64 ? 4 : 1); ++j) idx.push_back(0u);
     for (int j = 0; j < (f64 ? 32 : 8); ++j) vals.push_back(T(0));
   }
-  const size_t smem_op = ((vals.size() * sizeof(T) + 15) / 16 * 16) + ((idx.size() * 4 + 15) / 16 * 16) +
-                         ((off.size() * 4 + 15) / 16 * 16) + ((rowmap.size() * 4 + 15) / 16 * 16) +
-                         ((chunks.size() * sizeof(ChunkDesc) + 15) / 16 * 16);
-  if (geo.occ == 2) smem_total = smem_total / 2 - 2048;
-  if (smem_op > smem_budget || smem_op + 8192 > smem_total) return false;
-  size_t stage_elems = 0;
-  const int LDBh = PV * geo.NE + 4;
-  for (auto &c : chunks)
-    stage_elems = std::max(stage_elems, c.kind == KIND_FLUX ? flux_stage_elems(c.nrows, geo.NE, LDBh, opt.curved) : (size_t)c.nrows * LDBh);
-  if (smem_op + (size_t)geo.NG * PANEL_NSTAGE * stage_elems * sizeof(T) + 16 > smem_total) {
-    // MAC rows per chunk that would fit: scale the tallest chunk down proportionally (flux chunks carry 4/3 rows + metrics)
-    if (smem_total > smem_op + 4096) {
-      const double room = (double)(smem_total - smem_op - 1024) / ((double)PANEL_NSTAGE * geo.NG * sizeof(T));
-      *kc_fit = (int)(kcmax * room / (double)stage_elems);
-    }
-    return false;
-  }
+  // every array is copied to shared memory by one bulk copy: sizes are multiples of 16 bytes
+  auto pad16 = [](auto &v) {
+    using E = typename std::remove_reference<decltype(v[0])>::type;
+    while ((v.size() * sizeof(E)) % 16) v.push_back(E());
+  };
+  pad16(vals);
+  pad16(idx);
+  pad16(off);
+  pad16(rowmap);
+  const size_t smem_op = vals.size() * sizeof(T) + idx.size() * 4 + off.size() * 4 + rowmap.size() * 4 + chunks.size() * sizeof(ChunkDesc);
+  if (geo.occ == 2) smem_total = smem_total / 2 - 1024;
+  if (smem_op > smem_budget) return false;
+  size_t stage_bytes = 0;
+  for (auto &c : chunks) stage_bytes = std::max(stage_bytes, (size_t)PV * geo.NE * c.step * sizeof(T));
+  stage_bytes = (stage_bytes + 1023) / 1024 * 1024;
+  // 1 kB to align the ring, the ring, 256 B of mbarriers
+  const size_t fixed = 1024 + (smem_op + 1023) / 1024 * 1024 + 256;
+  if (fixed + 2 * geo.NG * stage_bytes > smem_total) return false;
+  int nstage = (int)((smem_total - fixed) / (geo.NG * stage_bytes));
+  nstage = std::min(nstage, PANEL_MAXSTAGE);
+  if (getenv("FRB_NSTAGE")) nstage = std::max(2, std::min(nstage, atoi(getenv("FRB_NSTAGE"))));
   panel_op_free(p);
   p.M = M;
   p.K = K;
@@ -498,27 +539,37 @@ bool panel_op_build_kc(PanelOp<T> &p, int M, int K, const double *A, const std::
   p.NE = geo.NE;
   p.NG = geo.NG;
   p.occ = geo.occ;
-  p.KC = kcmax;
-  p.stage_elems = (int)stage_elems;
-  p.curved = opt.curved;
   p.nchunks = nchunks;
   p.NS = NS;
+  p.nstage = nstage;
+  p.stage_bytes = (int)stage_bytes;
   p.nblk = nblk;
   p.nidx = (int)idx.size();
+  p.nsrc = (int)srcs.size();
+  for (int i = 0; i < p.nsrc; ++i) {
+    p.src_rows[i] = srcs[i].rows;
+    p.src_step[i] = src_step[i];
+  }
+#ifdef FRB_DEBUG_KNOBS
   p.dbg = getenv("FRB_PANEL_DBG") ? atoi(getenv("FRB_PANEL_DBG")) : 0;
   if (getenv("FRB_PANEL_VERBOSE"))
-    fprintf(stderr, "panel_op %s M=%d K=%d %s G=%d WR=%d WC=%d NIT=%d CX=%d NE=%d NG=%d occ=%d warps=%d KC=%d nchunks=%d nblk=%d smem_op=%zu stage=%zu B density=%.2f macs/col=%.0f (dense %d)\n",
-            f64 ? "f64" : "f32", M, K, sparse ? "sparse" : "dense", G, WR, geo.WC, NIT, geo.CX, geo.NE, geo.NG, geo.occ, geo.NG * WR * geo.WC, kcmax,
-            nchunks, nblk, smem_op, stage_elems * sizeof(T), density, (double)macs, M * K);
+    fprintf(stderr, "panel_op %s M=%d K=%d %s G=%d WR=%d WC=%d NIT=%d CX=%d NE=%d NG=%d occ=%d warps=%d+%d nchunks=%d nblk=%d smem_op=%zu stage=%zu x %d density=%.2f macs/col=%.0f (dense %d)\n",
+            f64 ? "f64" : "f32", M, K, sparse ? "sparse" : "dense", G, WR, geo.WC, NIT, geo.CX, geo.NE, geo.NG, geo.occ, geo.NG * WR * geo.WC, geo.NG,
+            nchunks, nblk, smem_op, stage_bytes, nstage, density, (double)macs, M * K);
+#endif
   p.sparse = sparse ? 1 : 0;
   p.macs_per_col = (double)macs;
   p.density = density;
   p.smem_op = smem_op;
+  p.bytes_vals = vals.size() * sizeof(T);
+  p.bytes_idx = idx.size() * 4;
+  p.bytes_off = off.size() * 4;
+  p.bytes_rowmap = rowmap.size() * 4;
+  p.bytes_chunks = chunks.size() * sizeof(ChunkDesc);
   auto up = [](auto *&dst, const auto &h) {
     using E = typename std::remove_reference<decltype(h[0])>::type;
-    const size_t nb = std::max<size_t>(h.size(), 1) * sizeof(E);
-    FR_CUDA_TRY(cudaMalloc((void **)&dst, nb));
-    if (!h.empty()) FR_CUDA_TRY(cudaMemcpy((void *)dst, h.data(), h.size() * sizeof(E), cudaMemcpyHostToDevice));
+    FR_CUDA_TRY(cudaMalloc((void **)&dst, h.size() * sizeof(E)));
+    FR_CUDA_TRY(cudaMemcpy((void *)dst, h.data(), h.size() * sizeof(E), cudaMemcpyHostToDevice));
   };
   up(p.vals, vals);
   up(p.idx, idx);
@@ -528,19 +579,15 @@ bool panel_op_build_kc(PanelOp<T> &p, int M, int K, const double *A, const std::
   return true;
 }
 
+template <typename T>
+inline size_t panel_smem_bytes(const PanelOp<T> &op) {
+  return 1024 + (op.smem_op + 1023) / 1024 * 1024 + (size_t)op.NG * op.nstage * op.stage_bytes + 256;
+}
+
 // ------------------------------------------------------------------------------------------------ device side
 #ifdef __CUDACC__
 
-__device__ __forceinline__ void pcp_async16(void *smem, const void *gmem, int src_bytes) {
-  unsigned s = (unsigned)__cvta_generic_to_shared(smem);
-  asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;\n" ::"r"(s), "l"(gmem), "r"(src_bytes));
-}
 __device__ __forceinline__ void prefetch_l2(const void *p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
-__device__ __forceinline__ void pcp_commit() { asm volatile("cp.async.commit_group;\n" ::); }
-template <int N>
-__device__ __forceinline__ void pcp_wait() {
-  asm volatile("cp.async.wait_group %0;\n" ::"n"(N));
-}
 
 __device__ __forceinline__ void dmma884(double &c0, double &c1, double a, double b) {
   asm("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};\n"
@@ -559,43 +606,21 @@ struct OpSmem {
 };
 
 template <typename T>
-__device__ __forceinline__ char *op_smem_carve(char *base, const PanelOp<T> &op, OpSmem<T> &v) {
-  auto al = [](size_t n) { return (n + 15) / 16 * 16; };
-  const size_t nv = (size_t)(op.nblk + 2) * (sizeof(T) == 8 ? 32 : 8) * sizeof(T);
+__device__ __forceinline__ void op_smem_carve(char *base, const PanelOp<T> &op, OpSmem<T> &v) {
   v.vals = reinterpret_cast<const T *>(base);
-  base += al(nv);
+  base += op.bytes_vals;
   v.idx = reinterpret_cast<const uint32_t *>(base);
-  base += al((size_t)op.nidx * 4);
+  base += op.bytes_idx;
   v.off = reinterpret_cast<const int *>(base);
-  base += al(((size_t)op.nchunks * op.NS + 1) * 4);
+  base += op.bytes_off;
   v.rowmap = reinterpret_cast<const int *>(base);
-  base += al((size_t)op.NS * 8 * 4);
+  base += op.bytes_rowmap;
   v.chunks = reinterpret_cast<const ChunkDesc *>(base);
-  base += al((size_t)op.nchunks * sizeof(ChunkDesc));
-  return base;
 }
 
-// Copy the operator image global -> shared with cp.async (all threads), one commit group.
-template <typename T>
-__device__ __forceinline__ void op_smem_load(char *base, const PanelOp<T> &op, int tid, int nthreads) {
-  auto al = [](size_t n) { return (n + 15) / 16 * 16; };
-  auto copy = [&](char *dst, const void *src, size_t nbytes) {
-    const int np = (int)(al(nbytes) / 16);
-    for (int p = tid; p < np; p += nthreads) {
-      const int rem = (int)nbytes - 16 * p;
-      pcp_async16(dst + 16 * p, reinterpret_cast<const char *>(src) + 16 * p, rem >= 16 ? 16 : rem);
-    }
-    return dst + al(nbytes);
-  };
-  char *b = base;
-  b = copy(b, op.vals, (size_t)(op.nblk + 2) * (sizeof(T) == 8 ? 32 : 8) * sizeof(T));
-  b = copy(b, op.idx, (size_t)op.nidx * 4);
-  b = copy(b, op.off, ((size_t)op.nchunks * op.NS + 1) * 4);
-  b = copy(b, op.rowmap, (size_t)op.NS * 8 * 4);
-  b = copy(b, op.chunks, (size_t)op.nchunks * sizeof(ChunkDesc));
-}
-
-// ---- accumulators and the multiply-accumulate core.  Panel columns in shared memory: c = v*NE + e, row pitch LDB.
+// ---- accumulators and the multiply-accumulate core.  A stage holds the chunk as planes (tma.cuh):
+//   FP64: plane(v, cb16) = v*(NE/16) + cb16, `pp` = step*128 bytes each, rows of 16 doubles, 128-byte swizzle;
+//   FP32: plane(v) of step rows of NE floats.
 template <typename T, int NIT, int CX>
 struct Acc;
 
@@ -611,16 +636,30 @@ struct Acc<double, NIT, CX> {
 #pragma unroll
         for (int v = 0; v < PV; ++v) c[i][b][v][0] = c[i][b][v][1] = 0.0;
   }
-  // elements of the panel this warp-column owns: [wc*8*CX, (wc+1)*8*CX)
-  __device__ __forceinline__ void mac_chunk(const OpSmem<double> &A, int chunk, int NS, int slot0, const double *Bst, int LDB,
+  // Per-lane constants of the B-fragment loads: lane = (column c = lane/4 of the 8-column block, k = lane%4).  Column block
+  // cbi = wc*CX + cb of the panel sits in 16-block cbi/2, half cbi%2: byte (half*4 + c/2)*16 + (c%2)*8 of the 128-byte line,
+  // XORed with the line's swizzle term, which the row offsets of idx carry in bits 4..6.
+  __device__ __forceinline__ static uint32_t lane_term(int cbi, int lane) {
+    const int c = lane >> 2;
+    return ((uint32_t)(((cbi & 1) << 2) | (c >> 1)) << 4) | ((uint32_t)(c & 1) << 3);
+  }
+  // Sparse operator: the warp's blocks of this chunk are contiguous across its NIT slots, so one software pipeline runs
+  // through all of them: operator value and row offset are fetched two blocks ahead, the B fragments one block ahead of the
+  // DMMAs that consume them.
+  __device__ __forceinline__ void mac_chunk(const OpSmem<double> &A, int chunk, const ChunkDesc &cd, int NS, int slot0, const char *stage,
                                             int NE, int wc, int lane) {
-    // 32-bit byte-offset arithmetic inside the shared window.  The warp's blocks of this chunk are contiguous across
-    // its NIT slots, so one software pipeline runs through all of them: operator value and row offset are fetched two
-    // blocks ahead, the B fragments one block ahead of the DMMAs that consume them.
-    const char *bcol = reinterpret_cast<const char *>(Bst + wc * 8 * CX + (lane >> 2));
+    const uint32_t pp = (uint32_t)cd.step * 128u;
+    const uint32_t vs = (uint32_t)(NE >> 4) * pp;
+    uint32_t lt[CX];
+    const char *pl[CX];
+#pragma unroll
+    for (int cb = 0; cb < CX; ++cb) {
+      const int cbi = wc * CX + cb;
+      lt[cb] = lane_term(cbi, lane);
+      pl[cb] = stage + (uint32_t)(cbi >> 1) * pp;
+    }
     const char *av = reinterpret_cast<const char *>(A.vals) + lane * 8;
     const char *ai = reinterpret_cast<const char *>(A.idx) + (lane & 3) * 4;
-    const uint32_t vs = (uint32_t)NE * 8u;
     const int *offp = A.off + chunk * NS + slot0;
     int b = offp[0];
     double a0 = *reinterpret_cast<const double *>(av + (uint32_t)b * 256u);
@@ -628,12 +667,12 @@ struct Acc<double, NIT, CX> {
     uint32_t ro1 = *reinterpret_cast<const uint32_t *>(ai + (uint32_t)b * 16u + 16u);
     double bf0[PV][CX];
     {
-      const char *bp = bcol + *reinterpret_cast<const uint32_t *>(ai + (uint32_t)b * 16u);
+      const uint32_t ro0 = *reinterpret_cast<const uint32_t *>(ai + (uint32_t)b * 16u);
 #pragma unroll
-      for (int v = 0; v < PV; ++v) {
+      for (int cb = 0; cb < CX; ++cb) {
+        const char *bp = pl[cb] + (ro0 ^ lt[cb]);
 #pragma unroll
-        for (int cb = 0; cb < CX; ++cb) bf0[v][cb] = *reinterpret_cast<const double *>(bp + cb * 64);
-        bp += vs;
+        for (int v = 0; v < PV; ++v) bf0[v][cb] = *reinterpret_cast<const double *>(bp + v * vs);
       }
     }
 #pragma unroll
@@ -642,12 +681,11 @@ struct Acc<double, NIT, CX> {
 #pragma unroll 2
       for (; b < bend; ++b) {
         double bf1[PV][CX];
-        const char *bp = bcol + ro1;
 #pragma unroll
-        for (int v = 0; v < PV; ++v) {
+        for (int cb = 0; cb < CX; ++cb) {
+          const char *bp = pl[cb] + (ro1 ^ lt[cb]);
 #pragma unroll
-          for (int cb = 0; cb < CX; ++cb) bf1[v][cb] = *reinterpret_cast<const double *>(bp + cb * 64);
-          bp += vs;
+          for (int v = 0; v < PV; ++v) bf1[v][cb] = *reinterpret_cast<const double *>(bp + v * vs);
         }
         const double a2 = *reinterpret_cast<const double *>(av + (uint32_t)b * 256u + 512u);
         const uint32_t ro2 = *reinterpret_cast<const uint32_t *>(ai + (uint32_t)b * 16u + 32u);
@@ -665,25 +703,33 @@ struct Acc<double, NIT, CX> {
       }
     }
   }
-  // Dense operator: the NIT row groups of the warp share the chunk's rows, so the B fragments of a k-block (stage rows
-  // 4b..4b+3) are loaded once and feed NIT x 5 x CX DMMAs; no index list.
-  __device__ __forceinline__ void mac_dense(const OpSmem<double> &A, const ChunkDesc &cd, int NS, int slot0, const double *Bst,
-                                            int LDB, int NE, int wc, int lane) {
-    const char *bcol = reinterpret_cast<const char *>(Bst + wc * 8 * CX + (lane >> 2));
+  // Dense operator: the NIT row groups of the warp share the chunk's k-blocks, so the B fragments of a k-block are loaded
+  // once and feed NIT x 5 x CX DMMAs; the block's four stage rows come from the row table.
+  __device__ __forceinline__ void mac_dense(const OpSmem<double> &A, const ChunkDesc &cd, int NS, int slot0, const char *stage, int NE,
+                                            int wc, int lane) {
+    const uint32_t pp = (uint32_t)cd.step * 128u;
+    const uint32_t vs = (uint32_t)(NE >> 4) * pp;
+    uint32_t lt[CX];
+    const char *pl[CX];
+#pragma unroll
+    for (int cb = 0; cb < CX; ++cb) {
+      const int cbi = wc * CX + cb;
+      lt[cb] = lane_term(cbi, lane);
+      pl[cb] = stage + (uint32_t)(cbi >> 1) * pp;
+    }
     const char *av = reinterpret_cast<const char *>(A.vals) + ((uint32_t)(cd.base * NS + slot0) * 32u + lane) * 8u;
-    const uint32_t vs = (uint32_t)NE * 8u, rs = (uint32_t)LDB * 8u, as = (uint32_t)NS * 256u;
-    const int nb = (cd.nrows + 3) >> 2, last = cd.nrows - 1;
-    const int kl = lane & 3;
+    const uint32_t *rt = A.idx + cd.base * 4 + (lane & 3);
+    const uint32_t as = (uint32_t)NS * 256u;
+    const int nb = cd.nblk;
 #pragma unroll 2
     for (int b = 0; b < nb; ++b) {
-      const int row = min(4 * b + kl, last);           // padded rows of the last block: operator is zero, data must be finite
-      const char *bp = bcol + (uint32_t)row * rs;
+      const uint32_t ro = rt[b * 4];
       double bf[PV][CX];
 #pragma unroll
-      for (int v = 0; v < PV; ++v) {
+      for (int cb = 0; cb < CX; ++cb) {
+        const char *bp = pl[cb] + (ro ^ lt[cb]);
 #pragma unroll
-        for (int cb = 0; cb < CX; ++cb) bf[v][cb] = *reinterpret_cast<const double *>(bp + cb * 64);
-        bp += vs;
+        for (int v = 0; v < PV; ++v) bf[v][cb] = *reinterpret_cast<const double *>(bp + v * vs);
       }
       const char *ap = av + (uint32_t)b * as;
 #pragma unroll
@@ -727,7 +773,7 @@ struct Acc<double, NIT, CX> {
 #pragma unroll
     for (int i = 0; i < NIT; ++i) g(i, 0, lane >> 2);
   }
-  static constexpr int EW = 2;   // consecutive elements per foreach2 call
+  static constexpr int EW = 2;   // consecutive elements per foreach_tile call
   static constexpr int ROWS = 1; // rows per thread per slot
   static constexpr int NSLOT = NIT;
 };
@@ -746,11 +792,11 @@ struct Acc<float, NIT, CX> {
 #pragma unroll
           for (int j = 0; j < CX; ++j) c[i][r][v][j] = 0.f;
   }
-  __device__ __forceinline__ void mac_chunk(const OpSmem<float> &A, int chunk, int NS, int slot0, const float *Bst, int LDB,
+  __device__ __forceinline__ void mac_chunk(const OpSmem<float> &A, int chunk, const ChunkDesc &cd, int NS, int slot0, const char *stage,
                                             int NE, int wc, int lane) {
-    const char *bcol = reinterpret_cast<const char *>(Bst + wc * 32 * CX + lane * CX);
+    const char *bcol = stage + (uint32_t)(wc * 32 * CX + lane * CX) * 4u;
     const char *avp = reinterpret_cast<const char *>(A.vals);
-    const uint32_t vs = (uint32_t)NE * 4u;
+    const uint32_t vs = (uint32_t)cd.step * (uint32_t)NE * 4u;
 #pragma unroll
     for (int i = 0; i < NIT; ++i) {
       const int b0 = A.off[chunk * NS + slot0 + i], b1 = A.off[chunk * NS + slot0 + i + 1];
@@ -782,11 +828,11 @@ struct Acc<float, NIT, CX> {
     }
   }
   // Dense operator: one B row feeds the NIT row groups of the warp.
-  __device__ __forceinline__ void mac_dense(const OpSmem<float> &A, const ChunkDesc &cd, int NS, int slot0, const float *Bst,
-                                            int LDB, int NE, int wc, int lane) {
-    const char *bp0 = reinterpret_cast<const char *>(Bst + wc * 32 * CX + lane * CX);
+  __device__ __forceinline__ void mac_dense(const OpSmem<float> &A, const ChunkDesc &cd, int NS, int slot0, const char *stage, int NE,
+                                            int wc, int lane) {
+    const char *bp0 = stage + (uint32_t)(wc * 32 * CX + lane * CX) * 4u;
     const char *ap0 = reinterpret_cast<const char *>(A.vals) + (uint32_t)(cd.base * NS + slot0) * 32u;
-    const uint32_t vs = (uint32_t)NE * 4u, rs = (uint32_t)LDB * 4u, as = (uint32_t)NS * 32u;
+    const uint32_t rs = (uint32_t)NE * 4u, vs = (uint32_t)cd.step * rs, as = (uint32_t)NS * 32u;
 #pragma unroll 2
     for (int k = 0; k < cd.nrows; ++k) {
       const char *bp = bp0 + (uint32_t)k * rs;

@@ -1,14 +1,13 @@
 // Fused panel kernels (fusion targets F-A and F-B of SURVEY 7.2):
-//   fused_grad: S3 + S4 + S6         G_i = (1/|J|) sum_alpha S[alpha][i] ( [M460 | M6] [U; C] )_alpha ;  F~ = S (f_inv(U) - f_visc(U,G))
+//   fused_grad: S3 + S4              G_i = (1/|J|) sum_alpha S[alpha][i] ( [M460 | M6] [U; C] )_alpha
 //               the three alpha components of a solution point sit in one thread (triple packing), so the transform to
-//               physical gradients and the transformed flux at that point are formed in registers in the epilogue;
+//               physical gradients is formed in registers in the epilogue;
 //   fused_div : S8 + S9 + S10        dudt = -(1/|J|) [ M132 | M3 ] [F~; D]  (+ Runge-Kutta stage update in the epilogue).
 // (A first version formed F~ inside fused_div from U, G and the metrics staged in shared memory; ncu showed the CTA waiting
 //  at barriers on a long, serial FP64 flux evaluation that only part of the threads could share, profiles/r01_*.md.)
 // Both run on the persistent panel main loop (panel_kernel.cuh) with the operator resident in shared memory.
 #include "kernels.cuh"
 #include "panel_kernel.cuh"
-#include "physics.cuh"
 
 namespace frb {
 
@@ -189,28 +188,25 @@ struct RkEpilogue {
 };
 
 template <typename T>
-struct DivArgs {
+struct alignas(64) DivArgs {
+  TmaProducer<T> prod;
   PanelOp<T> op;
-  PlainProducer<T> prod;
   RkEpilogue<T> epi;
   long long npanels;
 };
 
 template <typename T, int NIT, int CX>
 __global__ void __launch_bounds__(32 * panel_maxw<T>(NIT, CX)) k_fused_div(const __grid_constant__ DivArgs<T> a) {
-  extern __shared__ __align__(16) char panel_smem[];
+  extern __shared__ __align__(1024) char panel_smem[];
   panel_mainloop<T, NIT, CX>(a.op, a.prod, a.epi, a.npanels, 1, panel_smem);
 }
 
 // ------------------------------------------------------------------------------------------------ fused_grad
 // epilogue S4: physical gradient from the three reference components held by one thread
-template <typename T, bool FLUX>
+template <typename T>
 struct GradEpilogue {
   const T *smats, *rcpdjac;
-  T *grad;                  // [3][Nu][5][ld]  physical gradients G (read again by S5)
-  const T *u;               // stage input (for the flux)
-  T *ftil;                  // [3][Nu][5][ld]  transformed flux F~, or nullptr
-  PhysParams<T> ph;
+  T *grad;                  // [3][Nu][5][ld]  physical gradients G (read again by S5 and S6)
   long long ld, neles;
   int nupts, curved, NE;
   template <typename ACC>
@@ -247,70 +243,31 @@ struct GradEpilogue {
 #pragma unroll
       for (int j = 0; j < EW; ++j)
         if (col + j >= neles) rj[j] = T(0);      // padding lanes: zero
-      T uu[PV][EW];
-      if constexpr (FLUX) {
-#pragma unroll
-        for (int v = 0; v < PV; ++v) VecIO<T, EW>::ld(u + ((long long)rho * 5 + v) * ld + col, uu[v]);
-      }
-      T q[3][PV][EW];
 #pragma unroll
       for (int i = 0; i < 3; ++i)
 #pragma unroll
         for (int v = 0; v < PV; ++v) {
+          T q[EW];
 #pragma unroll
-          for (int j = 0; j < EW; ++j) q[i][v][j] = rj[j] * (S[0][i][j] * t0[v][j] + S[1][i][j] * t1[v][j] + S[2][i][j] * t2[v][j]);
-          VecIO<T, EW>::st(grad + (((long long)i * nupts + rho) * 5 + v) * ld + col, q[i][v]);
+          for (int j = 0; j < EW; ++j) q[j] = rj[j] * (S[0][i][j] * t0[v][j] + S[1][i][j] * t1[v][j] + S[2][i][j] * t2[v][j]);
+          VecIO<T, EW>::st(grad + (((long long)i * nupts + rho) * 5 + v) * ld + col, q);
         }
-      if constexpr (FLUX) {
-      // S6 at this solution point: F~_alpha = sum_i S[alpha][i] (f^inv_i(U) - f^visc_i(U, G))
-      T ft[3][PV][EW];
-#pragma unroll
-      for (int j = 0; j < EW; ++j) {
-        const bool live = col + j < neles;
-        T u1[5], q1[3][5], f[3][5], rr, vel[3], pr;
-#pragma unroll
-        for (int v = 0; v < 5; ++v) u1[v] = live ? uu[v][j] : T(1);
-#pragma unroll
-        for (int i = 0; i < 3; ++i)
-#pragma unroll
-          for (int v = 0; v < 5; ++v) q1[i][v] = q[i][v][j];
-        inviscid_flux(u1, ph.gamma, f, rr, vel, pr);
-        subtract_viscous_flux(u1, q1, rr, vel, ph.gamma, ph.mu, ph.prandtl, f);
-#pragma unroll
-        for (int a = 0; a < 3; ++a)
-#pragma unroll
-          for (int v = 0; v < 5; ++v)
-            ft[a][v][j] = live ? S[a][0][j] * f[0][v] + S[a][1][j] * f[1][v] + S[a][2][j] * f[2][v] : T(0);
-      }
-#pragma unroll
-      for (int a = 0; a < 3; ++a)
-#pragma unroll
-        for (int v = 0; v < PV; ++v) VecIO<T, EW>::st(ftil + (((long long)a * nupts + rho) * 5 + v) * ld + col, ft[a][v]);
-      }
     });
   }
 };
 
 template <typename T>
-struct GradArgs {
+struct alignas(64) GradArgs {
+  TmaProducer<T> prod;
   PanelOp<T> op;
-  PlainProducer<T> prod;
-  GradEpilogue<T, false> epi;   // FLUX = true (S6 in the epilogue) is parity-tested but slower, see api.cu kFuseFluxIntoGrad
+  GradEpilogue<T> epi;
   long long npanels;
 };
 
 template <typename T, int NIT, int CX>
 __global__ void __launch_bounds__(32 * panel_maxw<T>(NIT, CX)) k_fused_grad(const __grid_constant__ GradArgs<T> a) {
-  extern __shared__ __align__(16) char panel_smem[];
+  extern __shared__ __align__(1024) char panel_smem[];
   panel_mainloop<T, NIT, CX>(a.op, a.prod, a.epi, a.npanels, 1, panel_smem);
-}
-
-template <typename K, typename A>
-void launch_panel(K k, const A &a, int nthreads, size_t smem, long long ntot, int ng, int occ, cudaStream_t s) {
-  FR_CUDA_TRY(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-  const long long grid = std::min<long long>((ntot + ng - 1) / ng, (long long)device_sm_count() * occ);
-  k<<<(unsigned)grid, nthreads, smem, s>>>(a);
-  FR_CUDA_TRY(cudaGetLastError());
 }
 
 }  // namespace
@@ -331,9 +288,9 @@ bool fused_div_build(PanelOp<T> &op, int nu, int nf, const double *M132, const d
     for (int k = 0; k < 3 * nu; ++k) A[(size_t)j * K + k] = M132[(size_t)m * 3 * nu + k];
     for (int k = 0; k < nf; ++k) A[(size_t)j * K + 3 * nu + k] = M3[(size_t)m * nf + k];
   }
-  std::vector<KSource> srcs{KSource{3 * nu, KIND_PLAIN, 1}, KSource{nf, KIND_PLAIN, 1}};
+  std::vector<KSource> srcs{KSource{3 * nu}, KSource{nf}};
   PackOptions opt;
-  opt.min_ne = 16;
+  opt.min_ne = sizeof(T) == 8 ? 16 : 32;
   opt.max_ne = sizeof(T) == 8 ? 64 : 128;
   opt.cand = cand;
   opt.row_ids = ids.data();
@@ -345,17 +302,15 @@ int launch_fused_div(const PanelOp<T> &op, const EleView<T> &ev, const T *ftil, 
                      cudaStream_t s) {
   DivArgs<T> a;
   a.op = op;
-  a.prod = PlainProducer<T>();
-  a.prod.src[0] = MatRef<T>{ftil, 5 * ev.ld, 0};
-  a.prod.src[1] = MatRef<T>{d, 5 * ev.ld, 0};
-  a.prod.cm = ColMap{op.NE, ev.ld, 0, ev.ld};
+  a.op.pf_epi = 1;
+  a.prod.tm[0] = tmap_state(ftil, 3ll * ev.nupts, ev.ld, op.NE, op.src_step[0]);
+  a.prod.tm[1] = tmap_state(d, (long long)ev.nfpts, ev.ld, op.NE, op.src_step[1]);
+  a.prod.plain = 0;
   a.epi = RkEpilogue<T>{ev.rcpdjac, ev.ld, ev.neles, ev.affine ? 0 : 1, op.NE, sa};
   a.npanels = ev.ld / op.NE;
-  const size_t smem = panel_smem_bytes(op);
-  const int nthreads = 32 * op.WR * op.WC * op.NG;
 #define FR_CASE(NIT_, CX_)                                                          \
   if (op.NIT == NIT_ && op.CX == CX_) {                                             \
-    launch_panel(k_fused_div<T, NIT_, CX_>, a, nthreads, smem, a.npanels, op.NG, op.occ, s);       \
+    panel_launch(k_fused_div<T, NIT_, CX_>, a, op, a.npanels, s);                   \
     return 1;                                                                       \
   }
   if constexpr (sizeof(T) == 8) {
@@ -392,9 +347,9 @@ bool fused_grad_build(PanelOp<T> &op, int nu, int nf, const double *M460, const 
           A[(size_t)ml * K + k] += acc;
         }
     }
-  std::vector<KSource> srcs{KSource{nu, KIND_PLAIN, 1}, KSource{nf, KIND_PLAIN, 1}};
+  std::vector<KSource> srcs{KSource{nu}, KSource{nf}};
   PackOptions opt;
-  opt.min_ne = 16;
+  opt.min_ne = sizeof(T) == 8 ? 16 : 32;
   opt.max_ne = sizeof(T) == 8 ? 64 : 128;
   opt.triple = 1;
   opt.cand = cand;
@@ -403,27 +358,20 @@ bool fused_grad_build(PanelOp<T> &op, int nu, int nf, const double *M460, const 
 }
 
 template <typename T>
-int launch_fused_grad(const PanelOp<T> &op, const EleView<T> &ev, const T *u, const T *c, T *grad, T *ftil,
-                      const PhysParams<T> &ph, cudaStream_t s) {
+int launch_fused_grad(const PanelOp<T> &op, const EleView<T> &ev, const T *u, const T *c, T *grad, cudaStream_t s) {
   GradArgs<T> a;
   a.op = op;
-  // The L2 prefetch of the epilogue's metric terms pays only in FP64 with per-element terms (tet S3+S4 1.54 -> 1.46 ms); with
-  // per-point terms (20 lines per thread) and in FP32 it costs more issue slots than the latency it hides (pri S3+S4 FP64
-  // 1.07 -> 1.00 ms without, tet S3+S4 FP32 1.27 -> 1.18 ms; profiles/r01_j_panel_source_level.md item 7).  Bit 2 of dbg makes
-  // panel_mainloop skip it -- decided here so that the kernels' code is untouched (an in-kernel test cost FP64 tets 12 %).
-  if (!ev.affine || sizeof(T) == 4) a.op.dbg |= 4;
-  ColMap cm{op.NE, ev.ld, 0, ev.ld};
-  a.prod = PlainProducer<T>();
-  a.prod.src[0] = MatRef<T>{u, 5 * ev.ld, 0};
-  a.prod.src[1] = MatRef<T>{c, 5 * ev.ld, 0};
-  a.prod.cm = cm;
-  a.epi = GradEpilogue<T, false>{ev.smats, ev.rcpdjac, grad, u, ftil, ph, ev.ld, ev.neles, ev.nupts, ev.affine ? 0 : 1, op.NE};
+  // The L2 prefetch of the epilogue's metric terms pays only in FP64 with per-element terms; with per-point terms (20 lines per
+  // thread) and in FP32 it costs more issue slots than the latency it hides (profiles/r01_j_panel_source_level.md item 7).
+  a.op.pf_epi = (ev.affine && sizeof(T) == 8) ? 1 : 0;
+  a.prod.tm[0] = tmap_state(u, (long long)ev.nupts, ev.ld, op.NE, op.src_step[0]);
+  a.prod.tm[1] = tmap_state(c, (long long)ev.nfpts, ev.ld, op.NE, op.src_step[1]);
+  a.prod.plain = 0;
+  a.epi = GradEpilogue<T>{ev.smats, ev.rcpdjac, grad, ev.ld, ev.neles, ev.nupts, ev.affine ? 0 : 1, op.NE};
   a.npanels = ev.ld / op.NE;
-  const size_t smem = panel_smem_bytes(op);
-  const int nthreads = 32 * op.WR * op.WC * op.NG;
 #define FR_CASE(NIT_, CX_)                                                          \
   if (op.NIT == NIT_ && op.CX == CX_) {                                             \
-    launch_panel(k_fused_grad<T, NIT_, CX_>, a, nthreads, smem, a.npanels, op.NG, op.occ, s);      \
+    panel_launch(k_fused_grad<T, NIT_, CX_>, a, op, a.npanels, s);                  \
     return 1;                                                                       \
   }
   if constexpr (sizeof(T) == 8) {
@@ -440,8 +388,7 @@ int launch_fused_grad(const PanelOp<T> &op, const EleView<T> &ev, const T *u, co
   template int launch_fused_div<T>(const PanelOp<T> &, const EleView<T> &, const T *, const T *, const StageArgs<T> &,     \
                                    cudaStream_t);                                                                          \
   template bool fused_grad_build<T>(PanelOp<T> &, int, int, const double *, const double *, int, const double *, int, int);                             \
-  template int launch_fused_grad<T>(const PanelOp<T> &, const EleView<T> &, const T *, const T *, T *, T *,                \
-                                    const PhysParams<T> &, cudaStream_t);
+  template int launch_fused_grad<T>(const PanelOp<T> &, const EleView<T> &, const T *, const T *, T *, cudaStream_t);
 FR_INST(double)
 FR_INST(float)
 

@@ -1,9 +1,17 @@
-// The persistent panel main loop shared by the plain operator product and its fused variants (see panel.cuh).
+// The persistent, warp-specialised panel main loop shared by the plain operator product and its fused variants (panel.cuh).
+//
+// Warps of a CTA:  [group 0 consumers | group 1 consumers | ... | one producer warp per group].
+//   producer (one elected lane): for every (panel, chunk) of its group, wait until the ring stage is empty, arm the stage's
+//     full barrier with the byte count and issue the tiled copy/copies (cp.async.bulk.tensor) that fill it;
+//   consumers: wait on the full barrier, multiply the chunk into their register accumulators, release the stage (one arrive
+//     per warp on the empty barrier), and after the panel's last chunk run the epilogue on their own rows and columns.
+// No warp ever waits for another consumer warp: a warp in its (latency-bound) epilogue leaves the tensor pipe to the warps that
+// are already multiplying the next panel, as far ahead as the ring is deep.
 #pragma once
 #include "panel.cuh"
+#include "tma.cuh"
 
 namespace frb {
-
 
 // Where a panel's columns live in a global matrix: column(v, e) = p*pstride + v*vstride + e, valid iff
 // p*pstride + v*vlim + e < lim.  State matrices [rows][5][ld]: pstride = NE, vstride = ld, vlim = 0, lim = ld.
@@ -12,68 +20,30 @@ struct ColMap {
   long long pstride, vstride, vlim, lim;
 };
 
+// ---- producer: B chunks are rows of up to two stacked global matrices, described by tensor maps (tma.cuh)
 template <typename T>
-struct MatRef {
-  const T *p;
-  long long ld, bstride;   // row stride, batch stride (elements)
-};
-
-// ---- producer: B chunks are plain rows of up to two stacked global matrices
-template <typename T>
-struct PlainProducer {
-  MatRef<T> src[2];
-  ColMap cm;
-  static constexpr bool kTransform = false;
-  // per-thread copy lane, fixed for the life of the CTA (init): each thread owns one 16-byte column piece (variable v,
-  // elements e..e+CTV) and walks down the rows, so a piece costs two pointer bumps and the copy
-  int l_sub, l_rpi, l_v, l_e, l_wide;
-  __device__ __forceinline__ void init(int NE, int tid, int nthreads) {
-    constexpr int CTV = 16 / (int)sizeof(T);
-    const int lg = 31 - __clz(NE / CTV);
-    const int ppr = PV << lg;                         // pieces per row
-    l_wide = nthreads >= ppr;                         // the usual case: one sweep of the group covers >= 1 whole row
-    l_rpi = l_wide ? nthreads / ppr : 1;              // rows per sweep
-    l_sub = l_wide ? tid / ppr : 0;
-    const int col = tid - l_sub * ppr;
-    l_v = col >> lg;
-    l_e = (col - (l_v << lg)) * CTV;
-  }
-  __device__ __forceinline__ void issue_col(const ChunkDesc &cd, long long batch, long long pl, T *stage, int LDB, int NE, int v,
-                                            int e) const {
-    constexpr int CTV = 16 / (int)sizeof(T);
-    long long nv = cm.lim - pl * cm.pstride - v * cm.vlim - e;
-    nv = nv < 0 ? 0 : (nv > CTV ? CTV : nv);
-    const int nbytes = (int)nv * (int)sizeof(T);
-    const T *mp = cd.src ? src[1].p : src[0].p;
-    const long long mld = cd.src ? src[1].ld : src[0].ld, mbs = cd.src ? src[1].bstride : src[0].bstride;
-    const T *g = mp;
-    long long gstep = 0;
-    if (nv > 0) {
-      g = mp + batch * mbs + (long long)(cd.row0 + l_sub) * mld + pl * cm.pstride + v * cm.vstride + e;
-      gstep = (long long)l_rpi * mld;
-    }
-    T *sp = stage + l_sub * LDB + v * NE + e;
-    const int sstep = l_rpi * LDB;
-    for (int r = l_sub; r < cd.nrows; r += l_rpi) {
-      pcp_async16(sp, g, nbytes);
-      g += gstep;
-      sp += sstep;
+struct alignas(64) TmaProducer {
+  CUtensorMap tm[PANEL_MAXSRC];
+  int plain;   // 1: plain matrix [K][N] (one copy per column block); 0: state matrix [rows][5][ld] (one copy per chunk)
+  int pad[15];
+  // called by one lane; `this` must be the kernel's __grid_constant__ parameter (the TMA unit reads the map through its address)
+  __device__ __forceinline__ void issue(const ChunkDesc &cd, long long batch, long long pl, uint32_t dst, uint32_t bar, int NE) const {
+    const CUtensorMap *m = &tm[cd.src];
+    if (!plain) {
+      if (sizeof(T) == 8) tma_load_4d(dst, m, 0, cd.row0, (int)(pl * (NE >> 4)), 0, bar);
+      else tma_load_3d(dst, m, (int)(pl * NE), cd.row0, 0, bar);
+    } else if (sizeof(T) == 8) {
+      const int nb = PV * (NE >> 4);
+      const uint32_t pp = (uint32_t)cd.step * 128u;
+      const int col0 = (int)(pl * PV * NE);
+      for (int j = 0; j < nb; ++j) tma_load_3d(dst + j * pp, m, col0 + j * 16, cd.row0, (int)batch, bar);
+    } else {
+      const uint32_t pp = (uint32_t)cd.step * (uint32_t)NE * 4u;
+      const int col0 = (int)(pl * PV * NE);
+#pragma unroll
+      for (int v = 0; v < PV; ++v) tma_load_3d(dst + v * pp, m, col0 + v * NE, cd.row0, (int)batch, bar);
     }
   }
-  __device__ __forceinline__ void issue(const ChunkDesc &cd, long long batch, long long pl, T *stage, int LDB, int NE, int tid,
-                                        int nthreads) const {
-    if (l_wide) {
-      if (l_sub < l_rpi) issue_col(cd, batch, pl, stage, LDB, NE, l_v, l_e);
-      return;
-    }
-    constexpr int CTV = 16 / (int)sizeof(T);
-    const int lg = 31 - __clz(NE / CTV);
-    for (int col = tid; col < (PV << lg); col += nthreads) {
-      const int v = col >> lg;
-      issue_col(cd, batch, pl, stage, LDB, NE, v, (col - (v << lg)) * CTV);
-    }
-  }
-  __device__ __forceinline__ void transform(const ChunkDesc &, long long, long long, T *, int, int, int, int) const {}
 };
 
 // ---- epilogue: C <- c1*acc + c2*C
@@ -135,96 +105,127 @@ struct PlainEpilogue {
   }
 };
 
-// ---- the persistent main loop.  Grid = any number of CTAs; CTA b owns panels b, b+grid, ...
+// ---- the persistent main loop.  Grid = any number of CTAs; CTA b, group g owns panels b*NG+g, b*NG+g + grid*NG, ...
+// `prod` must refer to the kernel's __grid_constant__ parameter.
 template <typename T, int NIT, int CX, class Prod, class Epi>
-__device__ __forceinline__ void panel_mainloop(const PanelOp<T> &op, const Prod &prod_in, const Epi &epi, long long npanels_per_batch,
-                                               int nbatch, char *smem) {
-  // A CTA holds NG (1 or 2) independent warp groups.  Each group owns its own accumulators, its own cp.async ring and its own
-  // stream of panels; they share only the operator image.  Group 1 starts half a panel late, so that one group's epilogue
-  // (global loads and stores, latency-bound) and chunk waits run under the other group's multiplies.
+__device__ __forceinline__ void panel_mainloop(const PanelOp<T> &op, const Prod &prod, const Epi &epi, long long npanels_per_batch,
+                                               int nbatch, char *smem_raw) {
   const int WC = op.WC, NS = op.NS, NE = op.NE, NG = op.NG;
-  const int nthreads = 32 * op.WR * WC;              // threads of one group
-  const int grp = threadIdx.x / nthreads;
-  const int tid = threadIdx.x - grp * nthreads, lane = tid & 31, warp = tid >> 5;
-  Prod prod(prod_in);
-  prod.init(NE, tid, nthreads);
-  const int wr = warp / WC, wc = warp - wr * WC;
-  const int LDB = PV * NE + 4;
+  const int nwc = op.WR * WC;                          // consumer warps of one group
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const bool producer = warp >= nwc * NG;
+  const int grp = producer ? warp - nwc * NG : warp / nwc;
+  const int nstage = op.nstage;
+  // ---- carve shared memory: operator image | ring (1024-byte aligned: the swizzle is a function of the address) | barriers
+  const uint32_t s0 = smem_u32(smem_raw);
+  const uint32_t ring0 = (s0 + (uint32_t)op.smem_op + 1023u) & ~1023u;
+  char *ringp = smem_raw + (ring0 - s0);
+  const uint32_t stage_bytes = (uint32_t)op.stage_bytes;
+  const uint32_t bars = ring0 + (uint32_t)(NG * nstage) * stage_bytes;
+  // barriers: full[g][s] at bars + (g*nstage + s)*16, empty[g][s] 8 bytes later; the image barrier closes the list
+  const uint32_t bar_img = bars + (uint32_t)(NG * nstage) * 16u;
+  if (threadIdx.x == 0) {
+    for (int i = 0; i < NG * nstage; ++i) {
+      mbar_init(bars + i * 16, 1);
+      mbar_init(bars + i * 16 + 8, (uint32_t)nwc);
+    }
+    mbar_init(bar_img, 1);
+    mbar_fence_init();
+  }
+  __syncthreads();
   OpSmem<T> A;
-  char *ringp = op_smem_carve(smem, op, A);
-  op_smem_load(smem, op, threadIdx.x, blockDim.x);
-  pcp_commit();
-  const size_t stage_elems = (size_t)op.stage_elems;
-  T *ring = reinterpret_cast<T *>(ringp) + (size_t)grp * PANEL_NSTAGE * stage_elems;
+  op_smem_carve(smem_raw, op, A);
   const long long ntot = npanels_per_batch * nbatch;
   const long long first = (long long)blockIdx.x * NG + grp, stride = (long long)gridDim.x * NG;
   const long long mine = first < ntot ? (ntot - first + stride - 1) / stride : 0;
   const int nchunks = op.nchunks;
   const long long total = mine * nchunks;
-  auto group_barrier = [&]() {
-    if (NG == 1) __syncthreads();
-    else asm volatile("bar.sync %0, %1;" ::"r"(1 + grp), "r"(nthreads) : "memory");
-  };
-  // two cursors over (panel, chunk): one for the loads being issued, one for the chunk being multiplied
-  long long ipl = first, cpl = first;
-  int ic = 0, cc = 0, istage = 0, cstage = 0;
-  long long ibatch = ipl / npanels_per_batch;
-  ipl -= ibatch * npanels_per_batch;
-  long long cbatch = ibatch;
-  cpl = ipl;
-  bool image_ready = false;                          // the shared operator image (with the chunk table) has landed
-  auto issue = [&]() {
-    // chunk table: from shared memory once it is there -- a global read here sits on the critical path of every chunk
-    const ChunkDesc cd = image_ready ? A.chunks[ic] : op.chunks[ic];
-    prod.issue(cd, ibatch, ipl, ring + istage * stage_elems, LDB, NE, tid, nthreads);
-    if (++istage == PANEL_NSTAGE) istage = 0;
-    if (++ic == nchunks) {
-      ic = 0;
-      ipl += stride;
-      while (ipl >= npanels_per_batch) {
-        ipl -= npanels_per_batch;
-        ++ibatch;
+  const uint32_t gbar = bars + (uint32_t)(grp * nstage) * 16u;
+  const uint32_t gring = ring0 + (uint32_t)(grp * nstage) * stage_bytes;
+
+  if (producer) {
+    if (lane != 0) return;
+    if (grp == 0) {
+      // the operator image: five bulk copies counted on one barrier
+      mbar_expect_tx(bar_img, (uint32_t)op.smem_op);
+      uint32_t d = s0;
+      bulk_load(d, op.vals, (uint32_t)op.bytes_vals, bar_img);
+      d += (uint32_t)op.bytes_vals;
+      bulk_load(d, op.idx, (uint32_t)op.bytes_idx, bar_img);
+      d += (uint32_t)op.bytes_idx;
+      bulk_load(d, op.off, (uint32_t)op.bytes_off, bar_img);
+      d += (uint32_t)op.bytes_off;
+      bulk_load(d, op.rowmap, (uint32_t)op.bytes_rowmap, bar_img);
+      d += (uint32_t)op.bytes_rowmap;
+      bulk_load(d, op.chunks, (uint32_t)op.bytes_chunks, bar_img);
+    }
+    long long pl = first, batch = pl / npanels_per_batch;
+    pl -= batch * npanels_per_batch;
+    int stage = 0;
+    uint32_t phase = 0;
+    for (long long p = 0; p < mine; ++p) {
+      for (int c = 0; c < nchunks; ++c) {
+        const ChunkDesc cd = op.chunks[c];               // global (L1-resident); the image may not have landed yet
+        mbar_wait(gbar + stage * 16 + 8, phase ^ 1u);    // stage is empty
+        const uint32_t full = gbar + stage * 16;
+        mbar_expect_tx(full, (uint32_t)(PV * NE * (int)sizeof(T)) * (uint32_t)cd.step);
+        prod.issue(cd, batch, pl, gring + stage * stage_bytes, full, NE);
+        if (++stage == nstage) {
+          stage = 0;
+          phase ^= 1u;
+        }
+      }
+      pl += stride;
+      while (pl >= npanels_per_batch) {
+        pl -= npanels_per_batch;
+        ++batch;
       }
     }
-  };
-  for (int q = 0; q < PANEL_NSTAGE - 1; ++q) {
-    if (q < total) issue();
-    pcp_commit();
+    return;
   }
-  // the operator image was copied by all threads of the CTA: everyone's share must have landed before anyone reads it
-  pcp_wait<PANEL_NSTAGE - 1>();
-  __syncthreads();
-  image_ready = true;
+
+  // ---- consumers
+  const int tid = threadIdx.x - grp * nwc * 32;
+  const int cw = tid >> 5;                             // warp within the group
+  const int wr = cw / WC, wc = cw - wr * WC;
+  mbar_wait(bar_img, 0);
+  long long cpl = first, cbatch = cpl / npanels_per_batch;
+  cpl -= cbatch * npanels_per_batch;
+  // Group 1 starts half a panel late, so that one group's epilogue (global loads and stores, latency-bound) runs under the
+  // other group's multiplies.
   const long long stagger_q = total > 0 ? (nchunks / 2 < total ? nchunks / 2 : total - 1) : -1;
   if (NG == 2) {
-    if (grp == 1) asm volatile("bar.sync 3, %0;" ::"r"(2 * nthreads) : "memory");
-    else if (stagger_q < 0) asm volatile("bar.arrive 3, %0;" ::"r"(2 * nthreads) : "memory");
+    if (grp == 1) asm volatile("bar.sync 3, %0;" ::"r"(2 * nwc * 32) : "memory");
+    else if (stagger_q < 0) asm volatile("bar.arrive 3, %0;" ::"r"(2 * nwc * 32) : "memory");
   }
   Acc<T, NIT, CX> acc;
   acc.zero();
+  int stage = 0, cc = 0;
+  uint32_t phase = 0;
   for (long long q = 0; q < total; ++q) {
-    pcp_wait<PANEL_NSTAGE - 2>();
-    group_barrier();
-    if (q + PANEL_NSTAGE - 1 < total) issue();
-    pcp_commit();
-    T *stage = ring + cstage * stage_elems;
-    if (Prod::kTransform) {
-      const ChunkDesc cd = A.chunks[cc];
-      if (cd.kind != KIND_PLAIN) {                   // uniform over the group
-        prod.transform(cd, cbatch, cpl, stage, LDB, NE, tid, nthreads);
-        group_barrier();
-      }
-    }
+    mbar_wait(gbar + stage * 16, phase);
+    const char *st = ringp + (size_t)(grp * nstage + stage) * stage_bytes;
     // the epilogue's own global operands: pull them into L2 while the last chunk is multiplied
-    if (cc == nchunks - 1 && !(op.dbg & 4)) epi.prefetch(acc, A.rowmap, wr * NIT, cbatch, cpl, wc, lane);
-    if (!(op.dbg & 1)) {
-      if (op.sparse) acc.mac_chunk(A, cc, NS, wr * NIT, stage, LDB, NE, wc, lane);
-      else acc.mac_dense(A, A.chunks[cc], NS, wr * NIT, stage, LDB, NE, wc, lane);
+    if (cc == nchunks - 1 && op.pf_epi) epi.prefetch(acc, A.rowmap, wr * NIT, cbatch, cpl, wc, lane);
+#ifdef FRB_DEBUG_KNOBS
+    if (!(op.dbg & 1))
+#endif
+    {
+      if (op.sparse) acc.mac_chunk(A, cc, A.chunks[cc], NS, wr * NIT, st, NE, wc, lane);
+      else acc.mac_dense(A, A.chunks[cc], NS, wr * NIT, st, NE, wc, lane);
     }
-    if (NG == 2 && grp == 0 && q == stagger_q) asm volatile("bar.arrive 3, %0;" ::"r"(2 * nthreads) : "memory");
-    if (++cstage == PANEL_NSTAGE) cstage = 0;
+    __syncwarp();
+    if (lane == 0) mbar_arrive(gbar + stage * 16 + 8);
+    if (NG == 2 && grp == 0 && q == stagger_q) asm volatile("bar.arrive 3, %0;" ::"r"(2 * nwc * 32) : "memory");
+    if (++stage == nstage) {
+      stage = 0;
+      phase ^= 1u;
+    }
     if (++cc == nchunks) {
-      if (!(op.dbg & 2)) epi(acc, A.rowmap, wr * NIT, cbatch, cpl, wc, lane);
+#ifdef FRB_DEBUG_KNOBS
+      if (!(op.dbg & 2))
+#endif
+      epi(acc, A.rowmap, wr * NIT, cbatch, cpl, wc, lane);
       acc.zero();
       cc = 0;
       cpl += stride;
@@ -234,7 +235,6 @@ __device__ __forceinline__ void panel_mainloop(const PanelOp<T> &op, const Prod 
       }
     }
   }
-  pcp_wait<0>();
 }
 
 // Dispatch over the compile-time accumulator shapes.  FP64: NIT*CX <= 8; FP32: NIT*CX <= 4.
@@ -245,9 +245,17 @@ __device__ __forceinline__ void panel_mainloop(const PanelOp<T> &op, const Prod 
 #define FR_PANEL_TRIPLES_F64(X) X(3, 1) X(6, 1) X(3, 2)
 #define FR_PANEL_TRIPLES_F32(X) X(3, 1)
 
-template <typename T>
-inline size_t panel_smem_bytes(const PanelOp<T> &op) {
-  return op.smem_op + (size_t)op.NG * PANEL_NSTAGE * op.stage_elems * sizeof(T) + 16;
+// grid: one CTA per SM and CTA slot, never more than there are panel sets.  The opt-in to > 48 kB of dynamic shared memory is a
+// per-device function attribute; setting it on every launch keeps the launchers free of process-wide state (it is not a stream
+// operation, so it is legal under capture).
+template <typename T, typename K, typename A>
+inline void panel_launch(K k, const A &a, const PanelOp<T> &op, long long ntot, cudaStream_t s) {
+  const size_t smem = panel_smem_bytes(op);
+  FR_CUDA_TRY(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+  const int nthreads = 32 * (op.WR * op.WC * op.NG + op.NG);
+  const long long grid = std::min<long long>((ntot + op.NG - 1) / op.NG, (long long)device_sm_count() * op.occ);
+  k<<<(unsigned)grid, nthreads, smem, s>>>(a);
+  FR_CUDA_TRY(cudaGetLastError());
 }
 
 }  // namespace frb
