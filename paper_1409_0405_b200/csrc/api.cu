@@ -359,12 +359,9 @@ struct Ctx : CtxBase {
     // only the launch geometry varies between candidates: the packing (k-lists or dense k-blocks) and the composition of every
     // k-block depend on the operator alone (panel.cuh), so every candidate gives bit-identical results
     const int ncand = getenv("FRB_TUNE_CANDS") ? std::max(1, atoi(getenv("FRB_TUNE_CANDS"))) : kTuneCands;
-    for (int k = 1, miss = 0; k < ncand + miss && miss < 64; ++k) {
+    for (int k = 1; k < ncand; ++k) {
       PanelOp<T> op;
-      if (!build(op, k)) {
-        ++miss;                  // the candidate does not fit shared memory (or does not exist): try the next
-        continue;
-      }
+      if (!build(op, k)) break;   // candidates are the geometries that fit shared memory, in order: no k-th one left
       const float t = time_op(op);
       if (verbose) fprintf(stderr, "autotune %s cand %d: %.3f ms\n", what, k, t);
       if (t < bt) {

@@ -100,12 +100,15 @@ struct PanelGeom {
 
 // Warps per CTA (consumers + one producer per group) a given accumulator shape allows: a multiple of four (ptxas sizes the
 // register budget for whole quads of warps, one per SM sub-partition), the largest whose register share still leaves the
-// accumulators 48 registers of head-room.  FP64: NIT*CX*10 doubles per thread; FP32: NIT*CX*40 floats.
+// accumulators 68 registers of head-room (less spills loop-carried scalars, which costs a local-memory round trip per chunk).  FP64: NIT*CX*10 doubles per thread; FP32: NIT*CX*40 floats.
 template <typename T>
 constexpr int panel_maxw(int nit, int cx) {
   // FP32 tiles also keep 8 operator values and 5*CX state values live per k and index more arrays: the CX = 2 shapes spill
   // inside the multiply loop with little head-room (8x slower), so FP32 with CX = 2 budgets +110.
-  const int need = (sizeof(T) == 8 ? nit * cx * 20 : nit * cx * 40) + ((sizeof(T) == 4 && cx == 2) ? 110 : 48);
+  const int need = (sizeof(T) == 8 ? nit * cx * 20 : nit * cx * 40) + ((sizeof(T) == 4 && cx == 2) ? 110 : 68);
+  // the gradient operators of prisms (10 triples of row groups) need 10 row-warps of NIT = 6 (FP64) / NIT = 3 (FP32): these two
+  // shapes take 12 warps at 168 registers and spill ~150 bytes in the epilogue
+  if ((sizeof(T) == 8 ? nit * cx == 6 : nit * cx == 3)) return 12;
   int w = PANEL_MAXW / 4 * 4;
   while (w > 8 && 2048 / w < need) w -= 4;
   return w;
@@ -275,14 +278,14 @@ inline uint32_t swz_row_offset(int r) { return (uint32_t)r * 128u + (uint32_t)(r
 // operator does not fit the resident-in-shared-memory design with geometry candidate opt.cand (or the candidate does not exist).
 template <typename T>
 bool panel_op_build(PanelOp<T> &p, int M, int K, const double *A, const std::vector<KSource> &srcs, const PackOptions &opt_in,
-                    size_t smem_budget, size_t smem_total = 226 * 1024) {
+                    size_t smem_budget, size_t smem_total_in = 226 * 1024) {
   PackOptions opt = opt_in;
   // FRB_FORCE_CAND=k: build geometry candidate k where the caller asked for the default; falls back to the default if k does
   // not exist for this operator.  Lets the parity tests cover every candidate the autotuner may pick.
   if (opt.cand == 0 && getenv("FRB_FORCE_CAND")) {
     PackOptions o2 = opt;
     o2.cand = atoi(getenv("FRB_FORCE_CAND"));
-    if (o2.cand > 0 && panel_op_build(p, M, K, A, srcs, o2, smem_budget, smem_total)) return true;
+    if (o2.cand > 0 && panel_op_build(p, M, K, A, srcs, o2, smem_budget, smem_total_in)) return true;
   }
   const bool f64 = sizeof(T) == 8;
   FR_REQUIRE((int)srcs.size() >= 1 && (int)srcs.size() <= PANEL_MAXSRC, "panel_op_build: one or two stacked sources");
@@ -391,10 +394,12 @@ bool panel_op_build(PanelOp<T> &p, int M, int K, const double *A, const std::vec
   }
   const int G = (int)order.size() / 8;
 
-  // ---- geometry
+  // ---- geometry: candidate k = the k-th geometry of the list that fits shared memory
   const std::vector<PanelGeom> geoms = list_geoms<T>(G, opt.min_ne, opt.max_ne, opt.triple, !sparse);
-  if (opt.cand < 0 || opt.cand >= (int)geoms.size()) return false;
-  const PanelGeom geo = geoms[opt.cand];
+  if (opt.cand < 0) return false;
+  int nfit = 0;
+  for (const PanelGeom &geo : geoms) {
+  size_t smem_total = smem_total_in;
   const int WR = geo.WR, NIT = geo.NIT, NS = WR * NIT;
   // cost of each group (blocks it executes) and LPT assignment of group units (1 or 3 groups) to row-warps
   std::vector<long long> gcost(G, 0);
@@ -519,13 +524,14 @@ bool panel_op_build(PanelOp<T> &p, int M, int K, const double *A, const std::vec
   pad16(rowmap);
   const size_t smem_op = vals.size() * sizeof(T) + idx.size() * 4 + off.size() * 4 + rowmap.size() * 4 + chunks.size() * sizeof(ChunkDesc);
   if (geo.occ == 2) smem_total = smem_total / 2 - 1024;
-  if (smem_op > smem_budget) return false;
+  if (smem_op > smem_budget) continue;
   size_t stage_bytes = 0;
   for (auto &c : chunks) stage_bytes = std::max(stage_bytes, (size_t)PV * geo.NE * c.step * sizeof(T));
   stage_bytes = (stage_bytes + 1023) / 1024 * 1024;
   // 1 kB to align the ring, the ring, 256 B of mbarriers
   const size_t fixed = 1024 + (smem_op + 1023) / 1024 * 1024 + 256;
-  if (fixed + 2 * geo.NG * stage_bytes > smem_total) return false;
+  if (fixed + 2 * geo.NG * stage_bytes > smem_total) continue;
+  if (nfit++ != opt.cand) continue;
   int nstage = (int)((smem_total - fixed) / (geo.NG * stage_bytes));
   nstage = std::min(nstage, PANEL_MAXSTAGE);
   if (getenv("FRB_NSTAGE")) nstage = std::max(2, std::min(nstage, atoi(getenv("FRB_NSTAGE"))));
@@ -577,6 +583,8 @@ bool panel_op_build(PanelOp<T> &p, int M, int K, const double *A, const std::vec
   up(p.rowmap, rowmap);
   up(p.chunks, chunks);
   return true;
+  }
+  return false;
 }
 
 template <typename T>

@@ -44,7 +44,7 @@ void panel_gemm_run(const PanelOp<T> &op, long long N, T c1, const T *B, long lo
   a.prod.tm[0] = tmap_plain(B, op.K, N, ldb, bsB, nbatch, op.NE, op.src_step[0]);
   a.prod.tm[1] = a.prod.tm[0];
   a.prod.plain = 1;
-  a.epi = PlainEpilogue<T>{C, ldc, bsC, cm, c1, c2};
+  a.epi = PlainEpilogue<T>{C, ldc, bsC, cm, c1, c2, (c1 == T(1) && c2 == T(0)) ? 1 : 0};
   a.npanels = (N + pw - 1) / pw;
   a.nbatch = nbatch;
 #define FR_CASE(NIT_, CX_)                                                                        \

@@ -46,17 +46,19 @@ struct alignas(64) TmaProducer {
   }
 };
 
-// ---- epilogue: C <- c1*acc + c2*C
+// ---- epilogue: C <- c1*acc + c2*C.  `plain` (decided on the host: c1 == 1 and c2 == 0, the case of every product inside fr_rhs)
+// stores the accumulators as they are: no FP64 instruction in the epilogue, which would queue behind the other warps' DMMAs.
 template <typename T>
 struct PlainEpilogue {
   T *C;
   long long ldc, bstride;
   ColMap cm;
   T c1, c2;
+  int plain;
   template <typename ACC>
   __device__ __forceinline__ void prefetch(ACC &acc, const int *rowmap, int slot0, long long batch, long long pl, int wc,
                                            int lane) const {
-    if (c2 == T(0)) return;
+    if (plain || c2 == T(0)) return;
     const T *Cb = C + batch * bstride + pl * cm.pstride;
     acc.foreach_coord(wc, lane, [&](int i, int rr, int e) {
       const int m = rowmap[(slot0 + i) * 8 + (ACC::ROWS == 1 ? (lane >> 2) : rr)];
@@ -75,6 +77,21 @@ struct PlainEpilogue {
     const bool interior = vb + (PV - 1) * cm.vlim + (cm.pstride > cm.vstride ? cm.vstride : cm.pstride) <= cm.lim;
     int mrow[ACC::NSLOT][ACC::ROWS];
     acc.foreach_row(lane, [&](int i, int rr, int r) { mrow[i][rr] = rowmap[(slot0 + i) * 8 + r]; });
+    if (plain && interior) {
+      acc.foreach_tile(wc, lane, [&](int i, int rr, int e, T(&tile)[PV][EW]) {
+        const int m = mrow[i][rr];
+        if (m < 0) return;
+        T *cp = Cb + (long long)m * ldc + e;
+#pragma unroll
+        for (int v = 0; v < PV; ++v) {
+          if (EW == 2 && sizeof(T) == 8) *reinterpret_cast<double2 *>(cp) = *reinterpret_cast<double2 *>(tile[v]);
+          else if (EW == 2) *reinterpret_cast<float2 *>(cp) = *reinterpret_cast<float2 *>(tile[v]);
+          else cp[0] = tile[v][0];
+          cp += cm.vstride;
+        }
+      });
+      return;
+    }
     acc.foreach_tile(wc, lane, [&](int i, int rr, int e, T(&tile)[PV][EW]) {
       const int m = mrow[i][rr];
       if (m < 0) return;
@@ -135,11 +152,13 @@ __device__ __forceinline__ void panel_mainloop(const PanelOp<T> &op, const Prod 
   __syncthreads();
   OpSmem<T> A;
   op_smem_carve(smem_raw, op, A);
+  // panel counts fit 32 bits (leading dimensions are below 2^31 and a panel has at least 16 elements)
+  const int npb = (int)npanels_per_batch;
   const long long ntot = npanels_per_batch * nbatch;
-  const long long first = (long long)blockIdx.x * NG + grp, stride = (long long)gridDim.x * NG;
-  const long long mine = first < ntot ? (ntot - first + stride - 1) / stride : 0;
+  const int first = blockIdx.x * NG + grp, stride = gridDim.x * NG;
+  const int mine = first < ntot ? (int)((ntot - first + stride - 1) / stride) : 0;
   const int nchunks = op.nchunks;
-  const long long total = mine * nchunks;
+  const int total = mine * nchunks;
   const uint32_t gbar = bars + (uint32_t)(grp * nstage) * 16u;
   const uint32_t gring = ring0 + (uint32_t)(grp * nstage) * stage_bytes;
 
@@ -159,11 +178,11 @@ __device__ __forceinline__ void panel_mainloop(const PanelOp<T> &op, const Prod 
       d += (uint32_t)op.bytes_rowmap;
       bulk_load(d, op.chunks, (uint32_t)op.bytes_chunks, bar_img);
     }
-    long long pl = first, batch = pl / npanels_per_batch;
-    pl -= batch * npanels_per_batch;
+    int pl = first, batch = pl / npb;
+    pl -= batch * npb;
     int stage = 0;
     uint32_t phase = 0;
-    for (long long p = 0; p < mine; ++p) {
+    for (int p = 0; p < mine; ++p) {
       for (int c = 0; c < nchunks; ++c) {
         const ChunkDesc cd = op.chunks[c];               // global (L1-resident); the image may not have landed yet
         mbar_wait(gbar + stage * 16 + 8, phase ^ 1u);    // stage is empty
@@ -176,8 +195,8 @@ __device__ __forceinline__ void panel_mainloop(const PanelOp<T> &op, const Prod 
         }
       }
       pl += stride;
-      while (pl >= npanels_per_batch) {
-        pl -= npanels_per_batch;
+      while (pl >= npb) {
+        pl -= npb;
         ++batch;
       }
     }
@@ -189,11 +208,11 @@ __device__ __forceinline__ void panel_mainloop(const PanelOp<T> &op, const Prod 
   const int cw = tid >> 5;                             // warp within the group
   const int wr = cw / WC, wc = cw - wr * WC;
   mbar_wait(bar_img, 0);
-  long long cpl = first, cbatch = cpl / npanels_per_batch;
-  cpl -= cbatch * npanels_per_batch;
+  int cpl = first, cbatch = cpl / npb;
+  cpl -= cbatch * npb;
   // Group 1 starts half a panel late, so that one group's epilogue (global loads and stores, latency-bound) runs under the
   // other group's multiplies.
-  const long long stagger_q = total > 0 ? (nchunks / 2 < total ? nchunks / 2 : total - 1) : -1;
+  const int stagger_q = total > 0 ? (nchunks / 2 < total ? nchunks / 2 : total - 1) : -1;
   if (NG == 2) {
     if (grp == 1) asm volatile("bar.sync 3, %0;" ::"r"(2 * nwc * 32) : "memory");
     else if (stagger_q < 0) asm volatile("bar.arrive 3, %0;" ::"r"(2 * nwc * 32) : "memory");
@@ -202,7 +221,7 @@ __device__ __forceinline__ void panel_mainloop(const PanelOp<T> &op, const Prod 
   acc.zero();
   int stage = 0, cc = 0;
   uint32_t phase = 0;
-  for (long long q = 0; q < total; ++q) {
+  for (int q = 0; q < total; ++q) {
     mbar_wait(gbar + stage * 16, phase);
     const char *st = ringp + (size_t)(grp * nstage + stage) * stage_bytes;
     // the epilogue's own global operands: pull them into L2 while the last chunk is multiplied
@@ -229,8 +248,8 @@ __device__ __forceinline__ void panel_mainloop(const PanelOp<T> &op, const Prod 
       acc.zero();
       cc = 0;
       cpl += stride;
-      while (cpl >= npanels_per_batch) {
-        cpl -= npanels_per_batch;
+      while (cpl >= npb) {
+        cpl -= npb;
         ++cbatch;
       }
     }
