@@ -172,6 +172,18 @@ typedef struct {
   int32_t category;   /* 0 operator product, 1 point-wise at solution points, 2 interface / boundary */
 } fr_kernel_stat;
 fr_status fr_profile_kernels(fr_ctx *ctx, int32_t reps, fr_kernel_stat *out, int32_t cap, int32_t *n);
+/* The same for the right-hand side AS A RUNGE-KUTTA STAGE runs it (the variant fr_rk_step replays: S10 of SURVEY 8(a), the
+ * stage update X <- X + c1 K, Y <- X + c2 K, fused into the last kernel of each type, with both coefficients zero here so the
+ * internal state is unchanged). */
+fr_status fr_profile_stage_kernels(fr_ctx *ctx, int32_t reps, fr_kernel_stat *out, int32_t cap, int32_t *n);
+
+/* Failure detection off the hot path: counts the non-finite entries (NaN / Inf) of the internal solution register,
+ * padding columns excluded.  Synchronous. */
+fr_status fr_check_finite(fr_ctx *ctx, int64_t *n_nonfinite);
+
+/* The launch plan fr_setup chose (packing, warp grid, panel width, ring depth per operator), one line per operator, as a
+ * NUL-terminated string of at most cap - 1 characters.  Results never depend on it (bit-identical for every plan). */
+fr_status fr_plan_describe(const fr_ctx *ctx, char *buf, int64_t cap);
 
 /* End-to-end step on HOST buffers: copies u_host[t] (HOST, fr_state_layout layout and the context's precision,
  * ideally pinned) into the solution register, advances one step of size dt, copies the new state back into the
@@ -200,6 +212,9 @@ void fr_gemm_plan_destroy(fr_gemm_plan *plan);
 /* Measured device peaks used as roofline denominators: register-resident FMA
  * chains (TFLOP/s, FP64 and FP32) and a device-to-device copy (GB/s, read+write bytes).  Synchronous. */
 fr_status fr_probe_peaks(double *fp64_tflops, double *fp32_tflops, double *copy_gbs);
+/* The FP64 tensor pipe (mma.sync.m8n8k4.f64, what the FP64 operator products run on): TFLOP/s of
+ * register-resident chains, 512 flops per warp instruction.  The denominator of compute-bound FP64 roofline fractions. */
+fr_status fr_probe_dmma(double *fp64_tensor_tflops);
 
 #ifdef __cplusplus
 }

@@ -58,7 +58,8 @@ class fr_adapt_stats(C.Structure):
 SYMBOLS = ["fr_profile_kernels", "fr_rk_step_host", "fr_setup", "fr_state_layout", "fr_rhs", "fr_set_state", "fr_get_state", "fr_rk_step", "fr_rk_run",
            "fr_rk_adaptive_run",
            "fr_sync", "fr_launch_count", "fr_profile_rhs", "fr_last_error", "fr_global_error", "fr_destroy",
-           "fr_gemm", "fr_gemm_plan_create", "fr_gemm_plan_run", "fr_gemm_plan_destroy", "fr_probe_peaks"]
+           "fr_gemm", "fr_gemm_plan_create", "fr_gemm_plan_run", "fr_gemm_plan_destroy", "fr_probe_peaks", "fr_probe_dmma",
+           "fr_profile_stage_kernels", "fr_check_finite", "fr_plan_describe"]
 
 _lib = None
 
@@ -101,6 +102,10 @@ def load():
     lib.fr_gemm_plan_destroy.argtypes = [vp]
     lib.fr_gemm_plan_destroy.restype = None
     lib.fr_probe_peaks.argtypes = [_dp, _dp, _dp]
+    lib.fr_probe_dmma.argtypes = [_dp]
+    lib.fr_profile_stage_kernels.argtypes = [vp, C.c_int32, C.POINTER(fr_kernel_stat), C.c_int32, _i32p]
+    lib.fr_check_finite.argtypes = [vp, _i64p]
+    lib.fr_plan_describe.argtypes = [vp, C.c_char_p, C.c_int64]
     _lib = lib
     return lib
 
@@ -256,6 +261,24 @@ class Context:
         return [dict(name=arr[i].name.decode(), ms=arr[i].ms, alg_bytes=arr[i].alg_bytes, flops=arr[i].flops,
                      category=arr[i].category) for i in range(min(n.value, cap))]
 
+    def profile_stage_kernels(self, reps=5, cap=64):
+        """fr_profile_stage_kernels: the per-kernel breakdown of the right-hand side as an RK stage runs it."""
+        arr = (fr_kernel_stat * cap)()
+        n = C.c_int32(0)
+        self._check(self._lib.fr_profile_stage_kernels(self._h, reps, arr, cap, C.byref(n)))
+        return [dict(name=arr[i].name.decode(), ms=arr[i].ms, alg_bytes=arr[i].alg_bytes, flops=arr[i].flops,
+                     category=arr[i].category) for i in range(min(n.value, cap))]
+
+    def check_finite(self):
+        n = C.c_int64(0)
+        self._check(self._lib.fr_check_finite(self._h, C.byref(n)))
+        return int(n.value)
+
+    def plan_describe(self):
+        buf = C.create_string_buffer(8192)
+        self._check(self._lib.fr_plan_describe(self._h, buf, 8192))
+        return buf.value.decode()
+
     def rk_step_host(self, dt, host_ptrs):
         """fr_rk_step_host on HOST pointers (ints) in the device layout / precision."""
         hp = (C.c_void_p * self.netypes)(*[C.c_void_p(int(p)) for p in host_ptrs])
@@ -311,6 +334,16 @@ class GemmPlan:
             self.close()
         except Exception:
             pass
+
+
+def probe_dmma():
+    """fr_probe_dmma: TFLOP/s of the FP64 tensor pipe (mma.sync.m8n8k4.f64 chains)."""
+    lib = load()
+    a = C.c_double()
+    st = lib.fr_probe_dmma(C.byref(a))
+    if st != FR_OK:
+        raise FrError(st, "fr_probe_dmma failed")
+    return a.value
 
 
 def probe_peaks():

@@ -6,9 +6,17 @@
 #include <memory>
 #include <numeric>
 
+#include <nvtx3/nvToolsExt.h>
+
 #include "kernels.cuh"
 
 namespace frb {
+
+// NVTX range around one step of the right-hand side (SURVEY 5 "tracing"): a no-op unless a tool is attached
+struct NvtxRange {
+  explicit NvtxRange(const char *name) { nvtxRangePushA(name); }
+  ~NvtxRange() { nvtxRangePop(); }
+};
 
 static thread_local std::string g_error;
 
@@ -23,7 +31,9 @@ struct CtxBase {
   virtual void get_state(double *const *u) = 0;
   virtual void rk_step(double dt, long long nsteps) = 0;
   virtual void sync() = 0;
-  virtual void profile(int reps, double ms[4], fr_kernel_stat *out, int cap, int *n) = 0;
+  virtual void profile(int reps, double ms[4], fr_kernel_stat *out, int cap, int *n, bool stage = false) = 0;
+  virtual long long check_finite() = 0;
+  virtual std::string describe() const = 0;
   virtual void rk_step_host(double dt, void *const *u_host) = 0;
   virtual void rk_adaptive(double t0, double t1, double dt0, double atol, double rtol, long long max_attempts, fr_adapt_stats *st,
                            double *dt_hist, double *err_hist, long long hist_cap) = 0;
@@ -208,6 +218,8 @@ struct Ctx : CtxBase {
     FR_REQUIRE(c->gamma > 1.0, "gamma must be > 1");
     const bool ns = system == FR_NAVIER_STOKES;
     FR_REQUIRE(!ns || (c->mu >= 0.0 && c->prandtl > 0.0), "mu must be >= 0 and prandtl > 0");
+    FR_REQUIRE(!ns || (std::isfinite(c->ldg_beta) && std::isfinite(c->ldg_tau)), "ldg_beta and ldg_tau must be finite");
+    FR_REQUIRE(std::isfinite(c->gamma) && (!ns || (std::isfinite(c->mu) && std::isfinite(c->prandtl))), "gamma, mu and prandtl must be finite");
     ph.gamma = (T)c->gamma;
     ph.mu = (T)(ns ? c->mu : 0.0);
     ph.prandtl = (T)(ns ? c->prandtl : 1.0);
@@ -524,18 +536,21 @@ struct Ctx : CtxBase {
     for (auto &b : bnd) nbnd += (double)b->view.n;
     const double npr = (double)iv.npairs;
     auto do_S1 = [&](int t, cudaStream_t q) {   // S1: U_f = M0 U
+      NvtxRange r("S1 interp");
       EleData<T> &e = *el[t];
       const double n = (double)e.view.neles, nu = e.view.nupts, nf = e.view.nfpts;
       nk += gemm_run(e.pM0, 5 * e.view.ld, T(1), u[t], 5 * e.view.ld, 0, T(0), uf.p + tt.ubase[t], 5 * e.view.ld, 0, 1, q);
       mark(CAT_GEMM, t, "S1_M0", (nu + nf) * 5 * n, 2 * (e.pM0.pop ? e.pM0.pop->density : 1.0) * nf * nu * 5 * n);
     };
     auto do_S2 = [&]() {
+      NvtxRange r("S2 con_u");
       nk += launch_con_u(iv, tt, uf.p, cf.p, ph.beta, jump, s);   // S2
       for (auto &b : bnd) nk += launch_bc_con_u(b->view, tt, uf.p, cf.p, ph.gamma, jump, s);
       const double words = jump ? (ph.beta == T(0.5) ? 15 : 20) : 20;
       mark(CAT_IFACE, -1, jump ? "S2_con_u_jump" : "S2_con_u", npr * (words + 16 / w) + nbnd * (10 + 3 + 8 / w), npr * 15 + nbnd * 60);
     };
     auto do_grad = [&](int t, cudaStream_t q) {   // S3, S4, S5
+      NvtxRange r("S3-S5 gradient");
       EleData<T> &e = *el[t];
       const long long n5 = 5 * e.view.ld;
       const double n = (double)e.view.neles, nu = e.view.nupts, nf = e.view.nfpts;
@@ -560,6 +575,7 @@ struct Ctx : CtxBase {
       mark(CAT_GEMM, t, "S5_M0grad", (nu + nf) * 15 * n, 2 * (e.pM0.pop ? e.pM0.pop->density : 1.0) * nf * nu * 15 * n);
     };
     auto do_S7 = [&]() {
+      NvtxRange r("S7 comm_flux");
       nk += launch_comm_flux(iv, tt, uf.p, gf.p, ph, s);   // S7 (D overwrites U_f)
       for (auto &b : bnd) nk += launch_bc_comm_flux(b->view, tt, uf.p, gf.p, ph, s);
       const double sides = ns ? ((ph.beta == T(0.5) || ph.beta == T(-0.5)) ? 1 : 2) : 0;
@@ -567,6 +583,7 @@ struct Ctx : CtxBase {
            npr * (ns ? 420 : 160) + nbnd * (ns ? 420 : 200));
     };
     auto do_S6 = [&](int t, cudaStream_t q) {
+      NvtxRange r("S6 tdisf");
       EleData<T> &e = *el[t];
       const double n = (double)e.view.neles, nu = e.view.nupts;
       const double nmet = e.view.affine ? 1 : nu;
@@ -574,6 +591,7 @@ struct Ctx : CtxBase {
       mark(CAT_PW, t, "S6_tdisf", ((ns ? 35 : 20) * nu + 9 * nmet) * n, (ns ? 210 : 110) * nu * n);
     };
     auto do_div = [&](int t, cudaStream_t q) {   // S8, S9, S10
+      NvtxRange r("S8-S10 divergence + stage update");
       EleData<T> &e = *el[t];
       const long long n5 = 5 * e.view.ld;
       const double n = (double)e.view.neles, nu = e.view.nupts, nf = e.view.nfpts;
@@ -919,13 +937,20 @@ struct Ctx : CtxBase {
   }
 
   // Events between all kernels of `reps` RHS evaluations of the internal state; per-category and per-kernel means.
-  void profile(int reps, double ms[4], fr_kernel_stat *out, int cap, int *nout) override {
+  void profile(int reps, double ms[4], fr_kernel_stat *out, int cap, int *nout, bool stage) override {
     FR_REQUIRE(reps > 0, "reps must be positive");
     std::vector<const T *> up(nt);
     std::vector<StageArgs<T>> sa(nt);
+    if (stage) {
+      // the variant an RK45[2R+] stage runs (both registers read and written), with zero coefficients: X and Y keep their values
+      FR_CUDA_TRY(cudaStreamSynchronize(stream));
+      coef_host[7] = StageCoef{0.0, 0.0};
+      FR_CUDA_TRY(cudaMemcpyAsync(coef.p + 7, coef_host + 7, sizeof(StageCoef), cudaMemcpyHostToDevice, stream));
+    }
     for (int t = 0; t < nt; ++t) {
       up[t] = el[t]->X.p;
-      sa[t] = StageArgs<T>{nullptr, nullptr, nullptr, el[t]->Y.p, nullptr};
+      sa[t] = stage ? StageArgs<T>{coef.p + 7, el[t]->X.p, el[t]->X.p, el[t]->X.p, el[t]->Y.p}
+                    : StageArgs<T>{nullptr, nullptr, nullptr, el[t]->Y.p, nullptr};
     }
     launches += run_rhs(up.data(), sa.data(), nullptr);   // warm-up
     double acc[4] = {0, 0, 0, 0};
@@ -960,6 +985,39 @@ struct Ctx : CtxBase {
     if (nout) *nout = (int)ks.size();
     if (out)
       for (int i = 0; i < (int)ks.size() && i < cap; ++i) out[i] = ks[i];
+  }
+
+  long long check_finite() override {
+    FR_CUDA_TRY(cudaStreamSynchronize(stream));
+    long long bad = 0;
+    for (int t = 0; t < nt; ++t) {
+      const EleView<T> &v = el[t]->view;
+      std::vector<T> h((size_t)v.nupts * 5 * v.ld);
+      FR_CUDA_TRY(cudaMemcpy(h.data(), el[t]->X.p, h.size() * sizeof(T), cudaMemcpyDeviceToHost));
+      for (long long r = 0; r < (long long)v.nupts * 5; ++r)
+        for (long long k = 0; k < v.neles; ++k) bad += std::isfinite((double)h[(size_t)r * v.ld + k]) ? 0 : 1;
+    }
+    return bad;
+  }
+
+  std::string describe() const override {
+    std::string out;
+    char line[256];
+    auto add = [&](const char *type, const char *what, const PanelOp<T> &op) {
+      if (!op.ok()) return;
+      snprintf(line, sizeof line, "%s %s %s %dx%d %s warps=%dx%dx%d+%d NIT=%d CX=%d NE=%d stages=%dx%d B occ=%d\n", sizeof(T) == 8 ? "f64" : "f32",
+               type, what, op.M, op.K, op.sparse ? "k-lists" : "dense", op.NG, op.WR, op.WC, op.NG, op.NIT, op.CX, op.NE, op.nstage,
+               op.stage_bytes, op.occ);
+      out += line;
+    };
+    for (int t = 0; t < nt; ++t) {
+      const EleData<T> &e = *el[t];
+      if (e.pM0.pop) add(tname[t], "M0", *e.pM0.pop);
+      for (int i = 0; i < e.pM0.nparts; ++i) add(tname[t], "M0/rows", *e.pM0.part[i]);
+      for (auto &q : e.pGrad) add(tname[t], "[M460|M6]", q.op);
+      for (auto &q : e.pDiv) add(tname[t], "[M132|M3]", q.op);
+    }
+    return out;
   }
 
   // H2D of the state (device layout, context precision), one step, D2H -- the end-to-end user call.
@@ -1073,6 +1131,30 @@ fr_status fr_profile_kernels(fr_ctx *ctx, int32_t reps, fr_kernel_stat *out, int
     int nn = 0;
     ctx->impl->profile(reps, nullptr, out, cap, &nn);
     *n = nn;
+  });
+}
+fr_status fr_profile_stage_kernels(fr_ctx *ctx, int32_t reps, fr_kernel_stat *out, int32_t cap, int32_t *n) {
+  FR_CTX_CALL(ctx, {
+    FR_REQUIRE(n && (out || cap == 0), "n must be non-NULL (and out non-NULL when cap > 0)");
+    int nn = 0;
+    ctx->impl->profile(reps, nullptr, out, cap, &nn, true);
+    *n = nn;
+  });
+}
+fr_status fr_check_finite(fr_ctx *ctx, int64_t *n_nonfinite) {
+  FR_CTX_CALL(ctx, {
+    FR_REQUIRE(n_nonfinite, "n_nonfinite must be non-NULL");
+    *n_nonfinite = ctx->impl->check_finite();
+  });
+}
+fr_status fr_plan_describe(const fr_ctx *ctx, char *buf, int64_t cap) {
+  if (!ctx || !ctx->impl) return FR_EINVAL;
+  return guard(nullptr, [&] {
+    FR_REQUIRE(buf && cap > 0, "buf must be non-NULL and cap positive");
+    const std::string d = ctx->impl->describe();
+    const size_t nc = std::min<size_t>(d.size(), (size_t)cap - 1);
+    memcpy(buf, d.data(), nc);
+    buf[nc] = 0;
   });
 }
 fr_status fr_rk_step_host(fr_ctx *ctx, double dt, void *const *u_host) { FR_CTX_CALL(ctx, ctx->impl->rk_step_host(dt, u_host)); }

@@ -69,13 +69,86 @@ struct RkEpilogue {
       const long long col = e0 + e;
       if (curved || i == 0) prefetch_l2(rcpdjac + (curved ? (long long)m * ld : 0) + col);
       if (!sa.coef) return;
+      const T *p1 = sa.in1 + (long long)m * 5 * ld + col, *p2 = sa.in2 + (long long)m * 5 * ld + col;
 #pragma unroll
       for (int v = 0; v < PV; ++v) {
-        const long long idx = ((long long)m * 5 + v) * ld + col;
-        prefetch_l2(sa.in1 + idx);
-        if (sa.out2 && sa.in2 != sa.in1) prefetch_l2(sa.in2 + idx);
+        prefetch_l2(p1);
+        if (sa.out2 && sa.in2 != sa.in1) prefetch_l2(p2);
+        p1 += ld;
+        p2 += ld;
       }
     });
+  }
+  // One tile (row m, EW consecutive elements, all variables).  MASK: the panel holds padding columns (col >= neles), which are
+  // written as zero whatever the accumulators hold; interior panels skip the selects.
+  template <bool MASK, int EW>
+  __device__ __forceinline__ void tile_update(T (&tile)[PV][EW], int m, long long col, T c1, T c2, bool same) const {
+    const long long idx0 = (long long)m * 5 * ld + col;
+    T rj[EW];
+    VecIO<T, EW>::ldg(rcpdjac + (curved ? (long long)m * ld : 0) + col, rj);
+    bool live[EW];
+#pragma unroll
+    for (int j = 0; j < EW; ++j) live[j] = !MASK || col + j < neles;
+    auto sel = [&](int j, T x) { return (!MASK || live[j]) ? x : T(0); };
+    if (!sa.coef) {
+      T *o = sa.out1 + idx0;
+#pragma unroll
+      for (int v = 0; v < PV; ++v) {
+        T k[EW];
+#pragma unroll
+        for (int j = 0; j < EW; ++j) k[j] = sel(j, -tile[v][j] * rj[j]);
+        VecIO<T, EW>::st(o, k);
+        o += ld;
+      }
+      return;
+    }
+    // the loads of the tile together, then the stores: the stores may alias the loads, so the compiler would otherwise serialise
+    // load -> store -> load and expose one memory latency per variable
+    T a[PV][EW];
+    const T *pa = sa.in1 + idx0;
+#pragma unroll
+    for (int v = 0; v < PV; ++v) {
+      VecIO<T, EW>::ld(pa, a[v]);
+      pa += ld;
+    }
+    T *o1p = sa.out1 + idx0, *o2p = sa.out2 + idx0;
+    if (sa.out2 && !same) {
+      const T *pb = sa.in2 + idx0;
+#pragma unroll
+      for (int v = 0; v < PV; ++v) {
+        T bb[EW], k[EW], o1[EW], o2[EW];
+        VecIO<T, EW>::ld(pb, bb);
+#pragma unroll
+        for (int j = 0; j < EW; ++j) {
+          k[j] = -tile[v][j] * rj[j];
+          o2[j] = sel(j, bb[j] + c2 * k[j]);
+          o1[j] = sel(j, a[v][j] + c1 * k[j]);
+        }
+        VecIO<T, EW>::st(o2p, o2);
+        VecIO<T, EW>::st(o1p, o1);
+        pb += ld;
+        o1p += ld;
+        o2p += ld;
+      }
+      return;
+    }
+#pragma unroll
+    for (int v = 0; v < PV; ++v) {
+      T k[EW], o1[EW];
+#pragma unroll
+      for (int j = 0; j < EW; ++j) k[j] = -tile[v][j] * rj[j];
+      if (sa.out2) {
+        T o2[EW];
+#pragma unroll
+        for (int j = 0; j < EW; ++j) o2[j] = sel(j, a[v][j] + c2 * k[j]);
+        VecIO<T, EW>::st(o2p, o2);
+        o2p += ld;
+      }
+#pragma unroll
+      for (int j = 0; j < EW; ++j) o1[j] = sel(j, a[v][j] + c1 * k[j]);
+      VecIO<T, EW>::st(o1p, o1);
+      o1p += ld;
+    }
   }
   template <typename ACC>
   __device__ __forceinline__ void operator()(ACC &acc, const int *rowmap, int slot0, long long, long long pl, int wc, int lane) const {
@@ -89,101 +162,15 @@ struct RkEpilogue {
     int mrow[ACC::NSLOT][ACC::ROWS];
     acc.foreach_row(lane, [&](int i, int rr, int r) { mrow[i][rr] = rowmap[(slot0 + i) * 8 + r]; });
     const bool same = sa.in2 == sa.in1;
-    acc.foreach_tile(wc, lane, [&](int i, int rr, int e, T(&tile)[PV][EW]) {
-      const int m = mrow[i][rr];
-      if (m < 0) return;
-      const long long col = e0 + e;
-      const long long idx0 = (long long)m * 5 * ld + col;
-      T rj[EW];
-      VecIO<T, EW>::ldg(rcpdjac + (curved ? (long long)m * ld : 0) + col, rj);
-      bool live[EW];
-#pragma unroll
-      for (int j = 0; j < EW; ++j) live[j] = col + j < neles;
-      if constexpr (sizeof(T) == 4) {
-        // FP32: all global loads of the tile first -- the stores below may alias them, so the compiler would otherwise
-        // serialise load -> store -> load and expose one memory latency per variable.  (In FP64 the 20 extra registers
-        // spill: 0.95 -> 1.57 ms on the tetrahedra, so FP64 keeps the load-per-variable order.)
-        T a[PV][EW], b[PV][EW];
-        if (sa.coef) {
-#pragma unroll
-          for (int v = 0; v < PV; ++v) VecIO<T, EW>::ld(sa.in1 + idx0 + v * ld, a[v]);
-          if (sa.out2 && !same) {
-#pragma unroll
-            for (int v = 0; v < PV; ++v) VecIO<T, EW>::ld(sa.in2 + idx0 + v * ld, b[v]);
-          }
-        }
-#pragma unroll
-        for (int v = 0; v < PV; ++v) {
-          const long long idx = idx0 + v * ld;
-          T k[EW], o1[EW];
-#pragma unroll
-          for (int j = 0; j < EW; ++j) k[j] = live[j] ? -tile[v][j] * rj[j] : T(0);
-          if (!sa.coef) {
-            VecIO<T, EW>::st(sa.out1 + idx, k);
-          } else {
-            if (sa.out2) {
-              T o2[EW];
-#pragma unroll
-              for (int j = 0; j < EW; ++j) o2[j] = live[j] ? (same ? a[v][j] : b[v][j]) + c2 * k[j] : T(0);
-              VecIO<T, EW>::st(sa.out2 + idx, o2);
-            }
-#pragma unroll
-            for (int j = 0; j < EW; ++j) o1[j] = live[j] ? a[v][j] + c1 * k[j] : T(0);
-            VecIO<T, EW>::st(sa.out1 + idx, o1);
-          }
-        }
-      } else if (sa.coef && same) {
-        // FP64, RK45[2R+] (both updates start from the same register X): the five loads of the tile together, then the stores
-        T a[PV][EW];
-#pragma unroll
-        for (int v = 0; v < PV; ++v) VecIO<T, EW>::ld(sa.in1 + idx0 + v * ld, a[v]);
-#pragma unroll
-        for (int v = 0; v < PV; ++v) {
-          const long long idx = idx0 + v * ld;
-          T k[EW], o1[EW];
-#pragma unroll
-          for (int j = 0; j < EW; ++j) k[j] = live[j] ? -tile[v][j] * rj[j] : T(0);
-          if (sa.out2) {
-            T o2[EW];
-#pragma unroll
-            for (int j = 0; j < EW; ++j) o2[j] = live[j] ? a[v][j] + c2 * k[j] : T(0);
-            VecIO<T, EW>::st(sa.out2 + idx, o2);
-          }
-#pragma unroll
-          for (int j = 0; j < EW; ++j) o1[j] = live[j] ? a[v][j] + c1 * k[j] : T(0);
-          VecIO<T, EW>::st(sa.out1 + idx, o1);
-        }
-      } else {
-#pragma unroll
-        for (int v = 0; v < PV; ++v) {
-          const long long idx = idx0 + v * ld;
-          T k[EW], o1[EW];
-#pragma unroll
-          for (int j = 0; j < EW; ++j) k[j] = live[j] ? -tile[v][j] * rj[j] : T(0);
-          if (!sa.coef) {
-            VecIO<T, EW>::st(sa.out1 + idx, k);
-          } else {
-            T a[EW];
-            VecIO<T, EW>::ld(sa.in1 + idx, a);
-            if (sa.out2) {
-              T b[EW], o2[EW];
-              if (!same) {
-                VecIO<T, EW>::ld(sa.in2 + idx, b);
-              } else {
-#pragma unroll
-                for (int j = 0; j < EW; ++j) b[j] = a[j];
-              }
-#pragma unroll
-              for (int j = 0; j < EW; ++j) o2[j] = live[j] ? b[j] + c2 * k[j] : T(0);
-              VecIO<T, EW>::st(sa.out2 + idx, o2);
-            }
-#pragma unroll
-            for (int j = 0; j < EW; ++j) o1[j] = live[j] ? a[j] + c1 * k[j] : T(0);
-            VecIO<T, EW>::st(sa.out1 + idx, o1);
-          }
-        }
-      }
-    });
+    if (e0 + NE <= neles) {
+      acc.foreach_tile(wc, lane, [&](int i, int rr, int e, T(&tile)[PV][EW]) {
+        if (mrow[i][rr] >= 0) tile_update<false, EW>(tile, mrow[i][rr], e0 + e, c1, c2, same);
+      });
+    } else {
+      acc.foreach_tile(wc, lane, [&](int i, int rr, int e, T(&tile)[PV][EW]) {
+        if (mrow[i][rr] >= 0) tile_update<true, EW>(tile, mrow[i][rr], e0 + e, c1, c2, same);
+      });
+    }
   }
 };
 
@@ -219,9 +206,56 @@ struct GradEpilogue {
       if (rho < 0 || (!curved && i != 0)) return;
       const long long col = e0 + e;
       prefetch_l2(rcpdjac + (curved ? (long long)rho * ld : 0) + col);
+      const T *sp = smats + (curved ? (long long)rho * ld : 0) + col;
+      const long long sstep = curved ? (long long)nupts * ld : ld;
 #pragma unroll
-      for (int a = 0; a < 9; ++a) prefetch_l2(smats + (curved ? ((long long)a * nupts + rho) * ld : (long long)a * ld) + col);
+      for (int a = 0; a < 9; ++a) {
+        prefetch_l2(sp);
+        sp += sstep;
+      }
     });
+  }
+  // One solution point rho, EW consecutive elements: G_i = (1/|J|) sum_alpha S[alpha][i] G~_alpha, one column i of S at a time
+  // (three metric loads live instead of nine).  Metric terms are stored [alpha*3 + i][point][ld].
+  template <bool MASK, int EW>
+  __device__ __forceinline__ void point_transform(T (&t0)[PV][EW], T (&t1)[PV][EW], T (&t2)[PV][EW], int rho, long long col) const {
+    T rj[EW];
+    VecIO<T, EW>::ldg(rcpdjac + (curved ? (long long)rho * ld : 0) + col, rj);
+    if (MASK) {
+#pragma unroll
+      for (int j = 0; j < EW; ++j)
+        if (col + j >= neles) rj[j] = T(0);
+    }
+    const long long sstep = curved ? (long long)nupts * ld : ld;      // between metric terms
+    const T *sp = smats + (curved ? (long long)rho * ld : 0) + col;   // S[0][0]
+    T *gp = grad + (long long)rho * 5 * ld + col;
+    const long long gstep = (long long)nupts * 5 * ld;                 // between gradient components
+#pragma unroll
+    for (int i = 0; i < 3; ++i) {
+      T s0[EW], s1[EW], s2[EW];
+      VecIO<T, EW>::ldg(sp + i * sstep, s0);
+      VecIO<T, EW>::ldg(sp + (3 + i) * sstep, s1);
+      VecIO<T, EW>::ldg(sp + (6 + i) * sstep, s2);
+#pragma unroll
+      for (int j = 0; j < EW; ++j) {
+        s0[j] *= rj[j];
+        s1[j] *= rj[j];
+        s2[j] *= rj[j];
+      }
+      T *o = gp;
+#pragma unroll
+      for (int v = 0; v < PV; ++v) {
+        T q[EW];
+#pragma unroll
+        for (int j = 0; j < EW; ++j) {
+          q[j] = s0[j] * t0[v][j] + s1[j] * t1[v][j] + s2[j] * t2[v][j];
+          if (MASK && col + j >= neles) q[j] = T(0);     // 0 * (non-finite garbage of a padding column) would not be 0
+        }
+        VecIO<T, EW>::st(o, q);
+        o += ld;
+      }
+      gp += gstep;
+    }
   }
   template <typename ACC>
   __device__ __forceinline__ void operator()(ACC &acc, const int *rowmap, int slot0, long long, long long pl, int wc, int lane) const {
@@ -229,30 +263,17 @@ struct GradEpilogue {
     const long long e0 = pl * NE;
     int mrow[ACC::NSLOT][ACC::ROWS];
     acc.foreach_row(lane, [&](int i, int rr, int r) { mrow[i][rr] = rowmap[(slot0 + i) * 8 + r]; });
-    acc.foreach_triple(wc, lane, [&](int t, int rr, int e, T(&t0)[PV][EW], T(&t1)[PV][EW], T(&t2)[PV][EW]) {
-      const int rho = mrow[3 * t][rr];     // alpha = 0 rows are 0..Nu-1
-      if (rho < 0) return;
-      const long long col = e0 + e;
-      T rj[EW], S[3][3][EW];
-      VecIO<T, EW>::ldg(rcpdjac + (curved ? (long long)rho * ld : 0) + col, rj);
-#pragma unroll
-      for (int a = 0; a < 3; ++a)
-#pragma unroll
-        for (int i = 0; i < 3; ++i)
-          VecIO<T, EW>::ldg(smats + (curved ? ((long long)(a * 3 + i) * nupts + rho) * ld : (long long)(a * 3 + i) * ld) + col, S[a][i]);
-#pragma unroll
-      for (int j = 0; j < EW; ++j)
-        if (col + j >= neles) rj[j] = T(0);      // padding lanes: zero
-#pragma unroll
-      for (int i = 0; i < 3; ++i)
-#pragma unroll
-        for (int v = 0; v < PV; ++v) {
-          T q[EW];
-#pragma unroll
-          for (int j = 0; j < EW; ++j) q[j] = rj[j] * (S[0][i][j] * t0[v][j] + S[1][i][j] * t1[v][j] + S[2][i][j] * t2[v][j]);
-          VecIO<T, EW>::st(grad + (((long long)i * nupts + rho) * 5 + v) * ld + col, q);
-        }
-    });
+    if (e0 + NE <= neles) {
+      acc.foreach_triple(wc, lane, [&](int t, int rr, int e, T(&t0)[PV][EW], T(&t1)[PV][EW], T(&t2)[PV][EW]) {
+        const int rho = mrow[3 * t][rr];     // alpha = 0 rows are 0..Nu-1
+        if (rho >= 0) point_transform<false, EW>(t0, t1, t2, rho, e0 + e);
+      });
+    } else {
+      acc.foreach_triple(wc, lane, [&](int t, int rr, int e, T(&t0)[PV][EW], T(&t1)[PV][EW], T(&t2)[PV][EW]) {
+        const int rho = mrow[3 * t][rr];
+        if (rho >= 0) point_transform<true, EW>(t0, t1, t2, rho, e0 + e);
+      });
+    }
   }
 };
 
@@ -361,9 +382,9 @@ template <typename T>
 int launch_fused_grad(const PanelOp<T> &op, const EleView<T> &ev, const T *u, const T *c, T *grad, cudaStream_t s) {
   GradArgs<T> a;
   a.op = op;
-  // The L2 prefetch of the epilogue's metric terms pays only in FP64 with per-element terms; with per-point terms (20 lines per
-  // thread) and in FP32 it costs more issue slots than the latency it hides (profiles/r01_j_panel_source_level.md item 7).
-  a.op.pf_epi = (ev.affine && sizeof(T) == 8) ? 1 : 0;
+  // The epilogue's metric terms are pulled into L2 while the panel's first chunk is multiplied; with per-point terms in FP64
+  // (20 lines per thread) the prefetch costs more than the latency it hides (pri S3+S4 0.94 -> 1.04 ms).
+  a.op.pf_epi = (ev.affine || sizeof(T) == 4) ? 1 : 0;
   a.prod.tm[0] = tmap_state(u, (long long)ev.nupts, ev.ld, op.NE, op.src_step[0]);
   a.prod.tm[1] = tmap_state(c, (long long)ev.nfpts, ev.ld, op.NE, op.src_step[1]);
   a.prod.plain = 0;

@@ -224,8 +224,8 @@ __device__ __forceinline__ void panel_mainloop(const PanelOp<T> &op, const Prod 
   for (int q = 0; q < total; ++q) {
     mbar_wait(gbar + stage * 16, phase);
     const char *st = ringp + (size_t)(grp * nstage + stage) * stage_bytes;
-    // the epilogue's own global operands: pull them into L2 while the last chunk is multiplied
-    if (cc == nchunks - 1 && op.pf_epi) epi.prefetch(acc, A.rowmap, wr * NIT, cbatch, cpl, wc, lane);
+    // the epilogue's own global operands: pull them into L2 while the panel is multiplied
+    if (cc == 0 && op.pf_epi) epi.prefetch(acc, A.rowmap, wr * NIT, cbatch, cpl, wc, lane);
 #ifdef FRB_DEBUG_KNOBS
     if (!(op.dbg & 1))
 #endif

@@ -1,6 +1,12 @@
 """GPU parity tests (-m gpu): the CUDA path, called through the C ABI, against the CPU oracle element by
 element on the same seeded inputs.  Tolerances are BASELINE.json north_star's: max-norm relative error per
-conserved variable (reading R16) <= 1e-11 in FP64 and <= 2e-5 in FP32."""
+conserved variable (reading R16) <= 1e-11 in FP64 and <= 2e-5 in FP32 (reading R23 for where FP32 storage of
+the flux arrays alone exceeds 2e-5).  Every right-hand-side comparison appends its achieved error, the 2e-5
+target and the a-priori bound to a CSV (FRB_PARITY_CSV, default gpurun_out/parity_errors.csv), so what the
+kernels achieve can be audited: profiles/r02_parity_errors.md."""
+import csv
+import os
+
 import numpy as np
 import pytest
 
@@ -12,13 +18,37 @@ pytestmark = pytest.mark.gpu
 TOL = {"f64": 1e-11, "f32": 2e-5}
 
 
+R23_FACTOR = 2.0
+
+
 def _tolerance(prec, amp):
     """FP64: 1e-11 (north_star).  FP32: 2e-5 (north_star) wherever FP32 arithmetic can reach it; where the
-    a-priori round-off bound of the last step alone, 6 * 2^-24 * amp_k, is larger (smooth data on fine meshes:
-    the divergence is a small difference of large fluxes), that bound applies -- DESIGN.md reading R23."""
+    a-priori round-off bound of the last step alone, 2 * 2^-24 * amp_k, is larger (smooth data on fine meshes:
+    the divergence is a small difference of large fluxes), that bound applies -- DESIGN.md reading R23.  The factor 2:
+    one rounding of F~ / D when they are stored plus one for the accumulated products of the divergence, each at most
+    2^-24 relative to |M132||F~| + |M3||D|; the roundings upstream of F~ and D (flux evaluation, S1 .. S5) are not counted,
+    so the achieved errors recorded in the CSV are what shows the bound is not slack."""
     if prec == "f64":
         return np.full(5, TOL["f64"])
-    return np.maximum(TOL["f32"], 6 * EPS32 * amp)
+    return np.maximum(TOL["f32"], R23_FACTOR * EPS32 * amp)
+
+
+def _record(prec, mode, err, amp, tol, tag=""):
+    path = os.environ.get("FRB_PARITY_CSV", os.path.join(os.path.dirname(os.path.dirname(os.path.abspath(__file__))), "gpurun_out",
+                                                        "parity_errors.csv"))
+    try:
+        os.makedirs(os.path.dirname(path), exist_ok=True)
+        new = not os.path.exists(path)
+        with open(path, "a", newline="") as f:
+            w = csv.writer(f)
+            if new:
+                w.writerow(["test", "prec", "mode", "variable", "achieved_rel_err", "north_star_tol", "r23_bound", "asserted_tol", "amp"])
+            name = os.environ.get("PYTEST_CURRENT_TEST", "").split("::")[-1].split(" ")[0] + tag
+            for k in range(5):
+                w.writerow([name, prec, mode, k, "%.3e" % err[k], "%.1e" % TOL[prec],
+                            "" if prec == "f64" else "%.3e" % (R23_FACTOR * EPS32 * amp[k]), "%.3e" % tol[k], "%.3e" % amp[k]])
+    except OSError:
+        pass
 
 
 def _ctx(case, prec, mode="fused", stepper="rk45"):
@@ -26,14 +56,19 @@ def _ctx(case, prec, mode="fused", stepper="rk45"):
     return Context(case, prec=prec, mode=mode, stepper=stepper)
 
 
-def _check_rhs(case, prec, mode):
+def _check_rhs(case, prec, mode, tag=""):
+    """FP64: every variable on its own scale.  FP32: the momentum components share one scale (reading R16: a component that
+    vanishes by symmetry has none of its own)."""
     c = round_case_to_f32(case) if prec == "f32" else case
-    ref, amp = oracle_rhs_with_amplification(c)
+    joint = prec == "f32"
+    ref, amp = oracle_rhs_with_amplification(c, joint_momentum=joint)
     ctx = _ctx(case, prec, mode)
     got, raw = gpu_rhs(ctx, case["u0"])
-    err, den = field_errors(got, ref)
+    err, den = field_errors(got, ref, joint_momentum=joint)
+    tol = _tolerance(prec, amp)
+    _record(prec, mode, err, amp, tol, tag)
     assert np.all(np.isfinite(np.concatenate([g.ravel() for g in got])))
-    assert np.all(err <= _tolerance(prec, amp)), (prec, mode, err, _tolerance(prec, amp))
+    assert np.all(err <= tol), (prec, mode, err, tol)
     for r, u in zip(raw, case["u0"]):              # padding columns are written as zero
         assert np.all(r[:, :, u.shape[2]:] == 0)
     ctx.close()
@@ -91,13 +126,37 @@ def test_config2_16cubed_p3_ns(prec):
 @pytest.mark.parametrize("prec", ["f64", "f32"])
 def test_config3_small_cylinder_with_boundaries(prec, mode):
     case = cases.config3(p=2, ntheta=24, nz=4, nlayers=6, nr=6, numbering="random")
-    c = round_case_to_f32(case) if prec == "f32" else case
-    ref, amp = oracle_rhs_with_amplification(c)
-    ctx = _ctx(case, prec, mode)
-    got, _ = gpu_rhs(ctx, case["u0"])
-    err, den = field_errors(got, ref)
     # thin wall prisms (h0 = 1e-3) with a no-slip wall against a Mach-0.2 stream: |dudt| ~ 1e5 at the wall
-    assert np.all(err <= _tolerance(prec, amp)), (err, _tolerance(prec, amp))
+    _check_rhs(case, prec, mode)
+
+
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+def test_supersonic_farfield_parity(prec):
+    """A Mach-1.5 free stream drives the Riemann-invariant far field through its supersonic inflow
+    (upstream half of the outer boundary) and supersonic outflow (downstream half) branches, which the Mach-0.2 cases never reach."""
+    case = cases.config3(p=2, ntheta=24, nz=4, nlayers=6, nr=6, numbering="random", mach=1.5)
+    from oracle import fr_oracle as O
+    far = [b for b in case["bcs"] if b["type"] == "farfield"][0]
+    uf = [O._apply(e["M0"], u) for e, u in zip(case["eles"], case["u0"])]
+    ub = O._gather(uf, far["et"], far["fpt"], far["ele"])
+    vn = (ub[1:4] / ub[0] * far["n"]).sum(0)
+    c = np.sqrt(1.4 * 0.4 * (ub[4] - 0.5 * (ub[1:4] ** 2).sum(0) / ub[0]) / ub[0])
+    assert (vn <= -c).any() and (vn >= c).any() and (np.abs(vn) < c).any()      # all branches occur in this input
+    for mode in ("fused", "unfused"):
+        _check_rhs(case, prec, mode)
+
+
+@pytest.mark.parametrize("mode", ["unfused", "fused"])
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+@pytest.mark.parametrize("beta,tau", [(0.0, 0.0), (-0.5, 1.0), (0.3, 0.1), (0.25, 1.0)])
+def test_ldg_constants_parity(beta, tau, prec, mode):
+    """Other LDG constants than the default beta = 1/2, tau = 0.1 (reading R9): the R-side store of the common solution, the
+    two-sided common viscous flux, and the beta = +-1/2 special cases of the interface kernels."""
+    for p in (2, 3):
+        case = cases.config2(6, p, "ns", numbering="random", ldg_beta=beta, ldg_tau=tau)
+        _check_rhs(case, prec, mode, tag="/p%d" % p)
+    case = cases.config3(p=2, ntheta=24, nz=4, nlayers=6, nr=6, numbering="random", ldg_beta=beta, ldg_tau=tau)
+    _check_rhs(case, prec, mode, tag="/cyl")
 
 
 def test_free_stream_and_empty_boundary_lists_on_gpu():
@@ -238,16 +297,69 @@ def test_config3_full_size_sampled_parity(prec):
 
 
 # ---------------------------------------------------------------------------- every panel geometry the autotuner may pick
-@pytest.mark.parametrize("cand", [1, 2, 3, 4, 5, 6, 8, 10, 13, 1000, 1001, 1003])
+@pytest.mark.parametrize("cand", [1, 2, 3, 4, 5, 6, 8, 10, 13])
 def test_candidate_geometries_parity(cand, monkeypatch):
     """fr_setup times candidate geometries only on large meshes, so the small parity meshes always run candidate 0.  Force
-    candidate `cand` (FRB_FORCE_CAND: geometry index + 1000 for the opposite dense / k-list packing) for every operator and check
-    the right-hand side of the mixed config-2 mesh at p = 4 and p = 2 in both precisions."""
+    candidate `cand` (FRB_FORCE_CAND: index into the list of launch geometries that fit shared memory) for every operator and
+    check the right-hand side of the mixed config-2 mesh at p = 4 and p = 2 in both precisions."""
     monkeypatch.setenv("FRB_FORCE_CAND", str(cand))
     for p in (4, 2):
         case = cases.config2(6, p, "ns", numbering="random")
         for prec in ("f64", "f32"):
-            _check_rhs(case, prec, "fused")
+            _check_rhs(case, prec, "fused", tag="/p%d" % p)
+
+
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+def test_candidate_geometries_bitwise_identical(prec, monkeypatch):
+    """include/frb200.h promises bitwise-identical outputs for identical inputs although fr_setup picks launch geometries by
+    timing: the packing of an operator and the composition of every k-block depend on the operator alone (panel.cuh), so every
+    geometry must give the same bits.  Right-hand side and one RK45 step, candidates 0..13, mixed mesh at p = 4 and p = 3."""
+    for p in (4, 3):
+        case = cases.config2(6, p, "ns", numbering="random")
+        ref_raw = ref_state = None
+        for cand in range(0, 14):
+            monkeypatch.setenv("FRB_FORCE_CAND", str(cand))
+            ctx = _ctx(case, prec, "fused", stepper="rk45")
+            _, raw = gpu_rhs(ctx, case["u0"])
+            ctx.set_state(case["u0"])
+            ctx.rk_step(1e-4)
+            st = ctx.get_state()
+            ctx.close()
+            if ref_raw is None:
+                ref_raw, ref_state = raw, st
+                continue
+            for a, b in zip(raw, ref_raw):
+                assert np.array_equal(a, b), (p, cand)
+            for a, b in zip(st, ref_state):
+                assert np.array_equal(a, b), (p, cand)
+
+
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+def test_rk_step_host_parity(prec):
+    """fr_rk_step_host (the end-to-end call bench.py times: host buffers in the device layout in, one step, host buffers out)
+    against fr_set_state / fr_rk_step / fr_get_state and against the oracle's step."""
+    import torch
+    from oracle import fr_oracle as O
+    case = cases.config2(6, 3, "ns", numbering="random")
+    c = round_case_to_f32(case) if prec == "f32" else case
+    dt = 1e-4
+    ctx = _ctx(case, prec, stepper="rk45")
+    ctx.set_state(case["u0"])
+    ctx.rk_step(dt)
+    want = ctx.get_state()
+    tdt = torch.float64 if prec == "f64" else torch.float32
+    host = []
+    for u, ld in zip(case["u0"], ctx.ld):
+        h = torch.zeros((u.shape[0], 5, ld), dtype=tdt).pin_memory()
+        h[:, :, :u.shape[2]] = torch.from_numpy(u).to(tdt)
+        host.append(h)
+    ctx.rk_step_host(dt, [h.data_ptr() for h in host])
+    for h, w, u in zip(host, want, case["u0"]):
+        assert np.array_equal(h.numpy()[:, :, :u.shape[2]].astype(np.float64), w)
+    ref = O.rk45_step(lambda us: O.rhs(c["cfg"], c["eles"], c["ifc"], c["bcs"], us), c["u0"], dt)
+    num = max(np.abs(a - b).max() for a, b in zip(want, ref))
+    assert num / max(np.abs(b).max() for b in ref) <= (1e-13 if prec == "f64" else 1e-6)
+    ctx.close()
 
 
 # ---------------------------------------------------------------------------- row split of operators too tall for one CTA
@@ -428,4 +540,6 @@ def test_hex_affine_rk45_step():
     ctx.rk_step(1e-4)
     got = ctx.get_state()
     err, _ = field_errors([a - b for a, b in zip(got, case["u0"])], [a - b for a, b in zip(ref, case["u0"])])
-    assert max(err[0], err[1], err[2], err[4]) <= 1e-9, err
+    # the vortex is z-invariant: the increment of rho v_z is round-off, so the momentum components share their scale (reading R16)
+    err, _ = field_errors([a - b for a, b in zip(got, case["u0"])], [a - b for a, b in zip(ref, case["u0"])], joint_momentum=True)
+    assert err.max() <= 1e-9, err
