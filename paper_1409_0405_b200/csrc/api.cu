@@ -1175,8 +1175,13 @@ fr_status fr_gemm_plan_create(int32_t M, int32_t K, const double *A_host, fr_pre
     require_device();
     auto p = std::make_unique<fr_gemm_plan>();
     p->prec = prec;
-    if (prec == FR_F64) frb::gemm_plan_build(p->pd, M, K, A_host, 0.0);
-    else frb::gemm_plan_build(p->pf, M, K, A_host, 0.0);
+    if (prec == FR_F64) {
+      frb::gemm_plan_build(p->pd, M, K, A_host, 0.0);
+      frb::gemm_plan_tune(p->pd, A_host, 0.0);
+    } else {
+      frb::gemm_plan_build(p->pf, M, K, A_host, 0.0);
+      frb::gemm_plan_tune(p->pf, A_host, 0.0);
+    }
     *out = p.release();
   });
 }
@@ -1200,8 +1205,17 @@ void fr_gemm_plan_destroy(fr_gemm_plan *plan) {
 }
 fr_status fr_gemm(int32_t M, int32_t K, int64_t N, double c1, const double *A_host, const void *B_dev, int64_t ldb, double c2,
                   void *C_dev, int64_t ldc, fr_prec prec, void *cuda_stream) {
+  // a one-shot product takes the statically best geometry: timing candidates would cost more than the product
   fr_gemm_plan *p = nullptr;
-  fr_status st = fr_gemm_plan_create(M, K, A_host, prec, &p);
+  fr_status st = guard(nullptr, [&] {
+    FR_REQUIRE(prec == FR_F32 || prec == FR_F64, "prec must be FR_F32 or FR_F64");
+    require_device();
+    auto q = std::make_unique<fr_gemm_plan>();
+    q->prec = prec;
+    if (prec == FR_F64) frb::gemm_plan_build(q->pd, M, K, A_host, 0.0);
+    else frb::gemm_plan_build(q->pf, M, K, A_host, 0.0);
+    p = q.release();
+  });
   if (st != FR_OK) return st;
   st = fr_gemm_plan_run(p, N, c1, B_dev, ldb, c2, C_dev, ldc, cuda_stream);
   if (st == FR_OK) {

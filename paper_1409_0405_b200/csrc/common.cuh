@@ -84,6 +84,9 @@ struct GemmPlan {
 // operators handed to fr_setup); the public fr_gemm passes 0 (only exact zeros are skipped)
 template <typename T>
 void gemm_plan_build(GemmPlan<T> &p, int M, int K, const double *A_host, double drop_rel = 1.4210854715202004e-14);
+// times the plan's launch geometries on scratch matrices and keeps the fastest (fr_gemm_plan_create)
+template <typename T>
+void gemm_plan_tune(GemmPlan<T> &p, const double *A_host, double drop_rel);
 template <typename T>
 void gemm_plan_free(GemmPlan<T> &p);
 // C[b] <- c1 * A * B[b] + c2 * C[b], b < nbatch; returns the number of kernels launched

@@ -333,6 +333,71 @@ void gemm_plan_build(GemmPlan<T> &p, int M, int K, const double *A_host, double 
   FR_CUDA_TRY(cudaMemcpy(p.At, At.data(), At.size() * sizeof(T), cudaMemcpyHostToDevice));
 }
 
+// Time the launch geometries of a plan's panel operator on scratch matrices larger than L2 and keep the fastest (what Ctx::tune
+// does for the operators of fr_setup).  Results do not depend on the choice (panel.cuh).  FRB_AUTOTUNE=0 skips it.
+template <typename T>
+void gemm_plan_tune(GemmPlan<T> &p, const double *A_host, double drop_rel) {
+  const char *env = getenv("FRB_AUTOTUNE");
+  if (env && atoi(env) == 0) return;
+  if (!p.pop && p.nparts == 0) return;
+  const int M = p.pop ? p.M : p.part[0]->M, K = p.K;
+  // columns: 320 MB of B and C, a multiple of 5 * 128
+  long long N = (long long)(320e6 / ((double)(M + K) * sizeof(T)));
+  N = std::max<long long>(640, N / 640 * 640);
+  T *B = nullptr, *Cm = nullptr;
+  if (cudaMalloc(&B, (size_t)K * N * sizeof(T)) != cudaSuccess) return;
+  if (cudaMalloc(&Cm, (size_t)M * N * sizeof(T)) != cudaSuccess) {
+    cudaFree(B);
+    return;
+  }
+  cudaMemset(B, 0, (size_t)K * N * sizeof(T));
+  cudaEvent_t e0, e1;
+  cudaEventCreate(&e0);
+  cudaEventCreate(&e1);
+  auto time_op = [&](const PanelOp<T> &op) {
+    float best = 1e30f;
+    for (int rep = 0; rep < 4; ++rep) {
+      cudaEventRecord(e0, 0);
+      panel_gemm_run(op, N, T(1), B, N, 0, T(0), Cm, N, 0, 1, (cudaStream_t)0);
+      cudaEventRecord(e1, 0);
+      cudaEventSynchronize(e1);
+      float ms = 0;
+      cudaEventElapsedTime(&ms, e0, e1);
+      if (rep > 0) best = std::min(best, ms);
+    }
+    return best;
+  };
+  PanelOp<T> *cur = p.pop ? p.pop : p.part[0];
+  float bt = time_op(*cur);
+  int bestk = 0;
+  const int ncand = getenv("FRB_TUNE_CANDS") ? std::max(1, atoi(getenv("FRB_TUNE_CANDS"))) : 14;
+  for (int k = 1; k < ncand; ++k) {
+    PanelOp<T> op;
+    if (!panel_gemm_build(op, M, K, A_host, k, drop_rel)) break;
+    const float t = time_op(op);
+    if (t < bt) {
+      panel_op_free(*cur);
+      *cur = op;
+      bt = t;
+      bestk = k;
+    } else {
+      panel_op_free(op);
+    }
+  }
+  // row blocks: the other blocks take the same candidate (same shape up to the last block's height)
+  for (int i = 1; i < p.nparts && bestk > 0; ++i) {
+    PanelOp<T> op;
+    if (panel_gemm_build(op, p.part[i]->M, K, A_host + (size_t)p.part_row0[i] * K, bestk, drop_rel)) {
+      panel_op_free(*p.part[i]);
+      *p.part[i] = op;
+    }
+  }
+  cudaEventDestroy(e0);
+  cudaEventDestroy(e1);
+  cudaFree(B);
+  cudaFree(Cm);
+}
+
 template <typename T>
 void gemm_plan_free(GemmPlan<T> &p) {
   if (p.At) cudaFree(p.At);
@@ -397,6 +462,8 @@ int gemm_run(const GemmPlan<T> &p, long long N, T c1, const T *B, long long ldb,
 
 template void gemm_plan_build<double>(GemmPlan<double> &, int, int, const double *, double);
 template void gemm_plan_build<float>(GemmPlan<float> &, int, int, const double *, double);
+template void gemm_plan_tune<double>(GemmPlan<double> &, const double *, double);
+template void gemm_plan_tune<float>(GemmPlan<float> &, const double *, double);
 template void gemm_plan_free<double>(GemmPlan<double> &);
 template void gemm_plan_free<float>(GemmPlan<float> &);
 template int gemm_run<double>(const GemmPlan<double> &, long long, double, const double *, long long, long long, double,

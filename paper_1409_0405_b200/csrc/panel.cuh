@@ -102,13 +102,13 @@ struct PanelGeom {
 // register budget for whole quads of warps, one per SM sub-partition), the largest whose register share still leaves the
 // accumulators 68 registers of head-room (less spills loop-carried scalars, which costs a local-memory round trip per chunk).  FP64: NIT*CX*10 doubles per thread; FP32: NIT*CX*40 floats.
 template <typename T>
-constexpr int panel_maxw(int nit, int cx) {
+constexpr int panel_maxw(int nit, int cx, bool triple = false) {
   // FP32 tiles also keep 8 operator values and 5*CX state values live per k and index more arrays: the CX = 2 shapes spill
   // inside the multiply loop with little head-room (8x slower), so FP32 with CX = 2 budgets +110.
   const int need = (sizeof(T) == 8 ? nit * cx * 20 : nit * cx * 40) + ((sizeof(T) == 4 && cx == 2) ? 110 : 68);
-  // the gradient operators of prisms (10 triples of row groups) need 10 row-warps of NIT = 6 (FP64) / NIT = 3 (FP32): these two
-  // shapes take 12 warps at 168 registers and spill ~150 bytes in the epilogue
-  if ((sizeof(T) == 8 ? nit * cx == 6 : nit * cx == 3)) return 12;
+  // the gradient operators of prisms (10 triples of row groups) need 10 row-warps of NIT = 6 (FP64) / NIT = 3 (FP32): in the
+  // gradient kernels these two shapes take 12 warps at 168 registers and spill ~150 bytes in the epilogue
+  if (triple && (sizeof(T) == 8 ? nit * cx == 6 : nit * cx == 3)) return 12;
   int w = PANEL_MAXW / 4 * 4;
   while (w > 8 && 2048 / w < need) w -= 4;
   return w;
@@ -131,7 +131,7 @@ inline std::vector<PanelGeom> list_geoms(int G, int min_ne, int max_ne, int trip
         for (int CX = 2; CX >= 1; --CX) {
           if (f64 ? nit * CX > 8 : nit * CX > 4) continue;
           const int W = NG * WR * WC;                          // consumer warps
-          if (W + NG > panel_maxw<T>(nit, CX)) continue;
+          if (W + NG > panel_maxw<T>(nit, CX, triple != 0)) continue;
           const int NE = (f64 ? 8 : 32) * CX * WC;
           // panels tile the padded leading dimension (a multiple of 128) exactly; FP64 stages are made of 16-element blocks
           if (NE < min_ne || NE > max_ne || 128 % NE != 0 || (f64 && NE % 16)) continue;
@@ -146,7 +146,7 @@ inline std::vector<PanelGeom> list_geoms(int G, int min_ne, int max_ne, int trip
           all.push_back(PanelGeom{WR, WC, nit, CX, NE, score, NG, 1});
           // two CTAs per SM (half the shared memory and registers each): the other way to overlap one panel's epilogue with
           // another's multiplies; only timing (fr_setup autotuning) tells which wins
-          if (NG == 1 && 2 * (W + 1) <= panel_maxw<T>(nit, CX)) all.push_back(PanelGeom{WR, WC, nit, CX, NE, score * 0.9, NG, 2});
+          if (NG == 1 && 2 * (W + 1) <= panel_maxw<T>(nit, CX, triple != 0)) all.push_back(PanelGeom{WR, WC, nit, CX, NE, score * 0.9, NG, 2});
         }
       }
     }
