@@ -140,9 +140,15 @@ def _apply(A, B):
 
 
 # ----------------------------------------------------------------------------- right-hand side
-def rhs(cfg, eles, ifc, bcs, us, parts=None):
+def rhs(cfg, eles, ifc, bcs, us, parts=None, halo=None):
     """One evaluation of d u / d t, steps 1-6 of SURVEY 8(c).  If `parts` is a dict it receives the
     intermediates `ftil` (F~) and `d` (D) of step 6, for a-priori round-off bounds in the tests.
+
+    halo (domain decomposition: "exchange of interface data between ranks"): dict(et, fpt, ele,
+    exchange).  The flux-point pairs cut by the partition refer to their remote side as flux point 0 of element g of an extra
+    pseudo type with index len(eles); halo['exchange'](name, values [V, n_send]) -> [V, n_ghost] hands the own values at the
+    flux points (et, fpt, ele) to the peers and returns theirs -- once for U_f after step 1 and, for Navier-Stokes, once for the
+    three components of G_f after step 3.  No arithmetic is added: the ghost values enter steps 2 and 5 as any other side.
 
     cfg  : dict(system='euler'|'ns', gamma, mu, prandtl, ldg_beta, ldg_tau)
     eles : per element type dict(M0, M132, M3, M460, M6, smats [3,3,N_u,N_e], rcpdjac [N_u,N_e])
@@ -159,6 +165,9 @@ def rhs(cfg, eles, ifc, bcs, us, parts=None):
 
     # step 1: U_f = M0 U
     uf = [_apply(e["M0"], u) for e, u in zip(eles, us)]
+    if halo is not None:
+        H = (halo["et"], halo["fpt"], halo["ele"])
+        uf.append(halo["exchange"]("u", _gather(uf, *H))[None])          # ghost "type": [1 flux point, 5, n_ghost]
     uL, uR = _gather(uf, *L), _gather(uf, *R)
 
     def bc_states(b):
@@ -192,6 +201,9 @@ def rhs(cfg, eles, ifc, bcs, us, parts=None):
             g = np.stack([rj[:, None, :] * sum(S[a, i][:, None, :] * gt[a] for a in range(3)) for i in range(3)])
             grads.append(g)
             gf.append(np.stack([_apply(e["M0"], g[i]) for i in range(3)]))
+        if halo is not None:
+            own = np.concatenate([_gather([g[i] for g in gf], *H) for i in range(3)])          # [15, n_send]
+            gf.append(halo["exchange"]("g", own).reshape(3, 1, 5, -1))
 
     # step 4: transformed flux F~_alpha = sum_i S[alpha,i] (f^inv_i - f^visc_i)
     ftil = []

@@ -1,0 +1,120 @@
+"""Domain decomposition with halo exchange.
+
+CPU (world_size 2 and 3 over gloo): the partitioner's invariants, and the oracle run rank by rank on the split case with a real
+point-to-point exchange of U_f and G_f, against the oracle on the whole case.
+GPU (-m gpu, one device): the library's partitioned right-hand side (fr_rhs_phase + halo buffers), the ranks' phases launched one
+after the other with device copies standing in for the transport, against the single-context right-hand side bit for bit.
+"""
+import os
+import sys
+
+import numpy as np
+import pytest
+
+from fr_inputs import cases, partition as P
+from util import field_errors, oracle_rhs
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def _case(kind):
+    if kind == "box":
+        return cases.config2(4, 2, "ns", numbering="random", ldg_beta=0.3, ldg_tau=0.1)
+    return cases.config3(p=2, ntheta=16, nz=4, nlayers=4, nr=4, numbering="random")
+
+
+def test_partition_weights_and_split_invariants():
+    case = _case("cyl")
+    for nparts in (2, 3, 4):
+        part = P.partition(case, nparts)
+        w = np.zeros(nparts)
+        for t, pt in zip(case["etypes"], part):
+            w += np.bincount(pt, minlength=nparts) * P.WEIGHT[t]
+        assert w.max() / w.mean() < 1.05                       # weighted balance (hex : pri : tet = 3 : 2 : 1)
+        subs, maps = P.split_case(case, part)
+        # every element on exactly one rank; every flux point of a rank in exactly one pair or boundary list
+        for t, e in enumerate(case["eles"]):
+            ids = np.concatenate([g for mp in maps for (tt, g) in mp if tt == t])
+            assert np.array_equal(np.sort(ids), np.arange(e["neles"]))
+        ncut = 0
+        for r, s in enumerate(subs):
+            gt = len(s["eles"])
+            seen = [np.zeros((e["nfpts"], e["neles"]), dtype=int) for e in s["eles"]]
+            for side in ("l", "r"):
+                for t in range(gt):
+                    m = s["ifc"][side + "_et"] == t
+                    np.add.at(seen[t], (s["ifc"][side + "_fpt"][m], s["ifc"][side + "_ele"][m]), 1)
+            for b in s["bcs"]:
+                for t in range(gt):
+                    m = b["et"] == t
+                    np.add.at(seen[t], (b["fpt"][m], b["ele"][m]), 1)
+            assert all(np.all(x == 1) for x in seen)
+            gl, gr = s["ifc"]["l_et"] == gt, s["ifc"]["r_et"] == gt
+            assert not np.any(gl & gr)
+            g = np.concatenate([s["ifc"]["l_ele"][gl], s["ifc"]["r_ele"][gr]])
+            assert np.array_equal(np.sort(g), np.arange(s["halo"]["nghost"]))      # every ghost referenced exactly once
+            assert sum(p_["count"] for p_ in s["halo"]["peers"]) == s["halo"]["nghost"]
+            ncut += s["halo"]["nghost"]
+            # send counts are symmetric
+            for p_ in s["halo"]["peers"]:
+                back = [q for q in subs[p_["rank"]]["halo"]["peers"] if q["rank"] == r]
+                assert len(back) == 1 and back[0]["count"] == p_["count"]
+        assert ncut % 2 == 0 and ncut > 0
+
+
+def _oracle_worker(rank, world, port, kind, q):
+    import torch
+    import torch.distributed as dist
+    sys.path.insert(0, ROOT)
+    sys.path.insert(0, os.path.join(ROOT, "tests"))
+    from oracle import fr_oracle as O
+    os.environ["MASTER_ADDR"] = "127.0.0.1"
+    os.environ["MASTER_PORT"] = str(port)
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    case = _case(kind)
+    subs, maps = P.split_case(case, P.partition(case, world))
+    s = subs[rank]
+    h = s["halo"]
+
+    def exchange(name, own):
+        # own [V, n_send] in the peers' ghost order; returns [V, n_ghost]
+        out = np.empty_like(own)
+        ops, keep = [], []
+        for p_ in h["peers"]:
+            sl = slice(p_["start"], p_["start"] + p_["count"])
+            snd = torch.from_numpy(np.ascontiguousarray(own[:, sl]))
+            rcv = torch.empty_like(snd)
+            keep.append((sl, rcv))
+            ops += [dist.P2POp(dist.isend, snd, p_["rank"]), dist.P2POp(dist.irecv, rcv, p_["rank"])]
+        for w in dist.batch_isend_irecv(ops):
+            w.wait()
+        for sl, rcv in keep:
+            out[:, sl] = rcv.numpy()
+        return out
+
+    got = O.rhs(s["cfg"], s["eles"], s["ifc"], s["bcs"], s["u0"], halo=dict(et=h["et"], fpt=h["fpt"], ele=h["ele"], exchange=exchange))
+    q.put((rank, got))
+    dist.barrier()
+    dist.destroy_process_group()
+
+
+@pytest.mark.parametrize("kind,world", [("box", 2), ("cyl", 2), ("cyl", 3)])
+def test_partitioned_oracle_equals_whole_domain_oracle_gloo(kind, world):
+    import torch.multiprocessing as mp
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    port = 29500 + (os.getpid() * 7 + world * 13 + len(kind)) % 2000
+    procs = [ctx.Process(target=_oracle_worker, args=(r, world, port, kind, q)) for r in range(world)]
+    for p_ in procs:
+        p_.start()
+    res = dict(q.get(timeout=300) for _ in range(world))
+    for p_ in procs:
+        p_.join(timeout=60)
+        assert p_.exitcode == 0
+    case = _case(kind)
+    _, maps = P.split_case(case, P.partition(case, world))
+    got = P.assemble(case, maps, [res[r] for r in range(world)])
+    ref = oracle_rhs(case)
+    assert all(np.isfinite(g).all() for g in got)
+    err, _ = field_errors(got, ref)
+    assert err.max() < 1e-12, err
