@@ -90,6 +90,18 @@ typedef struct {
   double params[8];
 } fr_bc_desc;
 
+/* Domain decomposition (section 2.5: ranks exchange interface data).  A flux-point pair cut by the partition
+ * names its remote side in fr_iface_desc as element type `netypes` (one past the rank's own types), flux point 0, element g:
+ * "ghost" g, 0 <= g < nghost, each referenced by exactly one pair.  (et, fpt, ele)[g] is the OWN flux point of that same pair,
+ * whose interpolated state (and, for Navier-Stokes, gradient) the peer needs: send entry g and ghost g belong to one cut pair,
+ * so a rank's ghosts of a peer and what it sends to that peer are the same index range, ordered alike on both ranks.
+ * All pointers HOST, borrowed for fr_setup. */
+typedef struct {
+  int64_t nghost;
+  const int32_t *et, *fpt;
+  const int64_t *ele;
+} fr_halo_desc;
+
 typedef struct {
   fr_system system;
   fr_prec prec;
@@ -103,6 +115,7 @@ typedef struct {
   int32_t nbcs;
   const fr_bc_desc *bcs;        /* [nbcs], may be NULL if nbcs == 0 */
   void *cuda_stream;            /* cudaStream_t; NULL = default stream */
+  const fr_halo_desc *halo;     /* NULL: the whole domain is on this GPU */
 } fr_config;
 
 /* Validate, copy to the device, build the interface views.  On failure *out = NULL and
@@ -184,6 +197,24 @@ fr_status fr_check_finite(fr_ctx *ctx, int64_t *n_nonfinite);
 /* The launch plan fr_setup chose (packing, warp grid, panel width, ring depth per operator), one line per operator, as a
  * NUL-terminated string of at most cap - 1 characters.  Results never depend on it (bit-identical for every plan). */
 fr_status fr_plan_describe(const fr_ctx *ctx, char *buf, int64_t cap);
+
+/* Partitioned right-hand side (fr_config.halo): fr_rhs cut at its two exchange points.
+ *   phase 0: S1 (U_f = M0 U), then the own U_f at the cut flux points is packed into the U send buffer;
+ *   phase 1: the received U_f is unpacked into the ghost flux points; S2..S5; the own G_f is packed (Navier-Stokes);
+ *   phase 2: the received G_f is unpacked (Navier-Stokes); S7, S6, S8..S10 -> dudt.
+ * Between the phases the caller moves send buffers into the peers' receive buffers (fr_halo_buffers) on the context's stream --
+ * NCCL send/recv over NVLink through torch.distributed in paper_1409_0405_b200/halo.py.  u_dev / dudt_dev as for fr_rhs (dudt_dev
+ * may be NULL in phases 0 and 1).  Without a halo descriptor phases 0, 1, 2 in a row are exactly fr_rhs. */
+fr_status fr_rhs_phase(fr_ctx *ctx, int32_t phase, const void *const *u_dev, void *const *dudt_dev);
+/* The same for stage `stage` (0-based) of a Runge-Kutta step of size dt on the internal state (S10 fused into phase 2). */
+fr_status fr_rk_stage_phase(fr_ctx *ctx, double dt, int32_t stage, int32_t phase);
+/* Device buffers of the exchange: which = 0 the interpolated state (V = 5 values per flux point), 1 its gradient (V = 15).
+ * Layout of both buffers: for the flux points [start, start + count) exchanged with one peer, value v of flux point start + j
+ * is element V*start + v*count + j -- one contiguous message of V*count values per peer.  *nvalues = V * nghost.
+ * Owned by the context. */
+fr_status fr_halo_buffers(fr_ctx *ctx, int32_t which, void **send_dev, void **recv_dev, int64_t *nvalues);
+/* The peer segmentation the buffers use: (start, count) per peer, in ghost order; must cover [0, nghost) (FR_EINVAL otherwise). */
+fr_status fr_halo_set_peers(fr_ctx *ctx, int32_t npeers, const int64_t *start, const int64_t *count);
 
 /* End-to-end step on HOST buffers: copies u_host[t] (HOST, fr_state_layout layout and the context's precision,
  * ideally pinned) into the solution register, advances one step of size dt, copies the new state back into the

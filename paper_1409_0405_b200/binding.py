@@ -38,12 +38,17 @@ class fr_bc_desc(C.Structure):
                 ("n", _dp), ("mag", _dp), ("params", C.c_double * 8)]
 
 
+class fr_halo_desc(C.Structure):
+    _fields_ = [("nghost", C.c_int64), ("et", _i32p), ("fpt", _i32p), ("ele", _i64p)]
+
+
 class fr_config(C.Structure):
     _fields_ = [("system", C.c_int), ("prec", C.c_int), ("stepper", C.c_int), ("mode", C.c_int),
                 ("gamma", C.c_double), ("mu", C.c_double), ("prandtl", C.c_double),
                 ("ldg_beta", C.c_double), ("ldg_tau", C.c_double),
                 ("netypes", C.c_int32), ("eles", C.POINTER(fr_eles_desc)), ("ifaces", C.POINTER(fr_iface_desc)),
-                ("nbcs", C.c_int32), ("bcs", C.POINTER(fr_bc_desc)), ("cuda_stream", C.c_void_p)]
+                ("nbcs", C.c_int32), ("bcs", C.POINTER(fr_bc_desc)), ("cuda_stream", C.c_void_p),
+                ("halo", C.POINTER(fr_halo_desc))]
 
 
 class fr_kernel_stat(C.Structure):
@@ -59,7 +64,8 @@ SYMBOLS = ["fr_profile_kernels", "fr_rk_step_host", "fr_setup", "fr_state_layout
            "fr_rk_adaptive_run",
            "fr_sync", "fr_launch_count", "fr_profile_rhs", "fr_last_error", "fr_global_error", "fr_destroy",
            "fr_gemm", "fr_gemm_plan_create", "fr_gemm_plan_run", "fr_gemm_plan_destroy", "fr_probe_peaks", "fr_probe_dmma",
-           "fr_profile_stage_kernels", "fr_check_finite", "fr_plan_describe"]
+           "fr_profile_stage_kernels", "fr_check_finite", "fr_plan_describe", "fr_rhs_phase", "fr_rk_stage_phase",
+           "fr_halo_buffers", "fr_halo_set_peers"]
 
 _lib = None
 
@@ -106,6 +112,10 @@ def load():
     lib.fr_profile_stage_kernels.argtypes = [vp, C.c_int32, C.POINTER(fr_kernel_stat), C.c_int32, _i32p]
     lib.fr_check_finite.argtypes = [vp, _i64p]
     lib.fr_plan_describe.argtypes = [vp, C.c_char_p, C.c_int64]
+    lib.fr_rhs_phase.argtypes = [vp, C.c_int32, C.POINTER(vp), C.POINTER(vp)]
+    lib.fr_rk_stage_phase.argtypes = [vp, C.c_double, C.c_int32, C.c_int32]
+    lib.fr_halo_buffers.argtypes = [vp, C.c_int32, C.POINTER(vp), C.POINTER(vp), _i64p]
+    lib.fr_halo_set_peers.argtypes = [vp, C.c_int32, _i64p, _i64p]
     _lib = lib
     return lib
 
@@ -183,6 +193,16 @@ class Context:
         cfg.netypes, cfg.eles, cfg.ifaces = ne, eles, C.pointer(fd)
         cfg.nbcs, cfg.bcs = nb, bcs
         cfg.cuda_stream = C.c_void_p(stream)
+        self.halo = case.get("halo")
+        if self.halo is not None:
+            hd = fr_halo_desc()
+            hd.nghost = int(self.halo["nghost"])
+            for k, t, ct in (("et", np.int32, _i32p), ("fpt", np.int32, _i32p), ("ele", np.int64, _i64p)):
+                a = np.ascontiguousarray(self.halo[k], dtype=t)
+                self._keep.append(a)
+                setattr(hd, k, _ptr(a, ct))
+            self._keep.append(hd)
+            cfg.halo = C.pointer(hd)
         self.prec = prec
         self.dtype = np.float64 if prec == "f64" else np.float32
         self.netypes = ne
@@ -193,6 +213,10 @@ class Context:
         if st != FR_OK:
             raise FrError(st, lib.fr_global_error().decode())
         self._h = h
+        if self.halo is not None:
+            st_ = np.ascontiguousarray([p_["start"] for p_ in self.halo["peers"]], dtype=np.int64)
+            ct_ = np.ascontiguousarray([p_["count"] for p_ in self.halo["peers"]], dtype=np.int64)
+            self._check(lib.fr_halo_set_peers(h, len(st_), _ptr(st_, _i64p), _ptr(ct_, _i64p)))
         self.ld = []
         self.nbytes = []
         for t in range(ne):
@@ -260,6 +284,22 @@ class Context:
         self._check(self._lib.fr_profile_kernels(self._h, reps, arr, cap, C.byref(n)))
         return [dict(name=arr[i].name.decode(), ms=arr[i].ms, alg_bytes=arr[i].alg_bytes, flops=arr[i].flops,
                      category=arr[i].category) for i in range(min(n.value, cap))]
+
+    def rhs_phase(self, phase, u_ptrs, dudt_ptrs=None):
+        """fr_rhs_phase: phase 0, 1 or 2 of the partitioned right-hand side (the caller exchanges the halo buffers in between)."""
+        n = self.netypes
+        u = (C.c_void_p * n)(*[C.c_void_p(int(p)) for p in u_ptrs])
+        d = (C.c_void_p * n)(*[C.c_void_p(int(p)) for p in dudt_ptrs]) if dudt_ptrs is not None else None
+        self._check(self._lib.fr_rhs_phase(self._h, int(phase), u, d))
+
+    def rk_stage_phase(self, dt, stage, phase):
+        self._check(self._lib.fr_rk_stage_phase(self._h, float(dt), int(stage), int(phase)))
+
+    def halo_buffers(self, which):
+        """(send pointer, receive pointer, number of values) of the U_f (which = 0) or G_f (which = 1) exchange buffers."""
+        s_, r_, n = C.c_void_p(), C.c_void_p(), C.c_int64()
+        self._check(self._lib.fr_halo_buffers(self._h, int(which), C.byref(s_), C.byref(r_), C.byref(n)))
+        return s_.value or 0, r_.value or 0, int(n.value)
 
     def profile_stage_kernels(self, reps=5, cap=64):
         """fr_profile_stage_kernels: the per-kernel breakdown of the right-hand side as an RK stage runs it."""

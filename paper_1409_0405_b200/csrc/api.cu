@@ -33,6 +33,10 @@ struct CtxBase {
   virtual void sync() = 0;
   virtual void profile(int reps, double ms[4], fr_kernel_stat *out, int cap, int *n, bool stage = false) = 0;
   virtual long long check_finite() = 0;
+  virtual void rhs_phase(int phase, const void *const *u, void *const *dudt) = 0;
+  virtual void rk_stage_phase(double dt, int stage, int phase) = 0;
+  virtual void halo_buffers(int which, void **send, void **recv, int64_t *n) = 0;
+  virtual void halo_set_peers(int npeers, const int64_t *start, const int64_t *count) = 0;
   virtual std::string describe() const = 0;
   virtual void rk_step_host(double dt, void *const *u_host) = 0;
   virtual void rk_adaptive(double t0, double t1, double dt0, double atol, double rtol, long long max_attempts, fr_adapt_stats *st,
@@ -184,6 +188,12 @@ struct Ctx : CtxBase {
   DevBuf<double> err_partial, err_dev;      // [nt * rk_err_blocks()], [1 + 2]: sum of squares, then {atol, rtol}
   double *err_host = nullptr;               // pinned: [0] sum of squares read back, [1..2] staging of {atol, rtol}
   double tol_set[2] = {-1.0, -1.0};
+  // domain decomposition (fr_config.halo): the remote sides of cut pairs live in a ghost pseudo type (index nt) of the flat
+  // flux-point arrays; own values at the cut flux points travel through the send / receive buffers
+  long long nghost = 0;
+  HaloView hv{};
+  DevBuf<long long> h_offu, h_offg, h_ld, h_gcomp, h_pstart, h_pcnt, h_pj;
+  DevBuf<T> h_send[2], h_recv[2];
   int cmask = 0;                            // phases that run one branch per element type (run_rhs; FRB_CONCURRENT=mask, 0: one stream)
   std::vector<cudaStream_t> aux;
   std::vector<cudaEvent_t> ev_type;
@@ -303,6 +313,18 @@ struct Ctx : CtxBase {
       el.push_back(std::move(e));
     }
     for (int t = nt; t < FR_MAXTYPES; ++t) tt.ubase[t] = tt.gbase[t] = tt.ld[t] = tt.gcomp[t] = 0;
+    if (c->halo && c->halo->nghost > 0) {
+      FR_REQUIRE(nt < FR_MAXTYPES, "a halo needs a free element-type slot (at most 3 element types per rank)");
+      FR_REQUIRE(c->halo->et && c->halo->fpt && c->halo->ele, "halo arrays must be non-NULL");
+      nghost = c->halo->nghost;
+      const long long ldg = (nghost + 127) / 128 * 128;
+      tt.ubase[nt] = utot;
+      tt.gbase[nt] = gtot;
+      tt.ld[nt] = ldg;
+      tt.gcomp[nt] = 5 * ldg;                 // one flux point per ghost "element"
+      utot += 5 * ldg;
+      gtot += 15 * ldg;
+    }
     if (mode == FR_MODE_FUSED && ns) {
       // the jump formulation of S2 needs every type on the fused gradient kernel; otherwise fall back to C itself
       bool all = true;
@@ -430,7 +452,14 @@ struct Ctx : CtxBase {
     // every (type, element, flux point) exactly once across pairs and boundaries
     std::vector<std::vector<uint8_t>> seen(nt);
     for (int t = 0; t < nt; ++t) seen[t].assign(((size_t)el[t]->view.nfpts * el[t]->view.neles + 7) / 8, 0);
+    std::vector<uint8_t> gseen((size_t)nghost, 0);
     auto visit = [&](int t, long long e, int s) {
+      if (t == nt && nghost > 0) {           // the remote side of a cut pair
+        FR_REQUIRE(s == 0 && e >= 0 && e < nghost, "ghost reference out of range");
+        FR_REQUIRE(!gseen[(size_t)e], "a ghost is referenced more than once");
+        gseen[(size_t)e] = 1;
+        return;
+      }
       FR_REQUIRE(t >= 0 && t < nt, "flux-point reference: element type out of range");
       FR_REQUIRE(e >= 0 && e < el[t]->view.neles && s >= 0 && s < el[t]->view.nfpts,
                  "flux-point reference: element or flux point out of range");
@@ -455,6 +484,40 @@ struct Ctx : CtxBase {
       size_t cnt = 0;
       for (uint8_t b : seen[t]) cnt += __builtin_popcount(b);
       FR_REQUIRE(cnt == nbits, "unpaired flux points: every flux point must appear in a pair or a boundary list");
+    }
+    for (long long g = 0; g < nghost; ++g) FR_REQUIRE(gseen[(size_t)g], "every ghost must be the remote side of exactly one pair");
+    if (nghost > 0) {
+      // the own side of every cut pair: where its U_f and G_f sit in the flat arrays
+      const fr_halo_desc &h = *c->halo;
+      std::vector<long long> ou(nghost), og(nghost), hl(nghost), hg(nghost), ps(nghost, 0), pc(nghost, nghost), pj(nghost);
+      for (long long g = 0; g < nghost; ++g) {
+        const int t = h.et[g];
+        FR_REQUIRE(t >= 0 && t < nt && h.ele[g] >= 0 && h.ele[g] < el[t]->view.neles && h.fpt[g] >= 0 && h.fpt[g] < el[t]->view.nfpts,
+                   "halo send entry out of range");
+        const size_t bit = (size_t)h.fpt[g] * el[t]->view.neles + h.ele[g];
+        FR_REQUIRE(seen[t][bit >> 3] & (1u << (bit & 7)), "halo send entry is not a flux point of this rank");
+        const long long rel = (long long)h.fpt[g] * 5 * tt.ld[t] + h.ele[g];
+        ou[g] = tt.ubase[t] + rel;
+        og[g] = tt.gbase[t] + rel;
+        hl[g] = tt.ld[t];
+        hg[g] = tt.gcomp[t];
+        pj[g] = g;
+      }
+      h_offu.upload(ou);
+      h_offg.upload(og);
+      h_ld.upload(hl);
+      h_gcomp.upload(hg);
+      h_pstart.upload(ps);
+      h_pcnt.upload(pc);
+      h_pj.upload(pj);
+      hv = HaloView{nghost, h_offu.p, h_offg.p, h_ld.p, h_gcomp.p, h_pstart.p, h_pcnt.p, h_pj.p,
+                    tt.ubase[nt], tt.gbase[nt], tt.ld[nt], tt.gcomp[nt]};
+      h_send[0].alloc((size_t)5 * nghost);
+      h_recv[0].alloc((size_t)5 * nghost);
+      if (ph.ns) {
+        h_send[1].alloc((size_t)15 * nghost);
+        h_recv[1].alloc((size_t)15 * nghost);
+      }
     }
     // Pairs sorted by (type_L, block of kIfaceBlock consecutive e_L, sigma_L, e_L): inside a block the L side is read and written
     // in coalesced runs, and all flux points of a neighbourhood of elements are visited within a short time window, so the 32-byte
@@ -521,7 +584,9 @@ struct Ctx : CtxBase {
 
   // ------------------------------------------------------------------ one RHS evaluation (S1..S9/S10)
   // u[t]: stage input; sa[t]: what the last kernel of type t writes.  Returns kernels launched.
-  int run_rhs(const T *const *u, const StageArgs<T> *sa, Timeline *tl) {
+  // mask: which of the three phases between the halo exchanges run (include/frb200.h fr_rhs_phase); 7 = the whole right-hand side.
+  // With a halo, a whole evaluation in one call is only meaningful when the caller has filled the receive buffers some other way.
+  int run_rhs(const T *const *u, const StageArgs<T> *sa, Timeline *tl, int mask = 7) {
     int nk = 0;
     cudaStream_t s = stream;
     const bool ns = ph.ns;
@@ -614,7 +679,7 @@ struct Ctx : CtxBase {
       const double extra = sa[t].coef ? (sa[t].out2 ? 20 : 10) : 5;
       mark(CAT_PW, t, sa[t].coef ? "S9_S10_negdiv_rk" : "S9_negdivconf", ((5 + extra) * nu + nmet) * n, 5 * nu * n * (sa[t].coef ? 5 : 1));
     };
-    if (!tl && cmask && nt > 1) {
+    if (!tl && cmask && nt > 1 && mask == 7 && !nghost) {
       // The element types' chains are independent between the interface kernels (which read and write every type's flux
       // points): a phase whose bit is set in cmask runs one branch per type (1: S1, 2: S3..S5, 4: S6 beside S7, 8: S8..S10),
       // the interface kernels stay on the caller's stream.  Under capture the events become the edges of the step's graph.
@@ -661,15 +726,25 @@ struct Ctx : CtxBase {
         for (int t = 0; t < nt; ++t) wait(s, ev_type[t]);
       return nk;
     }
-    for (int t = 0; t < nt; ++t) do_S1(t, s);
-    if (ns) {
-      do_S2();
-      for (int t = 0; t < nt; ++t) do_grad(t, s);
+    if (mask & 1) {
+      for (int t = 0; t < nt; ++t) do_S1(t, s);
+      if (nghost) nk += launch_halo_pack(hv, 0, (const T *)uf.p, h_send[0].p, s);
     }
-    do_S7();
-    for (int t = 0; t < nt; ++t) {
-      do_S6(t, s);
-      do_div(t, s);
+    if (mask & 2) {
+      if (nghost) nk += launch_halo_unpack(hv, 0, (const T *)h_recv[0].p, uf.p, s);
+      if (ns) {
+        do_S2();
+        for (int t = 0; t < nt; ++t) do_grad(t, s);
+        if (nghost) nk += launch_halo_pack(hv, 1, (const T *)gf.p, h_send[1].p, s);
+      }
+    }
+    if (mask & 4) {
+      if (nghost && ns) nk += launch_halo_unpack(hv, 1, (const T *)h_recv[1].p, gf.p, s);
+      do_S7();
+      for (int t = 0; t < nt; ++t) {
+        do_S6(t, s);
+        do_div(t, s);
+      }
     }
     return nk;
   }
@@ -759,27 +834,91 @@ struct Ctx : CtxBase {
                                         -1563879915014.0 / 6823010717585.0, 606302364029.0 / 971179775848.0,
                                         1097981568119.0 / 3980877426909.0};
 
+  // stage input and fused stage update of stage i (S10 of SURVEY 8(a))
+  void stage_args(int i, bool adaptive, std::vector<const T *> &up, std::vector<StageArgs<T>> &sa) {
+    const int S = nstages();
+    for (int t = 0; t < nt; ++t) {
+      EleData<T> &e = *el[t];
+      up[t] = i == 0 ? e.X.p : e.Y.p;
+      const StageCoef *c = coef.p + i;
+      if (stepper == FR_RK4) {
+        if (i == 0) sa[t] = StageArgs<T>{c, e.X.p, e.X.p, e.ACC.p, e.Y.p};
+        else if (i < 3) sa[t] = StageArgs<T>{c, e.ACC.p, e.X.p, e.ACC.p, e.Y.p};
+        else sa[t] = StageArgs<T>{c, e.ACC.p, nullptr, e.X.p, nullptr};
+      } else if (stepper == FR_EULER1) {
+        sa[t] = StageArgs<T>{c, e.X.p, nullptr, e.X.p, nullptr};
+      } else {
+        // adaptive: the last stage writes Y_5 = X_4 + dt a_5 K_5 = X_4 too, for the error estimate
+        sa[t] = StageArgs<T>{c, e.X.p, e.X.p, e.X.p, (i < S - 1 || adaptive) ? e.Y.p : nullptr};
+      }
+    }
+  }
+
+  void rhs_phase(int phase, const void *const *u, void *const *dudt) override {
+    FR_REQUIRE(phase >= 0 && phase <= 2, "phase must be 0, 1 or 2");
+    FR_REQUIRE(u && (dudt || phase < 2), "u_dev must be non-NULL (and dudt_dev in phase 2)");
+    std::vector<const T *> up(nt);
+    std::vector<StageArgs<T>> sa(nt);
+    for (int t = 0; t < nt; ++t) {
+      FR_REQUIRE(u[t] && ((uintptr_t)u[t] % 16) == 0, "state pointers must be non-NULL and 16-byte aligned");
+      up[t] = (const T *)u[t];
+      T *o = (phase == 2) ? (T *)dudt[t] : nullptr;
+      FR_REQUIRE(phase < 2 || (o && (const T *)o != up[t] && ((uintptr_t)o % 16) == 0), "dudt pointers must be non-NULL, aligned and must not alias u");
+      sa[t] = StageArgs<T>{nullptr, nullptr, nullptr, o, nullptr};
+    }
+    launches += run_rhs(up.data(), sa.data(), nullptr, 1 << phase);
+  }
+
+  void rk_stage_phase(double dt, int stage, int phase) override {
+    FR_REQUIRE(std::isfinite(dt), "dt must be finite");
+    FR_REQUIRE(stage >= 0 && stage < nstages() && phase >= 0 && phase <= 2, "stage or phase out of range");
+    if (!(dt == coef_dt)) {
+      FR_CUDA_TRY(cudaStreamSynchronize(stream));
+      fill_coefs(dt);
+      FR_CUDA_TRY(cudaMemcpyAsync(coef.p, coef_host, 8 * sizeof(StageCoef), cudaMemcpyHostToDevice, stream));
+      coef_dt = dt;
+    }
+    std::vector<const T *> up(nt);
+    std::vector<StageArgs<T>> sa(nt);
+    stage_args(stage, false, up, sa);
+    launches += run_rhs(up.data(), sa.data(), nullptr, 1 << phase);
+  }
+
+  void halo_buffers(int which, void **send, void **recv, int64_t *n) override {
+    FR_REQUIRE(which == 0 || which == 1, "which must be 0 (state) or 1 (gradient)");
+    if (send) *send = h_send[which].p;
+    if (recv) *recv = h_recv[which].p;
+    if (n) *n = (int64_t)h_send[which].n;
+  }
+
+  void halo_set_peers(int npeers, const int64_t *start, const int64_t *count) override {
+    FR_REQUIRE(nghost > 0, "the context has no halo");
+    FR_REQUIRE(npeers > 0 && start && count, "peer arrays must be non-NULL");
+    std::vector<long long> ps(nghost), pc(nghost), pj(nghost);
+    long long next = 0;
+    for (int p = 0; p < npeers; ++p) {
+      FR_REQUIRE(start[p] == next && count[p] > 0, "peer segments must tile [0, nghost) in order");
+      for (long long j = 0; j < count[p]; ++j) {
+        ps[next + j] = start[p];
+        pc[next + j] = count[p];
+        pj[next + j] = j;
+      }
+      next += count[p];
+    }
+    FR_REQUIRE(next == nghost, "peer segments must cover every ghost");
+    FR_CUDA_TRY(cudaStreamSynchronize(stream));
+    FR_CUDA_TRY(cudaMemcpy(h_pstart.p, ps.data(), ps.size() * sizeof(long long), cudaMemcpyHostToDevice));
+    FR_CUDA_TRY(cudaMemcpy(h_pcnt.p, pc.data(), pc.size() * sizeof(long long), cudaMemcpyHostToDevice));
+    FR_CUDA_TRY(cudaMemcpy(h_pj.p, pj.data(), pj.size() * sizeof(long long), cudaMemcpyHostToDevice));
+  }
+
   int enqueue_step(bool adaptive = false) {
     int nk = 0;
     const int S = nstages();
     std::vector<const T *> up(nt);
     std::vector<StageArgs<T>> sa(nt);
     for (int i = 0; i < S; ++i) {
-      for (int t = 0; t < nt; ++t) {
-        EleData<T> &e = *el[t];
-        up[t] = i == 0 ? e.X.p : e.Y.p;
-        const StageCoef *c = coef.p + i;
-        if (stepper == FR_RK4) {
-          if (i == 0) sa[t] = StageArgs<T>{c, e.X.p, e.X.p, e.ACC.p, e.Y.p};
-          else if (i < 3) sa[t] = StageArgs<T>{c, e.ACC.p, e.X.p, e.ACC.p, e.Y.p};
-          else sa[t] = StageArgs<T>{c, e.ACC.p, nullptr, e.X.p, nullptr};
-        } else if (stepper == FR_EULER1) {
-          sa[t] = StageArgs<T>{c, e.X.p, nullptr, e.X.p, nullptr};
-        } else {
-          // adaptive: the last stage writes Y_5 = X_4 + dt a_5 K_5 = X_4 too, for the error estimate
-          sa[t] = StageArgs<T>{c, e.X.p, e.X.p, e.X.p, (i < S - 1 || adaptive) ? e.Y.p : nullptr};
-        }
-      }
+      stage_args(i, adaptive, up, sa);
       nk += run_rhs(up.data(), sa.data(), nullptr);
       if (adaptive) {
         // dt (b_i - bhat_i) K_i = g_i (Y_i - X_i)  (rk_adapt.cu)
@@ -1156,6 +1295,16 @@ fr_status fr_plan_describe(const fr_ctx *ctx, char *buf, int64_t cap) {
     memcpy(buf, d.data(), nc);
     buf[nc] = 0;
   });
+}
+fr_status fr_rhs_phase(fr_ctx *ctx, int32_t phase, const void *const *u_dev, void *const *dudt_dev) {
+  FR_CTX_CALL(ctx, ctx->impl->rhs_phase(phase, u_dev, dudt_dev));
+}
+fr_status fr_rk_stage_phase(fr_ctx *ctx, double dt, int32_t stage, int32_t phase) { FR_CTX_CALL(ctx, ctx->impl->rk_stage_phase(dt, stage, phase)); }
+fr_status fr_halo_buffers(fr_ctx *ctx, int32_t which, void **send_dev, void **recv_dev, int64_t *nvalues) {
+  FR_CTX_CALL(ctx, ctx->impl->halo_buffers(which, send_dev, recv_dev, nvalues));
+}
+fr_status fr_halo_set_peers(fr_ctx *ctx, int32_t npeers, const int64_t *start, const int64_t *count) {
+  FR_CTX_CALL(ctx, ctx->impl->halo_set_peers(npeers, start, count));
 }
 fr_status fr_rk_step_host(fr_ctx *ctx, double dt, void *const *u_host) { FR_CTX_CALL(ctx, ctx->impl->rk_step_host(dt, u_host)); }
 int64_t fr_launch_count(const fr_ctx *ctx) { return ctx && ctx->impl ? ctx->impl->launches : 0; }

@@ -58,6 +58,20 @@ template <typename T>
 int launch_bc_comm_flux(const BndView<T> &bv, const TypeTab &tt, T *uf, const T *gf, const PhysParams<T> &ph,
                         cudaStream_t s);
 
+// Halo exchange (include/frb200.h fr_halo_desc): gather the own values at the cut flux points into the send
+// buffer / scatter the received values into the ghost flux points.  Entry i: own flux point at src[off[i] + c*gcomp[i] + v*ld[i]]
+// (c < ncomp components of 5 variables), buffer element (5*ncomp)*pstart[i] + (5*c + v)*pcnt[i] + pj[i].
+struct HaloView {
+  long long n;
+  const long long *off_u, *off_g, *ld, *gcomp;   // own side of every cut pair
+  const long long *pstart, *pcnt, *pj;           // peer segment of entry i and its position in it
+  long long ghost_u, ghost_g, ghost_ld, ghost_gcomp;   // the ghost pseudo type in the flat flux-point arrays
+};
+template <typename T>
+int launch_halo_pack(const HaloView &hv, int which, const T *src, T *send, cudaStream_t s);
+template <typename T>
+int launch_halo_unpack(const HaloView &hv, int which, const T *recv, T *dst, cudaStream_t s);
+
 // Embedded error estimate of RK45[2R+] and its norm (rk_adapt.cu)
 int rk_err_blocks();
 template <typename T>

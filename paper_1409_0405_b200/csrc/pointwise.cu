@@ -324,6 +324,44 @@ int launch_bc_comm_flux(const BndView<T> &bv, const TypeTab &tt, T *uf, const T 
   return 1;
 }
 
+// ---- halo exchange: pack the own values at the cut flux points / unpack the received ones into the ghost flux points
+template <typename T>
+__global__ void __launch_bounds__(PW_BLOCK) k_halo_pack(HaloView hv, int ncomp, const T *__restrict__ src, T *__restrict__ send) {
+  const long long i = (long long)blockIdx.x * PW_BLOCK + threadIdx.x;
+  if (i >= hv.n) return;
+  const long long off = ncomp == 1 ? hv.off_u[i] : hv.off_g[i], ld = hv.ld[i], gc = hv.gcomp[i];
+  const long long cnt = hv.pcnt[i];
+  T *d = send + 5ll * ncomp * hv.pstart[i] + hv.pj[i];
+  for (int c = 0; c < ncomp; ++c)
+#pragma unroll
+    for (int v = 0; v < 5; ++v) d[(5 * c + v) * cnt] = src[off + c * gc + v * ld];
+}
+template <typename T>
+__global__ void __launch_bounds__(PW_BLOCK) k_halo_unpack(HaloView hv, int ncomp, const T *__restrict__ recv, T *__restrict__ dst) {
+  const long long i = (long long)blockIdx.x * PW_BLOCK + threadIdx.x;
+  if (i >= hv.n) return;
+  const long long cnt = hv.pcnt[i];
+  const T *r = recv + 5ll * ncomp * hv.pstart[i] + hv.pj[i];
+  T *d = dst + (ncomp == 1 ? hv.ghost_u : hv.ghost_g) + i;
+  for (int c = 0; c < ncomp; ++c)
+#pragma unroll
+    for (int v = 0; v < 5; ++v) d[c * hv.ghost_gcomp + v * hv.ghost_ld] = r[(5 * c + v) * cnt];
+}
+template <typename T>
+int launch_halo_pack(const HaloView &hv, int which, const T *src, T *send, cudaStream_t s) {
+  if (hv.n == 0) return 0;
+  k_halo_pack<T><<<(unsigned)((hv.n + PW_BLOCK - 1) / PW_BLOCK), PW_BLOCK, 0, s>>>(hv, which ? 3 : 1, src, send);
+  FR_CUDA_TRY(cudaGetLastError());
+  return 1;
+}
+template <typename T>
+int launch_halo_unpack(const HaloView &hv, int which, const T *recv, T *dst, cudaStream_t s) {
+  if (hv.n == 0) return 0;
+  k_halo_unpack<T><<<(unsigned)((hv.n + PW_BLOCK - 1) / PW_BLOCK), PW_BLOCK, 0, s>>>(hv, which ? 3 : 1, recv, dst);
+  FR_CUDA_TRY(cudaGetLastError());
+  return 1;
+}
+
 #define FR_INST(T)                                                                                              \
   template int launch_tdisf<T>(const EleView<T> &, const T *, T *, const PhysParams<T> &, cudaStream_t);       \
   template int launch_gradcoru<T>(const EleView<T> &, T *, cudaStream_t);                                      \
@@ -333,7 +371,9 @@ int launch_bc_comm_flux(const BndView<T> &bv, const TypeTab &tt, T *uf, const T 
                                    cudaStream_t);                                                               \
   template int launch_bc_con_u<T>(const BndView<T> &, const TypeTab &, const T *, T *, T, int, cudaStream_t);       \
   template int launch_bc_comm_flux<T>(const BndView<T> &, const TypeTab &, T *, const T *, const PhysParams<T> &, \
-                                      cudaStream_t);
+                                      cudaStream_t);                                                            \
+  template int launch_halo_pack<T>(const HaloView &, int, const T *, T *, cudaStream_t);                       \
+  template int launch_halo_unpack<T>(const HaloView &, int, const T *, T *, cudaStream_t);
 FR_INST(double)
 FR_INST(float)
 

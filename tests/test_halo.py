@@ -118,3 +118,63 @@ def test_partitioned_oracle_equals_whole_domain_oracle_gloo(kind, world):
     assert all(np.isfinite(g).all() for g in got)
     err, _ = field_errors(got, ref)
     assert err.max() < 1e-12, err
+
+
+# ---------------------------------------------------------------------------- the library's partitioned path, one device
+@pytest.mark.gpu
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+@pytest.mark.parametrize("kind,world", [("box", 2), ("cyl", 2), ("cyl", 3)])
+def test_partitioned_gpu_rhs_and_step_equal_single_context_bitwise(kind, world, prec):
+    """Every rank's part as its own context on the one device; the ranks' phases are launched one after the other and device
+    copies stand in for the NCCL transfers (paper_1409_0405_b200.halo.local_exchange).  The assembled right-hand side and the
+    state after one RK45[2R+] step must equal the single-context results bit for bit (the arithmetic per column and per
+    flux-point pair is the same; only where the data lives differs), and the oracle within the parity tolerance."""
+    import torch
+    from gpu_util import gpu_rhs, round_case_to_f32, to_device
+    from paper_1409_0405_b200 import Context, halo as H
+    case = _case(kind)
+    whole = Context(case, prec=prec, stepper="rk45")
+    got_whole, _ = gpu_rhs(whole, case["u0"])
+    dt = 1e-4 if kind == "box" else 1e-6
+    whole.set_state(case["u0"])
+    whole.rk_step(dt)
+    st_whole = whole.get_state()
+    assert all(np.isfinite(x).all() for x in st_whole)
+    whole.close()
+    subs, maps = P.split_case(case, P.partition(case, world))
+    ctxs = [Context(s, prec=prec, stepper="rk45") for s in subs]
+    xchs = [H.HaloExchange(c) for c in ctxs]
+    d_u = [to_device(c, s["u0"]) for c, s in zip(ctxs, subs)]
+    d_out = [[torch.full_like(t, float("nan")) for t in du] for du in d_u]
+    up = [[t.data_ptr() for t in du] for du in d_u]
+    op = [[t.data_ptr() for t in do] for do in d_out]
+    for ph in range(3):
+        for c, u, o in zip(ctxs, up, op):
+            c.rhs_phase(ph, u, o if ph == 2 else None)
+        torch.cuda.synchronize()
+        if ph < 2:
+            H.local_exchange(xchs, ph)
+            torch.cuda.synchronize()
+    parts = [[t.cpu().numpy().astype(np.float64)[:, :, :u.shape[2]] for t, u in zip(do, s["u0"])] for do, s in zip(d_out, subs)]
+    got = P.assemble(case, maps, parts)
+    for a, b in zip(got, got_whole):
+        assert np.array_equal(a, b)
+    c = round_case_to_f32(case) if prec == "f32" else case
+    err, _ = field_errors(got, oracle_rhs(c), joint_momentum=prec == "f32")
+    assert err.max() < (1e-11 if prec == "f64" else 2e-4), err
+    # one RK45[2R+] step on the internal states
+    for cx, s in zip(ctxs, subs):
+        cx.set_state(s["u0"])
+    for i in range(5):
+        for ph in range(3):
+            for cx in ctxs:
+                cx.rk_stage_phase(dt, i, ph)
+            torch.cuda.synchronize()
+            if ph < 2:
+                H.local_exchange(xchs, ph)
+                torch.cuda.synchronize()
+    st = P.assemble(case, maps, [cx.get_state() for cx in ctxs])
+    for a, b in zip(st, st_whole):
+        assert np.array_equal(a, b)
+    for cx in ctxs:
+        cx.close()
