@@ -350,6 +350,7 @@ struct Ctx : CtxBase {
     if (mode == FR_MODE_FUSED) autotune(c);
     coef.alloc(8);
     FR_CUDA_TRY(cudaMallocHost(&coef_host, 8 * sizeof(StageCoef)));
+    for (int i = 0; i < 8; ++i) coef_host[i] = StageCoef{0.0, 0.0};
     FR_CUDA_TRY(cudaDeviceSynchronize());
   }
 
@@ -1047,7 +1048,8 @@ struct Ctx : CtxBase {
       coef_dt = dt;
     }
     if (!graph) {
-      // warm the function attributes outside capture, then capture one step
+      // capture one step; the launchers' cudaFuncSetAttribute calls are not stream operations and are legal under capture, and
+      // first-use module loading inside a thread-local capture is permitted (every GPU test captures in a fresh process)
       cudaGraph_t g = nullptr;
       FR_CUDA_TRY(cudaStreamBeginCapture(stream, cudaStreamCaptureModeThreadLocal));
       int nk = 0;
