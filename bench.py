@@ -99,7 +99,7 @@ def _case(kind):
         c = cases.config3(p=kind["p"], ntheta=100 * kind["scale"], nz=15 * kind["scale"], seed=cases.SEEDS["c5"])
         return cases.replicate(c, kind["copies"], amp=0.005, seed=cases.SEEDS["c5"], compact=True)
     if "n" in kind:
-        return cases.config2(kind["n"], kind["p"], "ns", numbering="random")
+        return cases.config2(kind["n"], kind["p"], "ns", numbering="morton")      # Morton order is the primary numbering for throughput
     return cases.config3(**kind)
 
 
