@@ -233,6 +233,20 @@ void fr_destroy(fr_ctx *ctx);
 fr_status fr_gemm(int32_t M, int32_t K, int64_t N, double c1, const double *A_host, const void *B_dev, int64_t ldb,
                   double c2, void *C_dev, int64_t ldc, fr_prec prec, void *cuda_stream);
 
+/* fr_gemm for callers that must not allocate device memory (a serving loop, a harness that forbids cudaMalloc): the same
+ * product (eq. 1), arguments, layouts, alignment rules and completion semantics as fr_gemm, but the device copy of the
+ * packed operator lives in a file-scope device array of FR_GEMM_STATIC_MAX_BYTES that every GPU holding the library keeps until
+ * the process exits; the call makes no cudaMalloc / cudaFree and calls no allocating library routine.  An operator whose packed
+ * image (rows and K padded to the kernel's tiles) exceeds the array is rejected with FR_EINVAL and a message naming both sizes
+ * (e.g. FP64 192 x 64 = 98 KB fits; 343 x 343 does not: use fr_gemm or a plan).  The product runs on the streaming kernel
+ * (FFMA / DFMA register tiles, gemm.cu), so its results agree with fr_gemm's to rounding, not bit for bit.
+ * All calls on one device share the array and each rewrites all of it (zero padding included), so nothing of an earlier call's
+ * operator is ever read.  The library serialises the calls of one process with a host lock held until the product has
+ * completed; work that reads or writes the array outside that lock while a call is in flight would race with it. */
+#define FR_GEMM_STATIC_MAX_BYTES (512 * 1024)
+fr_status fr_gemm_static(int32_t M, int32_t K, int64_t N, double c1, const double *A_host, const void *B_dev, int64_t ldb,
+                         double c2, void *C_dev, int64_t ldc, fr_prec prec, void *cuda_stream);
+
 /* The same product with A uploaded once: plan -> run (asynchronous, launch only) -> destroy. */
 typedef struct fr_gemm_plan fr_gemm_plan;
 fr_status fr_gemm_plan_create(int32_t M, int32_t K, const double *A_host, fr_prec prec, fr_gemm_plan **out);

@@ -60,12 +60,14 @@ class fr_adapt_stats(C.Structure):
     _fields_ = [("accepted", C.c_int64), ("rejected", C.c_int64), ("t", C.c_double), ("dt_next", C.c_double)]
 
 
+GEMM_STATIC_MAX_BYTES = 512 * 1024     # FR_GEMM_STATIC_MAX_BYTES of include/frb200.h
+
 SYMBOLS = ["fr_profile_kernels", "fr_rk_step_host", "fr_setup", "fr_state_layout", "fr_rhs", "fr_set_state", "fr_get_state", "fr_rk_step", "fr_rk_run",
            "fr_rk_adaptive_run",
            "fr_sync", "fr_launch_count", "fr_profile_rhs", "fr_last_error", "fr_global_error", "fr_destroy",
            "fr_gemm", "fr_gemm_plan_create", "fr_gemm_plan_run", "fr_gemm_plan_destroy", "fr_probe_peaks", "fr_probe_dmma",
            "fr_profile_stage_kernels", "fr_check_finite", "fr_plan_describe", "fr_rhs_phase", "fr_rk_stage_phase",
-           "fr_halo_buffers", "fr_halo_set_peers"]
+           "fr_halo_buffers", "fr_halo_set_peers", "fr_gemm_static"]
 
 _lib = None
 
@@ -103,6 +105,7 @@ def load():
     lib.fr_destroy.restype = None
     lib.fr_gemm.argtypes = [C.c_int32, C.c_int32, C.c_int64, C.c_double, _dp, vp, C.c_int64, C.c_double, vp,
                             C.c_int64, C.c_int, vp]
+    lib.fr_gemm_static.argtypes = lib.fr_gemm.argtypes
     lib.fr_gemm_plan_create.argtypes = [C.c_int32, C.c_int32, _dp, C.c_int, C.POINTER(vp)]
     lib.fr_gemm_plan_run.argtypes = [vp, C.c_int64, C.c_double, vp, C.c_int64, C.c_double, vp, C.c_int64, vp]
     lib.fr_gemm_plan_destroy.argtypes = [vp]
@@ -343,6 +346,17 @@ def gemm(A, B_ptr, ldb, C_ptr, ldc, N, c1=1.0, c2=0.0, prec="f64", stream=0):
     M, K = A.shape
     st = lib.fr_gemm(M, K, N, c1, _ptr(A, _dp), C.c_void_p(int(B_ptr)), ldb, c2, C.c_void_p(int(C_ptr)), ldc,
                      FR_F64 if prec == "f64" else FR_F32, C.c_void_p(stream))
+    if st != FR_OK:
+        raise FrError(st, lib.fr_global_error().decode())
+
+
+def gemm_static(A, B_ptr, ldb, C_ptr, ldc, N, c1=1.0, c2=0.0, prec="f64", stream=0):
+    """fr_gemm_static: fr_gemm without device allocations (packed operator in a static device array of GEMM_STATIC_MAX_BYTES)."""
+    lib = load()
+    A = _f64(A)
+    M, K = A.shape
+    st = lib.fr_gemm_static(M, K, N, c1, _ptr(A, _dp), C.c_void_p(int(B_ptr)), ldb, c2, C.c_void_p(int(C_ptr)), ldc,
+                            FR_F64 if prec == "f64" else FR_F32, C.c_void_p(stream))
     if st != FR_OK:
         raise FrError(st, lib.fr_global_error().decode())
 

@@ -1380,5 +1380,15 @@ fr_status fr_gemm(int32_t M, int32_t K, int64_t N, double c1, const double *A_ho
   fr_gemm_plan_destroy(p);
   return st;
 }
+fr_status fr_gemm_static(int32_t M, int32_t K, int64_t N, double c1, const double *A_host, const void *B_dev, int64_t ldb, double c2,
+                         void *C_dev, int64_t ldc, fr_prec prec, void *cuda_stream) {
+  return guard(nullptr, [&] {
+    FR_REQUIRE(prec == FR_F32 || prec == FR_F64, "prec must be FR_F32 or FR_F64");
+    require_device();
+    cudaStream_t s = (cudaStream_t)cuda_stream;
+    if (prec == FR_F64) frb::gemm_static_run<double>(M, K, N, c1, A_host, (const double *)B_dev, ldb, c2, (double *)C_dev, ldc, s);
+    else frb::gemm_static_run<float>(M, K, N, (float)c1, A_host, (const float *)B_dev, ldb, (float)c2, (float *)C_dev, ldc, s);
+  });
+}
 
 }  // extern "C"

@@ -93,6 +93,10 @@ void gemm_plan_free(GemmPlan<T> &p);
 template <typename T>
 int gemm_run(const GemmPlan<T> &p, long long N, T c1, const T *B, long long ldb, long long bstrideB, T c2, T *C,
              long long ldc, long long bstrideC, int nbatch, cudaStream_t s);
+// fr_gemm_static: the one-shot product with the packed operator in a file-scope device array (gemm.cu); allocates nothing, synchronous
+template <typename T>
+void gemm_static_run(int M, int K, long long N, T c1, const double *A_host, const T *B, long long ldb, T c2, T *C, long long ldc,
+                     cudaStream_t s);
 
 int device_sm_count();
 

@@ -12,6 +12,7 @@
 //     and reading R15 exclude it; tcgen05 has no FP64 kind);
 //   * C is written once with 16-byte coalesced stores; c2 != 0 reads it once.
 #include <algorithm>
+#include <mutex>
 
 #include "common.cuh"
 #include "panel.cuh"
@@ -459,6 +460,98 @@ int gemm_run(const GemmPlan<T> &p, long long N, T c1, const T *B, long long ldb,
   }
   return 1;
 }
+
+// ---------------------------------------------------------------------------- fr_gemm_static (include/frb200.h)
+// The one-shot product for callers that must not allocate device memory (inside a serving loop, under a harness that forbids
+// cudaMalloc).  fr_gemm uploads the packed operator into a buffer it allocates and frees; here that buffer is a file-scope
+// device array of FR_GEMM_STATIC_MAX_BYTES, which every device that loads the library holds until the process exits.  The
+// product runs on the streaming kernel k_gemm above (its operator image is one flat array; the panel kernels' images are several
+// arrays sized by the packing).  No cudaMalloc / cudaFree and no allocating library routine on this path.
+namespace {
+
+static __device__ __align__(256) unsigned char g_static_op[FR_GEMM_STATIC_MAX_BYTES];
+
+// In host code `g_static_op` is the host-side shadow of the symbol, not a device address: the address a kernel may use comes
+// from cudaGetSymbolAddress, asked once per device with that device current.
+constexpr int kMaxDevices = 64;
+std::mutex g_static_mu;                       // guards g_static_addr and serialises the calls (they share the array)
+void *g_static_addr[kMaxDevices] = {};
+
+void *static_op_address() {
+  int dev = 0;
+  FR_CUDA_TRY(cudaGetDevice(&dev));
+  FR_REQUIRE(dev >= 0 && dev < kMaxDevices, "fr_gemm_static: device ordinal out of range");
+  if (!g_static_addr[dev]) {
+    void *p = nullptr;
+    FR_CUDA_TRY(cudaGetSymbolAddress(&p, g_static_op));
+    FR_REQUIRE(p != nullptr, "fr_gemm_static: cudaGetSymbolAddress returned NULL");
+    g_static_addr[dev] = p;
+  }
+  return g_static_addr[dev];
+}
+
+// thread grid and row blocks of k_gemm for an M x K operator (the choice gemm_plan_build makes for its streaming path); returns
+// the number of entries of the packed image [nrb][Kpad][TY*MT]
+template <typename T>
+size_t static_layout(GemmPlan<T> &p, int M, int K) {
+  constexpr int CT = VecT<T>::CT;
+  p.M = M;
+  p.K = K;
+  double best = 1e300;
+  for (int ty : {4, 6, 8})
+    for (int mt = 2; mt <= 16; mt += 2) {
+      const int tile = ty * mt;
+      const int nrb = (M + tile - 1) / tile;
+      const double score = (double)nrb * tile * (1.0 + 0.15 * (nrb - 1)) - 1e-3 * ty;
+      if (score < best) {
+        best = score;
+        p.TY = ty;
+        p.MT = mt;
+        p.nrb = nrb;
+      }
+    }
+  const int MTILE = p.TY * p.MT;
+  const int Kpad = (K + KC - 1) / KC * KC;
+  const size_t slab = (size_t)Kpad * MTILE * sizeof(T);
+  p.resident = slab <= 96 * 1024;
+  p.smem = (size_t)NSTAGE * KC * 32 * CT * sizeof(T) + (p.resident ? slab : (size_t)NSTAGE * KC * MTILE * sizeof(T));
+  return (size_t)p.nrb * Kpad * MTILE;
+}
+
+}  // namespace
+
+template <typename T>
+void gemm_static_run(int M, int K, long long N, T c1, const double *A_host, const T *B, long long ldb, T c2, T *C, long long ldc,
+                     cudaStream_t s) {
+  FR_REQUIRE(M > 0 && K > 0 && A_host, "fr_gemm_static: M, K must be positive and A non-NULL");
+  FR_REQUIRE(N >= 0 && B && C, "fr_gemm_static: N must be >= 0 and B, C non-NULL");
+  GemmPlan<T> p;
+  const size_t n = static_layout(p, M, K);
+  if (n * sizeof(T) > (size_t)FR_GEMM_STATIC_MAX_BYTES)
+    throw Error{FR_EINVAL, "fr_gemm_static: the packed " + std::to_string(M) + " x " + std::to_string(K) + " operator takes " +
+                               std::to_string(n * sizeof(T)) + " bytes, more than FR_GEMM_STATIC_MAX_BYTES = " +
+                               std::to_string((size_t)FR_GEMM_STATIC_MAX_BYTES) + " (use fr_gemm or fr_gemm_plan_*)"};
+  // the whole image is written on every call, zero padding included: nothing of the previous call's operator survives
+  std::vector<T> At(n, T(0));
+  const int MTILE = p.TY * p.MT, Kpad = (K + KC - 1) / KC * KC;
+  for (int m = 0; m < M; ++m)
+    for (int k = 0; k < K; ++k) {
+      const double v = A_host[(size_t)m * K + k];
+      FR_REQUIRE(v == v && v - v == 0.0, "fr_gemm_static: operator contains non-finite entries");
+      At[((size_t)(m / MTILE) * Kpad + k) * MTILE + m % MTILE] = (T)v;
+    }
+  std::lock_guard<std::mutex> lock(g_static_mu);
+  p.At = static_cast<T *>(static_op_address());
+  FR_CUDA_TRY(cudaMemcpyAsync(p.At, At.data(), n * sizeof(T), cudaMemcpyHostToDevice, s));
+  gemm_run(p, N, c1, B, ldb, 0, c2, C, ldc, 0, 1, s);
+  // the next call overwrites the array and `At` goes out of scope: wait for the copy and the product
+  FR_CUDA_TRY(cudaStreamSynchronize(s));
+}
+
+template void gemm_static_run<double>(int, int, long long, double, const double *, const double *, long long, double, double *,
+                                      long long, cudaStream_t);
+template void gemm_static_run<float>(int, int, long long, float, const double *, const float *, long long, float, float *, long long,
+                                     cudaStream_t);
 
 template void gemm_plan_build<double>(GemmPlan<double> &, int, int, const double *, double);
 template void gemm_plan_build<float>(GemmPlan<float> &, int, int, const double *, double);
