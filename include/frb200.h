@@ -252,6 +252,12 @@ typedef struct fr_gemm_plan fr_gemm_plan;
 fr_status fr_gemm_plan_create(int32_t M, int32_t K, const double *A_host, fr_prec prec, fr_gemm_plan **out);
 fr_status fr_gemm_plan_run(fr_gemm_plan *plan, int64_t N, double c1, const void *B_dev, int64_t ldb, double c2,
                            void *C_dev, int64_t ldc, void *cuda_stream);
+/* How the plan runs, one line per kernel launch: precision, rows of A it covers, packing ("dense", "k-lists", "dense, streamed" = an
+ * operator too large for shared memory whose packed blocks travel through the TMA ring with the chunks of B; otherwise such
+ * operators run as row blocks of A, one launch each), warp grid, panel width, chunk count and ring depth.  fr_gemm_plan_create
+ * times the candidate forms and keeps the fastest; every form gives bit-identical results.  NUL-terminated, at most cap - 1
+ * characters. */
+fr_status fr_gemm_plan_describe(const fr_gemm_plan *plan, char *buf, int64_t cap);
 void fr_gemm_plan_destroy(fr_gemm_plan *plan);
 
 /* Measured device peaks used as roofline denominators: register-resident FMA

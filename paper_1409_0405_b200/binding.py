@@ -67,7 +67,7 @@ SYMBOLS = ["fr_profile_kernels", "fr_rk_step_host", "fr_setup", "fr_state_layout
            "fr_sync", "fr_launch_count", "fr_profile_rhs", "fr_last_error", "fr_global_error", "fr_destroy",
            "fr_gemm", "fr_gemm_plan_create", "fr_gemm_plan_run", "fr_gemm_plan_destroy", "fr_probe_peaks", "fr_probe_dmma",
            "fr_profile_stage_kernels", "fr_check_finite", "fr_plan_describe", "fr_rhs_phase", "fr_rk_stage_phase",
-           "fr_halo_buffers", "fr_halo_set_peers", "fr_gemm_static"]
+           "fr_halo_buffers", "fr_halo_set_peers", "fr_gemm_static", "fr_gemm_plan_describe"]
 
 _lib = None
 
@@ -109,6 +109,7 @@ def load():
     lib.fr_gemm_plan_create.argtypes = [C.c_int32, C.c_int32, _dp, C.c_int, C.POINTER(vp)]
     lib.fr_gemm_plan_run.argtypes = [vp, C.c_int64, C.c_double, vp, C.c_int64, C.c_double, vp, C.c_int64, vp]
     lib.fr_gemm_plan_destroy.argtypes = [vp]
+    lib.fr_gemm_plan_describe.argtypes = [vp, C.c_char_p, C.c_int64]
     lib.fr_gemm_plan_destroy.restype = None
     lib.fr_probe_peaks.argtypes = [_dp, _dp, _dp]
     lib.fr_probe_dmma.argtypes = [_dp]
@@ -371,6 +372,14 @@ class GemmPlan:
         if st != FR_OK:
             raise FrError(st, lib.fr_global_error().decode())
         self._h = h
+
+    def describe(self):
+        """fr_gemm_plan_describe: one line per launch (packing, streamed or resident operator, geometry)."""
+        buf = C.create_string_buffer(8192)
+        st = self._lib.fr_gemm_plan_describe(self._h, buf, len(buf))
+        if st != FR_OK:
+            raise FrError(st, self._lib.fr_global_error().decode())
+        return buf.value.decode()
 
     def run(self, B_ptr, ldb, C_ptr, ldc, N, c1=1.0, c2=0.0, stream=0):
         st = self._lib.fr_gemm_plan_run(self._h, N, c1, C.c_void_p(int(B_ptr)), ldb, c2, C.c_void_p(int(C_ptr)), ldc,

@@ -1147,7 +1147,7 @@ struct Ctx : CtxBase {
     auto add = [&](const char *type, const char *what, const PanelOp<T> &op) {
       if (!op.ok()) return;
       snprintf(line, sizeof line, "%s %s %s %dx%d %s warps=%dx%dx%d+%d NIT=%d CX=%d NE=%d stages=%dx%d B occ=%d\n", sizeof(T) == 8 ? "f64" : "f32",
-               type, what, op.M, op.K, op.sparse ? "k-lists" : "dense", op.NG, op.WR, op.WC, op.NG, op.NIT, op.CX, op.NE, op.nstage,
+               type, what, op.M, op.K, op.sparse ? "k-lists" : (op.stream ? "dense, streamed" : "dense"), op.NG, op.WR, op.WC, op.NG, op.NIT, op.CX, op.NE, op.nstage,
                op.stage_bytes, op.occ);
       out += line;
     };
@@ -1177,6 +1177,27 @@ struct Ctx : CtxBase {
     FR_CUDA_TRY(cudaStreamSynchronize(stream));
   }
 };
+
+// one line per launch of a stand-alone operator-product plan (fr_gemm_plan_describe)
+template <typename T>
+std::string gemm_plan_describe(const GemmPlan<T> &p) {
+  std::string out;
+  char line[256];
+  auto add = [&](const PanelOp<T> &op, int row0) {
+    snprintf(line, sizeof line, "%s rows %d..%d of %dx%d %s warps=%dx%dx%d+%d NIT=%d CX=%d NE=%d chunks=%d stages=%dx%d B\n", sizeof(T) == 8 ? "f64" : "f32",
+             row0, row0 + op.M - 1, p.M, p.K, op.sparse ? "k-lists" : (op.stream ? "dense, streamed" : "dense"), op.NG, op.WR, op.WC, op.NG,
+             op.NIT, op.CX, op.NE, op.nchunks, op.nstage, op.stage_bytes);
+    out += line;
+  };
+  if (p.pop) add(*p.pop, 0);
+  for (int i = 0; i < p.nparts; ++i) add(*p.part[i], p.part_row0[i]);
+  if (!p.pop && p.nparts == 0) {
+    snprintf(line, sizeof line, "%s %dx%d register-tile kernel TY=%d MT=%d row blocks=%d %s\n", sizeof(T) == 8 ? "f64" : "f32", p.M, p.K, p.TY, p.MT,
+             p.nrb, p.resident ? "operator resident" : "operator streamed by cp.async");
+    out += line;
+  }
+  return out;
+}
 
 }  // namespace frb
 
@@ -1346,6 +1367,15 @@ fr_status fr_gemm_plan_run(fr_gemm_plan *plan, int64_t N, double c1, const void 
       frb::gemm_run(plan->pd, N, c1, (const double *)B_dev, ldb, 0, c2, (double *)C_dev, ldc, 0, 1, s);
     else
       frb::gemm_run(plan->pf, N, (float)c1, (const float *)B_dev, ldb, 0, (float)c2, (float *)C_dev, ldc, 0, 1, s);
+  });
+}
+fr_status fr_gemm_plan_describe(const fr_gemm_plan *plan, char *buf, int64_t cap) {
+  return guard(nullptr, [&] {
+    FR_REQUIRE(plan && buf && cap > 0, "plan and buf must be non-NULL and cap positive");
+    const std::string d = plan->prec == FR_F64 ? frb::gemm_plan_describe(plan->pd) : frb::gemm_plan_describe(plan->pf);
+    const size_t nc = std::min<size_t>(d.size(), (size_t)cap - 1);
+    memcpy(buf, d.data(), nc);
+    buf[nc] = 0;
   });
 }
 void fr_gemm_plan_destroy(fr_gemm_plan *plan) {

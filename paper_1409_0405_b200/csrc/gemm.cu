@@ -20,7 +20,7 @@
 namespace frb {
 
 template <typename T>
-bool panel_gemm_build(PanelOp<T> &op, int M, int K, const double *A, int cand = 0, double drop_rel = 1.4210854715202004e-14);
+bool panel_gemm_build(PanelOp<T> &op, int M, int K, const double *A, int cand = 0, double drop_rel = 1.4210854715202004e-14, int stream = 0);
 template <typename T>
 void panel_gemm_run(const PanelOp<T> &op, long long N, T c1, const T *B, long long ldb, long long bsB, T c2, T *C,
                     long long ldc, long long bsC, int nbatch, cudaStream_t s);
@@ -248,6 +248,49 @@ int device_sm_count() {
   return n > 0 ? n : 148;
 }
 
+// The panel-kernel forms of a plan.  stream = 0: the operator image stays in shared memory, as row blocks of A (one launch each,
+// every block re-reads B) when the whole image does not fit; stream = 1: the operator's packed blocks travel through the TMA ring with
+// the chunks of B (panel.cuh), which takes all rows a CTA's accumulators can hold in one pass -- row blocks only beyond that.  The
+// fewest blocks that work, rows per block a multiple of 8 and as even as possible.  Both forms give bit-identical results.
+template <typename T>
+bool plan_variant(GemmPlan<T> &p, int M, int K, const double *A_host, double drop_rel, int stream, int min_parts) {
+  for (int np = std::max(1, min_parts); np <= GemmPlan<T>::kMaxParts; ++np) {
+    const int per = np == 1 ? M : ((M + np - 1) / np + 7) / 8 * 8;
+    if (np > 1 && (long long)per * (np - 1) >= M) continue;
+    bool ok = true;
+    int n = 0;
+    PanelOp<T> *ops[GemmPlan<T>::kMaxParts] = {};
+    for (int r0 = 0; r0 < M && ok; r0 += per, ++n) {
+      ops[n] = new PanelOp<T>();
+      try {
+        ok = panel_gemm_build(*ops[n], std::min(per, M - r0), K, A_host + (size_t)r0 * K, 0, drop_rel, stream);
+      } catch (...) {
+        ok = false;
+      }
+    }
+    if (ok) {
+      p.M = M;
+      p.K = K;
+      if (np == 1) {
+        p.pop = ops[0];
+      } else {
+        p.nparts = n;
+        for (int i = 0; i < n; ++i) {
+          p.part[i] = ops[i];
+          p.part_row0[i] = i * per;
+        }
+      }
+      return true;
+    }
+    for (int i = 0; i < n; ++i) {
+      panel_op_free(*ops[i]);
+      delete ops[i];
+    }
+    if (np == 1 && getenv("FRB_NO_ROWSPLIT")) break;
+  }
+  return false;
+}
+
 template <typename T>
 void gemm_plan_build(GemmPlan<T> &p, int M, int K, const double *A_host, double drop_rel) {
   FR_REQUIRE(M > 0 && K > 0 && A_host, "gemm: M, K must be positive and A non-NULL");
@@ -255,47 +298,26 @@ void gemm_plan_build(GemmPlan<T> &p, int M, int K, const double *A_host, double 
   p.M = M;
   p.K = K;
   const int force_split = getenv("FRB_FORCE_SPLIT") ? atoi(getenv("FRB_FORCE_SPLIT")) : 0;
-  if (force_split < 2 || M < 16) {
-    // preferred path: operator resident in shared memory, all rows in one CTA (panel.cuh)
-    auto *pop = new PanelOp<T>();
-    bool ok = false;
-    try {
-      ok = panel_gemm_build(*pop, M, K, A_host, 0, drop_rel);
-    } catch (...) {
-      delete pop;
-      throw;
-    }
-    if (ok) {
-      p.pop = pop;
-      return;
-    }
-    delete pop;
+  // FRB_GEMM_STREAM: 0 never stream the operator, 1 stream whenever the resident image does not fit; default: the static rule below
+  const int stream_mode = getenv("FRB_GEMM_STREAM") ? atoi(getenv("FRB_GEMM_STREAM")) : -1;
+  const int min_parts = (force_split >= 2 && M >= 16) ? force_split : 1;
+  // preferred: operator resident in shared memory, all rows in one CTA (panel.cuh)
+  GemmPlan<T> res, str;
+  const bool have_res = plan_variant(res, M, K, A_host, drop_rel, 0, min_parts);
+  if (have_res && res.pop) {
+    p = res;
+    return;
   }
-  // row blocks of A on the panel kernel (rows per block a multiple of 8, as even as possible)
-  for (int np = std::max(2, force_split); np <= GemmPlan<T>::kMaxParts && getenv("FRB_NO_ROWSPLIT") == nullptr; ++np) {
-    const int per = ((M + np - 1) / np + 7) / 8 * 8;
-    if ((long long)per * (np - 1) >= M) continue;
-    bool ok = true;
-    int n = 0;
-    for (int r0 = 0; r0 < M && ok; r0 += per, ++n) {
-      auto *pop = new PanelOp<T>();
-      p.part[n] = pop;
-      p.part_row0[n] = r0;
-      try {
-        ok = panel_gemm_build(*pop, std::min(per, M - r0), K, A_host + (size_t)r0 * K, 0, drop_rel);
-      } catch (...) {
-        ok = false;
-      }
-    }
-    if (ok) {
-      p.nparts = n;
-      return;
-    }
-    for (int i = 0; i < n; ++i) {
-      panel_op_free(*p.part[i]);
-      delete p.part[i];
-      p.part[i] = nullptr;
-    }
+  const bool have_str = stream_mode != 0 && plan_variant(str, M, K, A_host, drop_rel, 1, min_parts);
+  if (have_res || have_str) {
+    // without timing (fr_gemm; fr_gemm_plan_create times both forms): streamed when the passes over B it saves outweigh twice the
+    // rows of C -- the rule that picks the faster form for every operator of BASELINE.json configs[3] (profiles/r02_e_gemm_sweep.md)
+    const long long nr = have_res ? res.nparts : 1 << 20, ns = have_str ? std::max(1, str.nparts) : 1 << 20;
+    const bool take_str = have_str && (!have_res || stream_mode == 1 || (nr - ns) * K > 2ll * M);
+    p = take_str ? str : res;
+    if (have_res && take_str) gemm_plan_free(res);
+    if (have_str && !take_str) gemm_plan_free(str);
+    return;
   }
   double best = 1e300;
   const int tys[3] = {4, 6, 8};
@@ -335,31 +357,39 @@ void gemm_plan_build(GemmPlan<T> &p, int M, int K, const double *A_host, double 
 }
 
 // Time the launch geometries of a plan's panel operator on scratch matrices larger than L2 and keep the fastest (what Ctx::tune
-// does for the operators of fr_setup).  Results do not depend on the choice (panel.cuh).  FRB_AUTOTUNE=0 skips it.
+// does for the operators of fr_setup); for an operator that does not fit shared memory, also time the other form of the plan
+// (resident row blocks / streamed operator) and keep the faster one.  Results do not depend on the choice (panel.cuh).
+// FRB_AUTOTUNE=0 skips it.
+namespace {
+
 template <typename T>
-void gemm_plan_tune(GemmPlan<T> &p, const double *A_host, double drop_rel) {
-  const char *env = getenv("FRB_AUTOTUNE");
-  if (env && atoi(env) == 0) return;
-  if (!p.pop && p.nparts == 0) return;
-  const int M = p.pop ? p.M : p.part[0]->M, K = p.K;
-  // columns: 320 MB of B and C, a multiple of 5 * 128
-  long long N = (long long)(320e6 / ((double)(M + K) * sizeof(T)));
-  N = std::max<long long>(640, N / 640 * 640);
-  T *B = nullptr, *Cm = nullptr;
-  if (cudaMalloc(&B, (size_t)K * N * sizeof(T)) != cudaSuccess) return;
-  if (cudaMalloc(&Cm, (size_t)M * N * sizeof(T)) != cudaSuccess) {
-    cudaFree(B);
-    return;
+struct TuneScratch {
+  T *B = nullptr, *C = nullptr;
+  long long N = 0;
+  cudaEvent_t e0 = nullptr, e1 = nullptr;
+  bool init(int M, int K) {
+    // columns: 320 MB of B and C, a multiple of 5 * 128
+    N = (long long)(320e6 / ((double)(M + K) * sizeof(T)));
+    N = std::max<long long>(640, N / 640 * 640);
+    if (cudaMalloc(&B, (size_t)K * N * sizeof(T)) != cudaSuccess) return false;
+    if (cudaMalloc(&C, (size_t)M * N * sizeof(T)) != cudaSuccess) return false;
+    cudaMemset(B, 0, (size_t)K * N * sizeof(T));
+    cudaEventCreate(&e0);
+    cudaEventCreate(&e1);
+    return true;
   }
-  cudaMemset(B, 0, (size_t)K * N * sizeof(T));
-  cudaEvent_t e0, e1;
-  cudaEventCreate(&e0);
-  cudaEventCreate(&e1);
-  auto time_op = [&](const PanelOp<T> &op) {
+  ~TuneScratch() {
+    if (e0) cudaEventDestroy(e0);
+    if (e1) cudaEventDestroy(e1);
+    if (B) cudaFree(B);
+    if (C) cudaFree(C);
+  }
+  template <typename F>
+  float time(F &&run) {
     float best = 1e30f;
     for (int rep = 0; rep < 4; ++rep) {
       cudaEventRecord(e0, 0);
-      panel_gemm_run(op, N, T(1), B, N, 0, T(0), Cm, N, 0, 1, (cudaStream_t)0);
+      run();
       cudaEventRecord(e1, 0);
       cudaEventSynchronize(e1);
       float ms = 0;
@@ -367,14 +397,23 @@ void gemm_plan_tune(GemmPlan<T> &p, const double *A_host, double drop_rel) {
       if (rep > 0) best = std::min(best, ms);
     }
     return best;
-  };
+  }
+};
+
+// geometry candidates of the plan's (first) panel operator; the other row blocks take the winner's index
+template <typename T>
+void tune_geometry(GemmPlan<T> &p, const double *A_host, double drop_rel, TuneScratch<T> &sc) {
   PanelOp<T> *cur = p.pop ? p.pop : p.part[0];
+  const int M = cur->M, K = p.K, stream = cur->stream;
+  auto time_op = [&](const PanelOp<T> &op) {
+    return sc.time([&] { panel_gemm_run(op, sc.N, T(1), sc.B, sc.N, 0, T(0), sc.C, sc.N, 0, 1, (cudaStream_t)0); });
+  };
   float bt = time_op(*cur);
   int bestk = 0;
   const int ncand = getenv("FRB_TUNE_CANDS") ? std::max(1, atoi(getenv("FRB_TUNE_CANDS"))) : 14;
   for (int k = 1; k < ncand; ++k) {
     PanelOp<T> op;
-    if (!panel_gemm_build(op, M, K, A_host, k, drop_rel)) break;
+    if (!panel_gemm_build(op, M, K, A_host, k, drop_rel, stream)) break;
     const float t = time_op(op);
     if (t < bt) {
       panel_op_free(*cur);
@@ -385,18 +424,35 @@ void gemm_plan_tune(GemmPlan<T> &p, const double *A_host, double drop_rel) {
       panel_op_free(op);
     }
   }
-  // row blocks: the other blocks take the same candidate (same shape up to the last block's height)
   for (int i = 1; i < p.nparts && bestk > 0; ++i) {
     PanelOp<T> op;
-    if (panel_gemm_build(op, p.part[i]->M, K, A_host + (size_t)p.part_row0[i] * K, bestk, drop_rel)) {
+    if (panel_gemm_build(op, p.part[i]->M, K, A_host + (size_t)p.part_row0[i] * K, bestk, drop_rel, stream)) {
       panel_op_free(*p.part[i]);
       *p.part[i] = op;
     }
   }
-  cudaEventDestroy(e0);
-  cudaEventDestroy(e1);
-  cudaFree(B);
-  cudaFree(Cm);
+}
+
+}  // namespace
+
+template <typename T>
+void gemm_plan_tune(GemmPlan<T> &p, const double *A_host, double drop_rel) {
+  const char *env = getenv("FRB_AUTOTUNE");
+  if (env && atoi(env) == 0) return;
+  if (!p.pop && p.nparts == 0) return;
+  TuneScratch<T> sc;
+  if (!sc.init(p.M, p.K)) return;
+  tune_geometry(p, A_host, drop_rel, sc);
+  const int cur_stream = (p.pop ? p.pop : p.part[0])->stream;
+  if ((p.pop && !cur_stream) || getenv("FRB_GEMM_STREAM")) return;   // the whole image is resident, or the form is forced
+  GemmPlan<T> q;
+  if (!plan_variant(q, p.M, p.K, A_host, drop_rel, 1 - cur_stream, 1)) return;
+  tune_geometry(q, A_host, drop_rel, sc);
+  auto time_plan = [&](const GemmPlan<T> &g) {
+    return sc.time([&] { gemm_run(g, sc.N, T(1), sc.B, sc.N, 0, T(0), sc.C, sc.N, 0, 1, (cudaStream_t)0); });
+  };
+  if (time_plan(q) < time_plan(p)) std::swap(p, q);
+  gemm_plan_free(q);
 }
 
 template <typename T>

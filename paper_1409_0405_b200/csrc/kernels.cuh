@@ -96,7 +96,7 @@ int launch_fused_grad(const PanelOp<T> &op, const EleView<T> &ev, const T *u, co
 // Plain operator product on the panel kernels (panel_gemm.cu); `cand` as above.
 // drop_rel: entries with |a| <= drop_rel * max|A| count as structural zeros (reading R24; 0 = exact zeros only)
 template <typename T>
-bool panel_gemm_build(PanelOp<T> &op, int M, int K, const double *A, int cand = 0, double drop_rel = 1.4210854715202004e-14);
+bool panel_gemm_build(PanelOp<T> &op, int M, int K, const double *A, int cand = 0, double drop_rel = 1.4210854715202004e-14, int stream = 0);
 template <typename T>
 void panel_gemm_run(const PanelOp<T> &op, long long N, T c1, const T *B, long long ldb, long long bsB, T c2, T *C,
                     long long ldc, long long bsC, int nbatch, cudaStream_t s);

@@ -32,7 +32,7 @@ namespace frb {
 
 constexpr int PV = FR_NVAR;          // variable segments per panel
 constexpr int PANEL_MAXW = 20;       // warps per CTA, producers included (fewer when the accumulators need more registers)
-constexpr int PANEL_MAXCHUNKS = 64;
+constexpr int PANEL_MAXCHUNKS = 160;
 constexpr int PANEL_KCMAX = 40;      // rows per chunk (upper bound; a multiple of 8)
 constexpr int PANEL_MAXSTAGE = 8;    // ring depth (upper bound)
 constexpr int PANEL_MAXSRC = 2;      // matrices stacked along K
@@ -61,6 +61,9 @@ struct PanelOp {
   int dbg = 0;                           // measurement aid (env FRB_PANEL_DBG): 1 skip multiply, 2 skip epilogue
 #endif
   int sparse = 0;                        // 1: per-group k-lists (idx/off); 0: dense, all slots share the chunk's k-blocks
+  int stream = 0;                        // 1: the operator does not stay in shared memory: the packed blocks of a chunk travel through
+                                         //    the ring behind the chunk's rows of B (dense packing only), at stage offset a_off
+  int a_off = 0;
   int nsrc = 0;
   int src_rows[PANEL_MAXSRC] = {0, 0};   // rows of each stacked source
   int src_step[PANEL_MAXSRC] = {0, 0};   // rows per chunk (TMA box height) of each source
@@ -205,6 +208,7 @@ struct PackOptions {
   const int *row_ids = nullptr;   // row split: the epilogue's row number of each row of A (nullptr = 0..M-1)
   // entries with |a| <= drop_rel * max|A| are treated as structural zeros (reading R24); 0: only exact zeros
   double drop_rel = 1.4210854715202004e-14;
+  int stream = 0;          // build the streamed-operator form (PanelOp::stream)
 };
 
 // Rows per chunk of a source with `rows` rows: the multiple of 8 (<= PANEL_KCMAX) with the fewest chunks, counting a fixed
@@ -307,14 +311,18 @@ bool panel_op_build(PanelOp<T> &p, int M, int K, const double *A, const std::vec
         ++nnz;
       }
   const double density = (double)nnz / ((double)M * K);
-  // ---- chunks: a function of the sources' row counts alone
+  // ---- chunks: a function of the sources' row counts alone.  (A streamed operator may cut a source into lower chunks, `step` rows
+  // each, so that a chunk's operator blocks fit a ring stage: steps are multiples of 8 and the k-blocks are formed inside groups of
+  // 8 rows, so the sequence of k-blocks -- the summation order -- is the same for every step.)
   std::vector<ChunkDesc> chunks;
   std::vector<int> chunk_k0;   // column of A behind stage row 0 of the chunk
   int src_step[PANEL_MAXSRC] = {0, 0};
-  {
+  auto make_chunks = [&](int step_cap) {
+    chunks.clear();
+    chunk_k0.clear();
     int k0 = 0, si = 0;
     for (auto &s : srcs) {
-      const int step = panel_chunk_step(s.rows);
+      const int step = std::min(panel_chunk_step(s.rows), step_cap);
       src_step[si] = step;
       for (int r = 0; r < s.rows; r += step) {
         chunks.push_back(ChunkDesc{si, r, std::min(step, s.rows - r), step, 0, 0, 0, 0});
@@ -323,8 +331,9 @@ bool panel_op_build(PanelOp<T> &p, int M, int K, const double *A, const std::vec
       k0 += s.rows;
       ++si;
     }
-  }
-  const int nchunks = (int)chunks.size();
+  };
+  make_chunks(PANEL_KCMAX);
+  int nchunks = (int)chunks.size();
   if (nchunks > PANEL_MAXCHUNKS) return false;
 
   // ---- rows -> groups of 8, for a given packing
@@ -375,11 +384,12 @@ bool panel_op_build(PanelOp<T> &p, int M, int K, const double *A, const std::vec
         }
     return lists;
   };
-  // ---- packing: k-lists when they save at least 15 % of the multiplies of the dense packing (a function of the operator alone)
+  // ---- packing: k-lists when they save at least 15 % of the multiplies of the dense packing (a function of the operator alone).
+  // A streamed operator is always packed densely (its blocks must be one contiguous range per chunk).
   bool sparse = false;
   std::vector<int> order = make_order(false);
   std::vector<std::vector<std::vector<int>>> lists;
-  if (opt.allow_sparse && density < 0.95) {
+  if (opt.allow_sparse && !opt.stream && density < 0.95) {
     std::vector<int> so = make_order(true);
     auto sl = make_lists(so);
     double ds = 0, dd = 0;
@@ -399,190 +409,228 @@ bool panel_op_build(PanelOp<T> &p, int M, int K, const double *A, const std::vec
   if (opt.cand < 0) return false;
   int nfit = 0;
   for (const PanelGeom &geo : geoms) {
-  size_t smem_total = smem_total_in;
-  const int WR = geo.WR, NIT = geo.NIT, NS = WR * NIT;
-  // cost of each group (blocks it executes) and LPT assignment of group units (1 or 3 groups) to row-warps
-  std::vector<long long> gcost(G, 0);
-  for (int g = 0; g < G; ++g)
-    for (int c = 0; c < nchunks; ++c) {
-      const int n = sparse ? (int)lists[g][c].size() : chunks[c].nrows;
-      gcost[g] += f64 ? (n + 3) / 4 * 4 : n;
-    }
-  const int gu = opt.triple ? 3 : 1;
-  const int GU = G / gu;
-  std::vector<int> uorder(GU);
-  std::iota(uorder.begin(), uorder.end(), 0);
-  auto ucost = [&](int u) {
-    long long c = 0;
-    for (int j = 0; j < gu; ++j) c += gcost[u * gu + j];
-    return c;
-  };
-  std::stable_sort(uorder.begin(), uorder.end(), [&](int a, int b) { return ucost(a) > ucost(b); });
-  std::vector<long long> wload(WR, 0);
-  std::vector<int> wcount(WR, 0);
-  std::vector<int> slot_group(NS, -1);
-  for (int u : uorder) {
-    int bw = -1;
-    for (int w = 0; w < WR; ++w)
-      if (wcount[w] + gu <= NIT && (bw < 0 || wload[w] < wload[bw])) bw = w;
-    FR_REQUIRE(bw >= 0, "panel_op_build: slot assignment failed");
-    for (int j = 0; j < gu; ++j) slot_group[bw * NIT + wcount[bw] + j] = u * gu + j;
-    wcount[bw] += gu;
-    wload[bw] += ucost(u);
-  }
-  // ---- pack
-  std::vector<T> vals;
-  std::vector<uint32_t> idx;
-  std::vector<int> off(sparse ? nchunks * NS + 1 : 1, 0);
-  std::vector<int> rowmap(NS * 8, -1);
-  for (int s = 0; s < NS; ++s)
-    if (slot_group[s] >= 0)
-      for (int r = 0; r < 8; ++r) {
-        const int m = order[8 * slot_group[s] + r];
-        rowmap[s * 8 + r] = (m >= 0 && opt.row_ids) ? opt.row_ids[m] : m;
+    size_t smem_total = smem_total_in;
+    if (geo.occ == 2) smem_total = smem_total / 2 - 1024;
+    const int WR = geo.WR, NIT = geo.NIT, NS = WR * NIT;
+    // cost of each group (blocks it executes) and LPT assignment of group units (1 or 3 groups) to row-warps
+    std::vector<long long> gcost(G, 0);
+    for (int g = 0; g < G; ++g)
+      for (int c = 0; c < nchunks; ++c) {
+        const int n = sparse ? (int)lists[g][c].size() : chunks[c].nrows;
+        gcost[g] += f64 ? (n + 3) / 4 * 4 : n;
       }
-  auto aval = [&](int m, int col) {
-    if (m < 0) return 0.0;
-    const double v = A[(size_t)m * K + col];
-    return std::fabs(v) > thr ? v : 0.0;
-  };
-  const uint32_t rs32 = (uint32_t)geo.NE * 4u;   // FP32: bytes between stage rows
-  long long macs = 0;
-  int nblk = 0;
-  if (!sparse) {
-    // dense: blocks ordered (chunk, k-block, slot); the rows of a k-block come from the row table idx[block][4] (FP64)
-    for (int c = 0; c < nchunks; ++c) {
-      chunks[c].base = nblk / NS;
-      if (f64) {
-        const auto blocks = dense_blocks_f64(chunks[c].nrows);
-        chunks[c].nblk = (int)blocks.size();
-        for (auto &b : blocks) {
-          for (int j = 0; j < 4; ++j) idx.push_back(swz_row_offset(j < (int)b.size() ? b[j] : b[0]));
-          for (int s = 0; s < NS; ++s) {
-            const int g = slot_group[s];
-            for (int lane = 0; lane < 32; ++lane) {
-              const int r = lane >> 2, j = lane & 3;
-              const int m = g >= 0 ? order[8 * g + r] : -1;
-              vals.push_back((T)(j < (int)b.size() ? aval(m, chunk_k0[c] + b[j]) : 0.0));
+    const int gu = opt.triple ? 3 : 1;
+    const int GU = G / gu;
+    std::vector<int> uorder(GU);
+    std::iota(uorder.begin(), uorder.end(), 0);
+    auto ucost = [&](int u) {
+      long long c = 0;
+      for (int j = 0; j < gu; ++j) c += gcost[u * gu + j];
+      return c;
+    };
+    std::stable_sort(uorder.begin(), uorder.end(), [&](int a, int b) { return ucost(a) > ucost(b); });
+    std::vector<long long> wload(WR, 0);
+    std::vector<int> wcount(WR, 0);
+    std::vector<int> slot_group(NS, -1);
+    for (int u : uorder) {
+      int bw = -1;
+      for (int w = 0; w < WR; ++w)
+        if (wcount[w] + gu <= NIT && (bw < 0 || wload[w] < wload[bw])) bw = w;
+      FR_REQUIRE(bw >= 0, "panel_op_build: slot assignment failed");
+      for (int j = 0; j < gu; ++j) slot_group[bw * NIT + wcount[bw] + j] = u * gu + j;
+      wcount[bw] += gu;
+      wload[bw] += ucost(u);
+    }
+    std::vector<int> rowmap(NS * 8, -1);
+    for (int s = 0; s < NS; ++s)
+      if (slot_group[s] >= 0)
+        for (int r = 0; r < 8; ++r) {
+          const int m = order[8 * slot_group[s] + r];
+          rowmap[s * 8 + r] = (m >= 0 && opt.row_ids) ? opt.row_ids[m] : m;
+        }
+    auto aval = [&](int m, int col) {
+      if (m < 0) return 0.0;
+      const double v = A[(size_t)m * K + col];
+      return std::fabs(v) > thr ? v : 0.0;
+    };
+    // every array is copied to shared memory by one bulk copy: sizes are multiples of 16 bytes
+    auto pad16 = [](auto &v) {
+      using E = typename std::remove_reference<decltype(v[0])>::type;
+      while ((v.size() * sizeof(E)) % 16) v.push_back(E());
+    };
+    pad16(rowmap);
+    const uint32_t rs32 = (uint32_t)geo.NE * 4u;   // FP32: bytes between stage rows
+    const size_t ablk = (size_t)NS * (f64 ? 256 : 32);   // bytes of one packed block row (all slots)
+    std::vector<T> vals;
+    std::vector<uint32_t> idx;
+    std::vector<int> off;
+    long long macs = 0;
+    int nblk = 0, nstage = 0;
+    size_t smem_op = 0, stage_bytes = 0, a_off = 0;
+    // ---- pack for the current chunks; false if the result does not fit
+    auto pack = [&]() {
+      vals.clear();
+      idx.clear();
+      off.assign(sparse ? nchunks * NS + 1 : 1, 0);
+      macs = 0;
+      nblk = 0;
+      if (!sparse) {
+        // dense: blocks ordered (chunk, k-block, slot); the rows of a k-block come from the row table idx[block][4] (FP64)
+        for (int c = 0; c < nchunks; ++c) {
+          chunks[c].base = nblk / NS;
+          if (f64) {
+            const auto blocks = dense_blocks_f64(chunks[c].nrows);
+            chunks[c].nblk = (int)blocks.size();
+            for (auto &b : blocks) {
+              for (int j = 0; j < 4; ++j) idx.push_back(swz_row_offset(j < (int)b.size() ? b[j] : b[0]));
+              for (int s = 0; s < NS; ++s) {
+                const int g = slot_group[s];
+                for (int lane = 0; lane < 32; ++lane) {
+                  const int r = lane >> 2, j = lane & 3;
+                  const int m = g >= 0 ? order[8 * g + r] : -1;
+                  vals.push_back((T)(j < (int)b.size() ? aval(m, chunk_k0[c] + b[j]) : 0.0));
+                }
+                if (g >= 0) macs += 32;
+                ++nblk;
+              }
             }
-            if (g >= 0) macs += 32;
-            ++nblk;
+          } else {
+            chunks[c].nblk = chunks[c].nrows;
+            for (int k = 0; k < chunks[c].nrows; ++k)
+              for (int s = 0; s < NS; ++s) {
+                const int g = slot_group[s];
+                for (int r = 0; r < 8; ++r) vals.push_back((T)aval(g >= 0 ? order[8 * g + r] : -1, chunk_k0[c] + k));
+                if (g >= 0) macs += 8;
+                ++nblk;
+              }
           }
         }
       } else {
-        chunks[c].nblk = chunks[c].nrows;
-        for (int k = 0; k < chunks[c].nrows; ++k)
+        for (int c = 0; c < nchunks; ++c)
           for (int s = 0; s < NS; ++s) {
+            off[c * NS + s] = nblk;
             const int g = slot_group[s];
-            for (int r = 0; r < 8; ++r) vals.push_back((T)aval(g >= 0 ? order[8 * g + r] : -1, chunk_k0[c] + k));
-            if (g >= 0) macs += 8;
-            ++nblk;
+            if (g < 0) continue;
+            const std::vector<int> &L = lists[g][c];
+            if (f64) {
+              for (auto &b : sparse_blocks_f64(L)) {
+                for (int j = 0; j < 4; ++j) idx.push_back(swz_row_offset(j < (int)b.size() ? b[j] : b[0]));
+                for (int lane = 0; lane < 32; ++lane) {
+                  const int r = lane >> 2, j = lane & 3;
+                  vals.push_back((T)(j < (int)b.size() ? aval(order[8 * g + r], chunk_k0[c] + b[j]) : 0.0));
+                }
+                ++nblk;
+                macs += 32;
+              }
+            } else {
+              for (int kk : L) {
+                idx.push_back((uint32_t)kk * rs32);
+                for (int r = 0; r < 8; ++r) vals.push_back((T)aval(order[8 * g + r], chunk_k0[c] + kk));
+                ++nblk;
+                macs += 8;
+              }
+            }
           }
+        off[nchunks * NS] = nblk;
+      }
+      // the sparse multiply loop prefetches two blocks ahead: two all-zero blocks close the arrays (not counted in nblk)
+      for (int d = 0; d < 2; ++d) {
+        for (int j = 0; j < (f64 ? 4 : 1); ++j) idx.push_back(0u);
+        for (int j = 0; j < (f64 ? 32 : 8); ++j) vals.push_back(T(0));
+      }
+      pad16(vals);
+      pad16(idx);
+      pad16(off);
+      smem_op = (opt.stream ? 0 : vals.size() * sizeof(T)) + idx.size() * 4 + off.size() * 4 + rowmap.size() * 4 + chunks.size() * sizeof(ChunkDesc);
+      if (smem_op > smem_budget) return false;
+      size_t bmax = 0, amax_b = 0;
+      for (auto &c : chunks) {
+        bmax = std::max(bmax, (size_t)PV * geo.NE * c.step * sizeof(T));
+        amax_b = std::max(amax_b, (size_t)c.nblk * ablk);
+      }
+      a_off = (bmax + 127) / 128 * 128;
+      stage_bytes = (a_off + (opt.stream ? amax_b : 0) + 1023) / 1024 * 1024;
+      // 1 kB to align the ring, the ring, 256 B of mbarriers
+      const size_t fixed = 1024 + (smem_op + 1023) / 1024 * 1024 + 256;
+      if (fixed + 2 * geo.NG * stage_bytes > smem_total) return false;
+      nstage = std::min((int)((smem_total - fixed) / (geo.NG * stage_bytes)), PANEL_MAXSTAGE);
+      return true;
+    };
+    bool fits = false;
+    if (!opt.stream) {
+      fits = pack();
+    } else {
+      // the highest chunks that leave a ring of four stages; failing that, the deepest ring any chunk height gives
+      int best_step = 0, best_stages = 0;
+      for (int step = PANEL_KCMAX; step >= 8; step -= 8) {
+        make_chunks(step);
+        nchunks = (int)chunks.size();
+        if (nchunks > PANEL_MAXCHUNKS || !pack()) continue;
+        if (nstage > best_stages) {
+          best_stages = nstage;
+          best_step = step;
+        }
+        if (nstage >= 4) break;
+      }
+      if (best_step) {
+        make_chunks(best_step);
+        nchunks = (int)chunks.size();
+        fits = pack();
       }
     }
-  } else {
-    for (int c = 0; c < nchunks; ++c)
-      for (int s = 0; s < NS; ++s) {
-        off[c * NS + s] = nblk;
-        const int g = slot_group[s];
-        if (g < 0) continue;
-        const std::vector<int> &L = lists[g][c];
-        if (f64) {
-          for (auto &b : sparse_blocks_f64(L)) {
-            for (int j = 0; j < 4; ++j) idx.push_back(swz_row_offset(j < (int)b.size() ? b[j] : b[0]));
-            for (int lane = 0; lane < 32; ++lane) {
-              const int r = lane >> 2, j = lane & 3;
-              vals.push_back((T)(j < (int)b.size() ? aval(order[8 * g + r], chunk_k0[c] + b[j]) : 0.0));
-            }
-            ++nblk;
-            macs += 32;
-          }
-        } else {
-          for (int kk : L) {
-            idx.push_back((uint32_t)kk * rs32);
-            for (int r = 0; r < 8; ++r) vals.push_back((T)aval(order[8 * g + r], chunk_k0[c] + kk));
-            ++nblk;
-            macs += 8;
-          }
-        }
-      }
-    off[nchunks * NS] = nblk;
-  }
-  // the sparse multiply loop prefetches two blocks ahead: two all-zero blocks close the arrays (not counted in nblk)
-  for (int d = 0; d < 2; ++d) {
-    for (int j = 0; j < (f64 ? 4 : 1); ++j) idx.push_back(0u);
-    for (int j = 0; j < (f64 ? 32 : 8); ++j) vals.push_back(T(0));
-  }
-  // every array is copied to shared memory by one bulk copy: sizes are multiples of 16 bytes
-  auto pad16 = [](auto &v) {
-    using E = typename std::remove_reference<decltype(v[0])>::type;
-    while ((v.size() * sizeof(E)) % 16) v.push_back(E());
-  };
-  pad16(vals);
-  pad16(idx);
-  pad16(off);
-  pad16(rowmap);
-  const size_t smem_op = vals.size() * sizeof(T) + idx.size() * 4 + off.size() * 4 + rowmap.size() * 4 + chunks.size() * sizeof(ChunkDesc);
-  if (geo.occ == 2) smem_total = smem_total / 2 - 1024;
-  if (smem_op > smem_budget) continue;
-  size_t stage_bytes = 0;
-  for (auto &c : chunks) stage_bytes = std::max(stage_bytes, (size_t)PV * geo.NE * c.step * sizeof(T));
-  stage_bytes = (stage_bytes + 1023) / 1024 * 1024;
-  // 1 kB to align the ring, the ring, 256 B of mbarriers
-  const size_t fixed = 1024 + (smem_op + 1023) / 1024 * 1024 + 256;
-  if (fixed + 2 * geo.NG * stage_bytes > smem_total) continue;
-  if (nfit++ != opt.cand) continue;
-  int nstage = (int)((smem_total - fixed) / (geo.NG * stage_bytes));
-  nstage = std::min(nstage, PANEL_MAXSTAGE);
-  if (getenv("FRB_NSTAGE")) nstage = std::max(2, std::min(nstage, atoi(getenv("FRB_NSTAGE"))));
-  panel_op_free(p);
-  p.M = M;
-  p.K = K;
-  p.WR = WR;
-  p.WC = geo.WC;
-  p.NIT = NIT;
-  p.CX = geo.CX;
-  p.NE = geo.NE;
-  p.NG = geo.NG;
-  p.occ = geo.occ;
-  p.nchunks = nchunks;
-  p.NS = NS;
-  p.nstage = nstage;
-  p.stage_bytes = (int)stage_bytes;
-  p.nblk = nblk;
-  p.nidx = (int)idx.size();
-  p.nsrc = (int)srcs.size();
-  for (int i = 0; i < p.nsrc; ++i) {
-    p.src_rows[i] = srcs[i].rows;
-    p.src_step[i] = src_step[i];
-  }
+    if (!fits) continue;
+    if (nfit++ != opt.cand) continue;
+    if (getenv("FRB_NSTAGE")) nstage = std::max(2, std::min(nstage, atoi(getenv("FRB_NSTAGE"))));
+    panel_op_free(p);
+    p.M = M;
+    p.K = K;
+    p.WR = WR;
+    p.WC = geo.WC;
+    p.NIT = NIT;
+    p.CX = geo.CX;
+    p.NE = geo.NE;
+    p.NG = geo.NG;
+    p.occ = geo.occ;
+    p.nchunks = nchunks;
+    p.NS = NS;
+    p.nstage = nstage;
+    p.stage_bytes = (int)stage_bytes;
+    p.nblk = nblk;
+    p.nidx = (int)idx.size();
+    p.nsrc = (int)srcs.size();
+    for (int i = 0; i < p.nsrc; ++i) {
+      p.src_rows[i] = srcs[i].rows;
+      p.src_step[i] = src_step[i];
+    }
 #ifdef FRB_DEBUG_KNOBS
-  p.dbg = getenv("FRB_PANEL_DBG") ? atoi(getenv("FRB_PANEL_DBG")) : 0;
-  if (getenv("FRB_PANEL_VERBOSE"))
-    fprintf(stderr, "panel_op %s M=%d K=%d %s G=%d WR=%d WC=%d NIT=%d CX=%d NE=%d NG=%d occ=%d warps=%d+%d nchunks=%d nblk=%d smem_op=%zu stage=%zu x %d density=%.2f macs/col=%.0f (dense %d)\n",
-            f64 ? "f64" : "f32", M, K, sparse ? "sparse" : "dense", G, WR, geo.WC, NIT, geo.CX, geo.NE, geo.NG, geo.occ, geo.NG * WR * geo.WC, geo.NG,
-            nchunks, nblk, smem_op, stage_bytes, nstage, density, (double)macs, M * K);
+    p.dbg = getenv("FRB_PANEL_DBG") ? atoi(getenv("FRB_PANEL_DBG")) : 0;
+    if (getenv("FRB_PANEL_VERBOSE"))
+      fprintf(stderr, "panel_op %s M=%d K=%d %s%s G=%d WR=%d WC=%d NIT=%d CX=%d NE=%d NG=%d occ=%d warps=%d+%d nchunks=%d nblk=%d smem_op=%zu stage=%zu x %d density=%.2f macs/col=%.0f (dense %d)\n",
+              f64 ? "f64" : "f32", M, K, sparse ? "sparse" : "dense", opt.stream ? " streamed" : "", G, WR, geo.WC, NIT, geo.CX, geo.NE, geo.NG, geo.occ,
+              geo.NG * WR * geo.WC, geo.NG, nchunks, nblk, smem_op, stage_bytes, nstage, density, (double)macs, M * K);
 #endif
-  p.sparse = sparse ? 1 : 0;
-  p.macs_per_col = (double)macs;
-  p.density = density;
-  p.smem_op = smem_op;
-  p.bytes_vals = vals.size() * sizeof(T);
-  p.bytes_idx = idx.size() * 4;
-  p.bytes_off = off.size() * 4;
-  p.bytes_rowmap = rowmap.size() * 4;
-  p.bytes_chunks = chunks.size() * sizeof(ChunkDesc);
-  auto up = [](auto *&dst, const auto &h) {
-    using E = typename std::remove_reference<decltype(h[0])>::type;
-    FR_CUDA_TRY(cudaMalloc((void **)&dst, h.size() * sizeof(E)));
-    FR_CUDA_TRY(cudaMemcpy((void *)dst, h.data(), h.size() * sizeof(E), cudaMemcpyHostToDevice));
-  };
-  up(p.vals, vals);
-  up(p.idx, idx);
-  up(p.off, off);
-  up(p.rowmap, rowmap);
-  up(p.chunks, chunks);
-  return true;
+    p.sparse = sparse ? 1 : 0;
+    p.stream = opt.stream ? 1 : 0;
+    p.a_off = (int)a_off;
+    p.macs_per_col = (double)macs;
+    p.density = density;
+    p.smem_op = smem_op;
+    p.bytes_vals = opt.stream ? 0 : vals.size() * sizeof(T);
+    p.bytes_idx = idx.size() * 4;
+    p.bytes_off = off.size() * 4;
+    p.bytes_rowmap = rowmap.size() * 4;
+    p.bytes_chunks = chunks.size() * sizeof(ChunkDesc);
+    auto up = [](auto *&dst, const auto &h) {
+      using E = typename std::remove_reference<decltype(h[0])>::type;
+      FR_CUDA_TRY(cudaMalloc((void **)&dst, h.size() * sizeof(E)));
+      FR_CUDA_TRY(cudaMemcpy((void *)dst, h.data(), h.size() * sizeof(E), cudaMemcpyHostToDevice));
+    };
+    up(p.vals, vals);
+    up(p.idx, idx);
+    up(p.off, off);
+    up(p.rowmap, rowmap);
+    up(p.chunks, chunks);
+    return true;
   }
   return false;
 }
@@ -713,8 +761,9 @@ struct Acc<double, NIT, CX> {
   }
   // Dense operator: the NIT row groups of the warp share the chunk's k-blocks, so the B fragments of a k-block are loaded
   // once and feed NIT x 5 x CX DMMAs; the block's four stage rows come from the row table.
+  // `ablocks`: the chunk's packed blocks (resident image: vals + base*NS*256; streamed operator: behind the chunk in the stage).
   __device__ __forceinline__ void mac_dense(const OpSmem<double> &A, const ChunkDesc &cd, int NS, int slot0, const char *stage, int NE,
-                                            int wc, int lane) {
+                                            int wc, int lane, const char *ablocks) {
     const uint32_t pp = (uint32_t)cd.step * 128u;
     const uint32_t vs = (uint32_t)(NE >> 4) * pp;
     uint32_t lt[CX];
@@ -725,7 +774,7 @@ struct Acc<double, NIT, CX> {
       lt[cb] = lane_term(cbi, lane);
       pl[cb] = stage + (uint32_t)(cbi >> 1) * pp;
     }
-    const char *av = reinterpret_cast<const char *>(A.vals) + ((uint32_t)(cd.base * NS + slot0) * 32u + lane) * 8u;
+    const char *av = ablocks + ((uint32_t)slot0 * 32u + lane) * 8u;
     const uint32_t *rt = A.idx + cd.base * 4 + (lane & 3);
     const uint32_t as = (uint32_t)NS * 256u;
     const int nb = cd.nblk;
@@ -837,9 +886,9 @@ struct Acc<float, NIT, CX> {
   }
   // Dense operator: one B row feeds the NIT row groups of the warp.
   __device__ __forceinline__ void mac_dense(const OpSmem<float> &A, const ChunkDesc &cd, int NS, int slot0, const char *stage, int NE,
-                                            int wc, int lane) {
+                                            int wc, int lane, const char *ablocks) {
     const char *bp0 = stage + (uint32_t)(wc * 32 * CX + lane * CX) * 4u;
-    const char *ap0 = reinterpret_cast<const char *>(A.vals) + (uint32_t)(cd.base * NS + slot0) * 32u;
+    const char *ap0 = ablocks + (uint32_t)slot0 * 32u;
     const uint32_t rs = (uint32_t)NE * 4u, vs = (uint32_t)cd.step * rs, as = (uint32_t)NS * 32u;
 #pragma unroll 2
     for (int k = 0; k < cd.nrows; ++k) {

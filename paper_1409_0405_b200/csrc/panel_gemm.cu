@@ -23,13 +23,14 @@ __global__ void __launch_bounds__(32 * panel_maxw<T>(NIT, CX)) k_panel_gemm(cons
 }  // namespace
 
 template <typename T>
-bool panel_gemm_build(PanelOp<T> &op, int M, int K, const double *A, int cand, double drop_rel) {
+bool panel_gemm_build(PanelOp<T> &op, int M, int K, const double *A, int cand, double drop_rel, int stream) {
   std::vector<KSource> srcs{KSource{K}};
   PackOptions opt;
   opt.min_ne = sizeof(T) == 8 ? 16 : 32;
   opt.max_ne = sizeof(T) == 8 ? 64 : 128;
   opt.cand = cand;
   opt.drop_rel = drop_rel;
+  opt.stream = stream;
   return panel_op_build(op, M, K, A, srcs, opt, 150 * 1024);
 }
 
@@ -61,8 +62,8 @@ void panel_gemm_run(const PanelOp<T> &op, long long N, T c1, const T *B, long lo
   throw Error{FR_ESTATE, "panel_gemm_run: no kernel for this accumulator shape"};
 }
 
-template bool panel_gemm_build<double>(PanelOp<double> &, int, int, const double *, int, double);
-template bool panel_gemm_build<float>(PanelOp<float> &, int, int, const double *, int, double);
+template bool panel_gemm_build<double>(PanelOp<double> &, int, int, const double *, int, double, int);
+template bool panel_gemm_build<float>(PanelOp<float> &, int, int, const double *, int, double, int);
 template void panel_gemm_run<double>(const PanelOp<double> &, long long, double, const double *, long long, long long, double,
                                      double *, long long, long long, int, cudaStream_t);
 template void panel_gemm_run<float>(const PanelOp<float> &, long long, float, const float *, long long, long long, float, float *,

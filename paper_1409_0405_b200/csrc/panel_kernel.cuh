@@ -168,7 +168,7 @@ __device__ __forceinline__ void panel_mainloop(const PanelOp<T> &op, const Prod 
       // the operator image: five bulk copies counted on one barrier
       mbar_expect_tx(bar_img, (uint32_t)op.smem_op);
       uint32_t d = s0;
-      bulk_load(d, op.vals, (uint32_t)op.bytes_vals, bar_img);
+      if (op.bytes_vals) bulk_load(d, op.vals, (uint32_t)op.bytes_vals, bar_img);   // a streamed operator keeps no blocks here
       d += (uint32_t)op.bytes_vals;
       bulk_load(d, op.idx, (uint32_t)op.bytes_idx, bar_img);
       d += (uint32_t)op.bytes_idx;
@@ -182,13 +182,18 @@ __device__ __forceinline__ void panel_mainloop(const PanelOp<T> &op, const Prod 
     pl -= batch * npb;
     int stage = 0;
     uint32_t phase = 0;
+    const uint32_t ablk = (uint32_t)NS * (sizeof(T) == 8 ? 256u : 32u);   // bytes of one packed block row (all slots)
     for (int p = 0; p < mine; ++p) {
       for (int c = 0; c < nchunks; ++c) {
         const ChunkDesc cd = op.chunks[c];               // global (L1-resident); the image may not have landed yet
         mbar_wait(gbar + stage * 16 + 8, phase ^ 1u);    // stage is empty
         const uint32_t full = gbar + stage * 16;
-        mbar_expect_tx(full, (uint32_t)(PV * NE * (int)sizeof(T)) * (uint32_t)cd.step);
+        // streamed operator: the chunk's packed blocks follow its rows of B into the stage (one bulk copy, L2-resident source)
+        const uint32_t abytes = op.stream ? (uint32_t)cd.nblk * ablk : 0u;
+        mbar_expect_tx(full, (uint32_t)(PV * NE * (int)sizeof(T)) * (uint32_t)cd.step + abytes);
         prod.issue(cd, batch, pl, gring + stage * stage_bytes, full, NE);
+        if (abytes)
+          bulk_load(gring + stage * stage_bytes + (uint32_t)op.a_off, reinterpret_cast<const char *>(op.vals) + (size_t)cd.base * ablk, abytes, full);
         if (++stage == nstage) {
           stage = 0;
           phase ^= 1u;
@@ -231,7 +236,12 @@ __device__ __forceinline__ void panel_mainloop(const PanelOp<T> &op, const Prod 
 #endif
     {
       if (op.sparse) acc.mac_chunk(A, cc, A.chunks[cc], NS, wr * NIT, st, NE, wc, lane);
-      else acc.mac_dense(A, A.chunks[cc], NS, wr * NIT, st, NE, wc, lane);
+      else {
+        const ChunkDesc &cd = A.chunks[cc];
+        const char *ablocks = op.stream ? st + op.a_off
+                                        : reinterpret_cast<const char *>(A.vals) + (uint32_t)(cd.base * NS) * (sizeof(T) == 8 ? 256u : 32u);
+        acc.mac_dense(A, cd, NS, wr * NIT, st, NE, wc, lane, ablocks);
+      }
     }
     __syncwarp();
     if (lane == 0) mbar_arrive(gbar + stage * 16 + 8);

@@ -102,6 +102,43 @@ def test_T7_gemm_vs_numpy(prec, M, K):
         assert np.array_equal(got[:, N:], C0[:, N:].astype(np.float64))     # columns beyond N untouched
 
 
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+@pytest.mark.parametrize("M,K", [(216, 648), (126, 378), (343, 1029), (375, 125)])
+def test_streamed_operator_equals_resident_row_blocks_bitwise(prec, M, K, monkeypatch):
+    """Operators whose packed image exceeds shared memory run either as row blocks of A with a resident image or with the image
+    streamed through the TMA ring (FRB_GEMM_STREAM = 0 / 1 forces the form; fr_gemm_plan_create otherwise times both).  The
+    k-blocks and their order are the same in both forms and for every chunk height, so the results must be bit-identical; both
+    are checked against the float64 product."""
+    import torch
+    from paper_1409_0405_b200 import binding
+    rng = np.random.Generator(np.random.PCG64(cases.SEEDS["c4"] + 7 * M + K))
+    tdt = torch.float64 if prec == "f64" else torch.float32
+    ndt = np.float64 if prec == "f64" else np.float32
+    N, ld = 5 * 1237, 5 * 1237 + 15
+    A = rng.standard_normal((M, K))
+    B = rng.uniform(-1, 1, (K, ld)).astype(ndt)
+    C0 = rng.uniform(-1, 1, (M, ld)).astype(ndt)
+    dB = torch.from_numpy(B).cuda()
+    monkeypatch.setenv("FRB_AUTOTUNE", "0")
+    out = {}
+    for form in ("0", "1"):
+        monkeypatch.setenv("FRB_GEMM_STREAM", form)
+        plan = binding.GemmPlan(A, prec)
+        desc = plan.describe()
+        assert ("streamed" in desc) == (form == "1"), desc
+        dC = torch.from_numpy(C0).cuda()
+        plan.run(dB.data_ptr(), ld, dC.data_ptr(), ld, N, c1=1.0, c2=0.5)
+        torch.cuda.synchronize()
+        out[form] = dC.cpu().numpy()
+        plan.close()
+    assert np.array_equal(out["0"], out["1"])
+    Ar = A.astype(ndt).astype(np.float64)
+    ref = Ar @ B[:, :N].astype(np.float64) + 0.5 * C0[:, :N].astype(np.float64)
+    scale = np.abs(Ar) @ np.abs(B[:, :N].astype(np.float64)) + 0.5 * np.abs(C0[:, :N])
+    assert np.abs(out["1"][:, :N].astype(np.float64) - ref).max() <= (1e-13 if prec == "f64" else 1e-5) * scale.max()
+    assert np.array_equal(out["1"][:, N:], C0[:, N:])
+
+
 # ---------------------------------------------------------------------------- RHS parity
 @pytest.mark.parametrize("mode", ["unfused", "fused"])
 def test_config1_rhs_fp64(mode):
