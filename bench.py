@@ -294,7 +294,8 @@ def _probe_flop_peaks():
     dm = binding.probe_dmma()
     FLOP_PEAK["f64"] = (dm, "tensor", "fr_probe_dmma (mma.m8n8k4.f64 chains), measured in this run")
     FLOP_PEAK["f32"] = (pk["fp32_tflops"], "alu", "fr_probe_peaks (FFMA chains), measured in this run")
-    return dict(fp64_tensor_tflops=dm, fp64_dfma_tflops=pk["fp64_tflops"], fp32_ffma_tflops=pk["fp32_tflops"], copy_gbs=pk["copy_gbs"])
+    alt = binding.probe_fp32_paths()   # FFMA2 (what the FP32 products issue), the same beside integer work, legacy TF32 mma
+    return dict(fp64_tensor_tflops=dm, fp64_dfma_tflops=pk["fp64_tflops"], fp32_ffma_tflops=pk["fp32_tflops"], copy_gbs=pk["copy_gbs"], **alt)
 
 
 def _groups(kernels):

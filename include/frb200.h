@@ -267,6 +267,12 @@ fr_status fr_probe_peaks(double *fp64_tflops, double *fp32_tflops, double *copy_
  * register-resident chains, 512 flops per warp instruction.  The denominator of compute-bound FP64 roofline fractions. */
 fr_status fr_probe_dmma(double *fp64_tensor_tflops);
 
+/* The FP32 alternatives weighed in DESIGN.md section 6, as register-resident chains (TFLOP/s): packed fma.rn.f32x2 (FFMA2: what the
+ * FP32 operator products use); FFMA and FFMA2 chains with eight integer multiply-adds beside every sixteen FMAs (the issue slots that
+ * address arithmetic costs a multiply loop); the legacy TF32 tensor path mma.sync.m16n8k8 (dense rate; an error-compensated 3xTF32
+ * product would run at a third of it).  Any pointer may be NULL. */
+fr_status fr_probe_fp32_paths(double *ffma2_tflops, double *ffma_mixed_tflops, double *ffma2_mixed_tflops, double *tf32_mma_tflops);
+
 #ifdef __cplusplus
 }
 #endif

@@ -67,7 +67,7 @@ SYMBOLS = ["fr_profile_kernels", "fr_rk_step_host", "fr_setup", "fr_state_layout
            "fr_sync", "fr_launch_count", "fr_profile_rhs", "fr_last_error", "fr_global_error", "fr_destroy",
            "fr_gemm", "fr_gemm_plan_create", "fr_gemm_plan_run", "fr_gemm_plan_destroy", "fr_probe_peaks", "fr_probe_dmma",
            "fr_profile_stage_kernels", "fr_check_finite", "fr_plan_describe", "fr_rhs_phase", "fr_rk_stage_phase",
-           "fr_halo_buffers", "fr_halo_set_peers", "fr_gemm_static", "fr_gemm_plan_describe"]
+           "fr_halo_buffers", "fr_halo_set_peers", "fr_gemm_static", "fr_gemm_plan_describe", "fr_probe_fp32_paths"]
 
 _lib = None
 
@@ -113,6 +113,7 @@ def load():
     lib.fr_gemm_plan_destroy.restype = None
     lib.fr_probe_peaks.argtypes = [_dp, _dp, _dp]
     lib.fr_probe_dmma.argtypes = [_dp]
+    lib.fr_probe_fp32_paths.argtypes = [_dp, _dp, _dp, _dp]
     lib.fr_profile_stage_kernels.argtypes = [vp, C.c_int32, C.POINTER(fr_kernel_stat), C.c_int32, _i32p]
     lib.fr_check_finite.argtypes = [vp, _i64p]
     lib.fr_plan_describe.argtypes = [vp, C.c_char_p, C.c_int64]
@@ -407,6 +408,16 @@ def probe_dmma():
     if st != FR_OK:
         raise FrError(st, "fr_probe_dmma failed")
     return a.value
+
+
+def probe_fp32_paths():
+    """fr_probe_fp32_paths: TFLOP/s of FFMA2 chains, FFMA / FFMA2 chains with integer work beside them, and mma.sync TF32."""
+    lib = load()
+    v = [C.c_double() for _ in range(4)]
+    st = lib.fr_probe_fp32_paths(*[C.byref(x) for x in v])
+    if st != FR_OK:
+        raise FrError(st, "fr_probe_fp32_paths failed")
+    return dict(zip(("ffma2_tflops", "ffma_mixed_tflops", "ffma2_mixed_tflops", "tf32_mma_tflops"), (x.value for x in v)))
 
 
 def probe_peaks():

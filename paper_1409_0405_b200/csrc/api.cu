@@ -1147,7 +1147,7 @@ struct Ctx : CtxBase {
     auto add = [&](const char *type, const char *what, const PanelOp<T> &op) {
       if (!op.ok()) return;
       snprintf(line, sizeof line, "%s %s %s %dx%d %s warps=%dx%dx%d+%d NIT=%d CX=%d NE=%d stages=%dx%d B occ=%d\n", sizeof(T) == 8 ? "f64" : "f32",
-               type, what, op.M, op.K, op.sparse ? "k-lists" : (op.stream ? "dense, streamed" : "dense"), op.NG, op.WR, op.WC, op.NG, op.NIT, op.CX, op.NE, op.nstage,
+               type, what, op.M, op.K, op.sparse ? "k-lists" : (op.streamed() ? "dense, streamed" : "dense"), op.NG, op.WR, op.WC, op.NG, op.NIT, op.CX, op.NE, op.nstage,
                op.stage_bytes, op.occ);
       out += line;
     };
@@ -1185,7 +1185,7 @@ std::string gemm_plan_describe(const GemmPlan<T> &p) {
   char line[256];
   auto add = [&](const PanelOp<T> &op, int row0) {
     snprintf(line, sizeof line, "%s rows %d..%d of %dx%d %s warps=%dx%dx%d+%d NIT=%d CX=%d NE=%d chunks=%d stages=%dx%d B\n", sizeof(T) == 8 ? "f64" : "f32",
-             row0, row0 + op.M - 1, p.M, p.K, op.sparse ? "k-lists" : (op.stream ? "dense, streamed" : "dense"), op.NG, op.WR, op.WC, op.NG,
+             row0, row0 + op.M - 1, p.M, p.K, op.sparse ? "k-lists" : (op.streamed() ? "dense, streamed" : "dense"), op.NG, op.WR, op.WC, op.NG,
              op.NIT, op.CX, op.NE, op.nchunks, op.nstage, op.stage_bytes);
     out += line;
   };

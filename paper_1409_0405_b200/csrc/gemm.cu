@@ -404,7 +404,7 @@ struct TuneScratch {
 template <typename T>
 void tune_geometry(GemmPlan<T> &p, const double *A_host, double drop_rel, TuneScratch<T> &sc) {
   PanelOp<T> *cur = p.pop ? p.pop : p.part[0];
-  const int M = cur->M, K = p.K, stream = cur->stream;
+  const int M = cur->M, K = p.K, stream = cur->streamed();
   auto time_op = [&](const PanelOp<T> &op) {
     return sc.time([&] { panel_gemm_run(op, sc.N, T(1), sc.B, sc.N, 0, T(0), sc.C, sc.N, 0, 1, (cudaStream_t)0); });
   };
@@ -443,7 +443,7 @@ void gemm_plan_tune(GemmPlan<T> &p, const double *A_host, double drop_rel) {
   TuneScratch<T> sc;
   if (!sc.init(p.M, p.K)) return;
   tune_geometry(p, A_host, drop_rel, sc);
-  const int cur_stream = (p.pop ? p.pop : p.part[0])->stream;
+  const int cur_stream = (p.pop ? p.pop : p.part[0])->streamed();
   if ((p.pop && !cur_stream) || getenv("FRB_GEMM_STREAM")) return;   // the whole image is resident, or the form is forced
   GemmPlan<T> q;
   if (!plan_variant(q, p.M, p.K, A_host, drop_rel, 1 - cur_stream, 1)) return;

@@ -61,9 +61,6 @@ struct PanelOp {
   int dbg = 0;                           // measurement aid (env FRB_PANEL_DBG): 1 skip multiply, 2 skip epilogue
 #endif
   int sparse = 0;                        // 1: per-group k-lists (idx/off); 0: dense, all slots share the chunk's k-blocks
-  int stream = 0;                        // 1: the operator does not stay in shared memory: the packed blocks of a chunk travel through
-                                         //    the ring behind the chunk's rows of B (dense packing only), at stage offset a_off
-  int a_off = 0;
   int nsrc = 0;
   int src_rows[PANEL_MAXSRC] = {0, 0};   // rows of each stacked source
   int src_step[PANEL_MAXSRC] = {0, 0};   // rows per chunk (TMA box height) of each source
@@ -77,6 +74,10 @@ struct PanelOp {
   size_t smem_op = 0;                    // bytes of the operator image in shared memory
   size_t bytes_vals = 0, bytes_idx = 0, bytes_off = 0, bytes_rowmap = 0, bytes_chunks = 0;   // each a multiple of 16
   bool ok() const { return vals != nullptr; }
+  // Streamed operator (plain products whose image exceeds shared memory): the packed blocks do not stay in shared memory
+  // (bytes_vals = 0) but travel through the ring behind each chunk's rows of B (dense packing, one source), at stage offset a_off().
+  __host__ __device__ bool streamed() const { return vals != nullptr && bytes_vals == 0; }
+  __host__ __device__ int a_off() const { return (PV * NE * src_step[0] * (int)sizeof(T) + 127) / 128 * 128; }
 };
 
 template <typename T>
@@ -466,7 +467,7 @@ bool panel_op_build(PanelOp<T> &p, int M, int K, const double *A, const std::vec
     std::vector<int> off;
     long long macs = 0;
     int nblk = 0, nstage = 0;
-    size_t smem_op = 0, stage_bytes = 0, a_off = 0;
+    size_t smem_op = 0, stage_bytes = 0;
     // ---- pack for the current chunks; false if the result does not fit
     auto pack = [&]() {
       vals.clear();
@@ -548,7 +549,7 @@ bool panel_op_build(PanelOp<T> &p, int M, int K, const double *A, const std::vec
         bmax = std::max(bmax, (size_t)PV * geo.NE * c.step * sizeof(T));
         amax_b = std::max(amax_b, (size_t)c.nblk * ablk);
       }
-      a_off = (bmax + 127) / 128 * 128;
+      const size_t a_off = (bmax + 127) / 128 * 128;   // = PanelOp::a_off(): one source, so bmax is the box of src_step[0] rows
       stage_bytes = (a_off + (opt.stream ? amax_b : 0) + 1023) / 1024 * 1024;
       // 1 kB to align the ring, the ring, 256 B of mbarriers
       const size_t fixed = 1024 + (smem_op + 1023) / 1024 * 1024 + 256;
@@ -610,8 +611,6 @@ bool panel_op_build(PanelOp<T> &p, int M, int K, const double *A, const std::vec
               geo.NG * WR * geo.WC, geo.NG, nchunks, nblk, smem_op, stage_bytes, nstage, density, (double)macs, M * K);
 #endif
     p.sparse = sparse ? 1 : 0;
-    p.stream = opt.stream ? 1 : 0;
-    p.a_off = (int)a_off;
     p.macs_per_col = (double)macs;
     p.density = density;
     p.smem_op = smem_op;
@@ -677,12 +676,13 @@ __device__ __forceinline__ void op_smem_carve(char *base, const PanelOp<T> &op, 
 // ---- accumulators and the multiply-accumulate core.  A stage holds the chunk as planes (tma.cuh):
 //   FP64: plane(v, cb16) = v*(NE/16) + cb16, `pp` = step*128 bytes each, rows of 16 doubles, 128-byte swizzle;
 //   FP32: plane(v) of step rows of NE floats.
-template <typename T, int NIT, int CX>
+// PACKED selects the FP32 form (packed pairs / scalar); FP64 has one form
+template <typename T, int NIT, int CX, bool PACKED = true>
 struct Acc;
 
 // FP64: per slot, CX column blocks of 8 elements x 5 variables, one m8n8k4 C fragment (2 doubles) each.
-template <int NIT, int CX>
-struct Acc<double, NIT, CX> {
+template <int NIT, int CX, bool PACKED>
+struct Acc<double, NIT, CX, PACKED> {
   double c[NIT][CX][PV][2];
   __device__ __forceinline__ void zero() {
 #pragma unroll
@@ -761,9 +761,10 @@ struct Acc<double, NIT, CX> {
   }
   // Dense operator: the NIT row groups of the warp share the chunk's k-blocks, so the B fragments of a k-block are loaded
   // once and feed NIT x 5 x CX DMMAs; the block's four stage rows come from the row table.
-  // `ablocks`: the chunk's packed blocks (resident image: vals + base*NS*256; streamed operator: behind the chunk in the stage).
+  // STREAM: the chunk's packed blocks sit behind the chunk in the stage (offset a_off) instead of in the resident image.
+  template <bool STREAM>
   __device__ __forceinline__ void mac_dense(const OpSmem<double> &A, const ChunkDesc &cd, int NS, int slot0, const char *stage, int NE,
-                                            int wc, int lane, const char *ablocks) {
+                                            int wc, int lane, int a_off) {
     const uint32_t pp = (uint32_t)cd.step * 128u;
     const uint32_t vs = (uint32_t)(NE >> 4) * pp;
     uint32_t lt[CX];
@@ -774,7 +775,8 @@ struct Acc<double, NIT, CX> {
       lt[cb] = lane_term(cbi, lane);
       pl[cb] = stage + (uint32_t)(cbi >> 1) * pp;
     }
-    const char *av = ablocks + ((uint32_t)slot0 * 32u + lane) * 8u;
+    const char *av = STREAM ? stage + a_off + ((uint32_t)slot0 * 32u + lane) * 8u
+                            : reinterpret_cast<const char *>(A.vals) + ((uint32_t)(cd.base * NS + slot0) * 32u + lane) * 8u;
     const uint32_t *rt = A.idx + cd.base * 4 + (lane & 3);
     const uint32_t as = (uint32_t)NS * 256u;
     const int nb = cd.nblk;
@@ -835,9 +837,151 @@ struct Acc<double, NIT, CX> {
   static constexpr int NSLOT = NIT;
 };
 
-// FP32: per slot, 8 rows x 5 variables x CX elements per lane.
+// ---- packed FP32 pairs: fma.rn.f32x2 (FFMA2, sm_100) does two IEEE FP32 fused multiply-adds per instruction -- the same
+// results as two FFMA at the same pipe rate for half the issue slots, which is what the FP32 multiply loops are short of.
+__device__ __forceinline__ void ffma2(unsigned long long &c, unsigned long long a, unsigned long long b) {
+  asm("fma.rn.f32x2 %0, %1, %2, %0;" : "+l"(c) : "l"(a), "l"(b));
+}
+__device__ __forceinline__ unsigned long long pack2(float lo, float hi) {
+  unsigned long long r;
+  asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi));
+  return r;
+}
+__device__ __forceinline__ void unpack2(unsigned long long v, float &lo, float &hi) {
+  asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v));
+}
+
+// FP32: per slot, 8 rows x 5 variables x CX elements per lane; rows 2q and 2q+1 share a register pair (the operator's packed
+// columns hold them next to each other, so a pair of operator values is one 64-bit half of the LDS.128 that fetches it).
 template <int NIT, int CX>
-struct Acc<float, NIT, CX> {
+struct Acc<float, NIT, CX, true> {
+  unsigned long long c[NIT][4][PV][CX];
+  __device__ __forceinline__ void zero() {
+#pragma unroll
+    for (int i = 0; i < NIT; ++i)
+#pragma unroll
+      for (int q = 0; q < 4; ++q)
+#pragma unroll
+        for (int v = 0; v < PV; ++v)
+#pragma unroll
+          for (int j = 0; j < CX; ++j) c[i][q][v][j] = 0ull;
+  }
+  // the chunk's B values of one stage row for this lane, each duplicated into both halves of a pair
+  __device__ __forceinline__ static void load_b(const char *bp, uint32_t vs, unsigned long long (&bd)[PV][CX]) {
+#pragma unroll
+    for (int v = 0; v < PV; ++v) {
+      if (CX == 2) {
+        const float2 t = *reinterpret_cast<const float2 *>(bp);
+        bd[v][0] = pack2(t.x, t.x);
+        bd[v][CX - 1] = pack2(t.y, t.y);
+      } else {
+        const float t = *reinterpret_cast<const float *>(bp);
+        bd[v][0] = pack2(t, t);
+      }
+      bp += vs;
+    }
+  }
+  // 8 operator values (one packed column of a slot) times the row of B
+  __device__ __forceinline__ void mac_col(int i, const char *ap, const unsigned long long (&bd)[PV][CX]) {
+    const ulonglong2 a01 = *reinterpret_cast<const ulonglong2 *>(ap);
+    const ulonglong2 a23 = *reinterpret_cast<const ulonglong2 *>(ap + 16);
+    const unsigned long long aq[4] = {a01.x, a01.y, a23.x, a23.y};
+#pragma unroll
+    for (int q = 0; q < 4; ++q)
+#pragma unroll
+      for (int v = 0; v < PV; ++v)
+#pragma unroll
+        for (int j = 0; j < CX; ++j) ffma2(c[i][q][v][j], aq[q], bd[v][j]);
+  }
+  __device__ __forceinline__ void mac_chunk(const OpSmem<float> &A, int chunk, const ChunkDesc &cd, int NS, int slot0, const char *stage,
+                                            int NE, int wc, int lane) {
+    const char *bcol = stage + (uint32_t)(wc * 32 * CX + lane * CX) * 4u;
+    const char *avp = reinterpret_cast<const char *>(A.vals);
+    const uint32_t vs = (uint32_t)cd.step * (uint32_t)NE * 4u;
+#pragma unroll
+    for (int i = 0; i < NIT; ++i) {
+      const int b0 = A.off[chunk * NS + slot0 + i], b1 = A.off[chunk * NS + slot0 + i + 1];
+#pragma unroll 2
+      for (int b = b0; b < b1; ++b) {
+        unsigned long long bd[PV][CX];
+        load_b(bcol + A.idx[b], vs, bd);
+        mac_col(i, avp + (uint32_t)b * 32u, bd);
+      }
+    }
+  }
+  // Dense operator: one B row feeds the NIT row groups of the warp.
+  template <bool STREAM>
+  __device__ __forceinline__ void mac_dense(const OpSmem<float> &A, const ChunkDesc &cd, int NS, int slot0, const char *stage, int NE,
+                                            int wc, int lane, int a_off) {
+    const char *bp0 = stage + (uint32_t)(wc * 32 * CX + lane * CX) * 4u;
+    const char *ap0 = STREAM ? stage + a_off + (uint32_t)slot0 * 32u
+                             : reinterpret_cast<const char *>(A.vals) + (uint32_t)(cd.base * NS + slot0) * 32u;
+    const uint32_t rs = (uint32_t)NE * 4u, vs = (uint32_t)cd.step * rs, as = (uint32_t)NS * 32u;
+#pragma unroll 2
+    for (int k = 0; k < cd.nrows; ++k) {
+      unsigned long long bd[PV][CX];
+      load_b(bp0 + (uint32_t)k * rs, vs, bd);
+      const char *ap = ap0 + (uint32_t)k * as;
+#pragma unroll
+      for (int i = 0; i < NIT; ++i) mac_col(i, ap + i * 32, bd);
+    }
+  }
+  // rows 2q and 2q+1 of slot i as float tiles
+  __device__ __forceinline__ void rows_of(int i, int q, float (&t0)[PV][CX], float (&t1)[PV][CX]) const {
+#pragma unroll
+    for (int v = 0; v < PV; ++v)
+#pragma unroll
+      for (int j = 0; j < CX; ++j) unpack2(c[i][q][v][j], t0[v][j], t1[v][j]);
+  }
+  template <typename F>
+  __device__ __forceinline__ void foreach_tile(int wc, int lane, F &&f) {
+#pragma unroll
+    for (int i = 0; i < NIT; ++i)
+#pragma unroll
+      for (int q = 0; q < 4; ++q) {
+        float t0[PV][CX], t1[PV][CX];
+        rows_of(i, q, t0, t1);
+        f(i, 2 * q, wc * 32 * CX + lane * CX, t0);
+        f(i, 2 * q + 1, wc * 32 * CX + lane * CX, t1);
+      }
+  }
+  template <typename F>
+  __device__ __forceinline__ void foreach_coord(int wc, int lane, F &&f) {
+#pragma unroll
+    for (int i = 0; i < NIT; ++i)
+#pragma unroll
+      for (int r = 0; r < 8; ++r) f(i, r, wc * 32 * CX + lane * CX);
+  }
+  template <typename F>
+  __device__ __forceinline__ void foreach_triple(int wc, int lane, F &&f) {
+#pragma unroll
+    for (int t = 0; t < NIT / 3; ++t)
+#pragma unroll
+      for (int q = 0; q < 4; ++q) {
+        float a0[PV][CX], a1[PV][CX], b0[PV][CX], b1[PV][CX], c0[PV][CX], c1[PV][CX];
+        rows_of(3 * t, q, a0, a1);
+        rows_of(3 * t + 1, q, b0, b1);
+        rows_of(3 * t + 2, q, c0, c1);
+        f(t, 2 * q, wc * 32 * CX + lane * CX, a0, b0, c0);
+        f(t, 2 * q + 1, wc * 32 * CX + lane * CX, a1, b1, c1);
+      }
+  }
+  template <typename G>
+  __device__ __forceinline__ void foreach_row(int lane, G &&g) {
+#pragma unroll
+    for (int i = 0; i < NIT; ++i)
+#pragma unroll
+      for (int r = 0; r < 8; ++r) g(i, r, r);
+  }
+  static constexpr int EW = CX;
+  static constexpr int ROWS = 8;
+  static constexpr int NSLOT = NIT;
+};
+
+// FP32, scalar form (FFMA): per slot, 8 rows x 5 variables x CX elements per lane.  Kept for the gradient kernels, whose 12-warp /
+// 168-register budget has no room for the register-pair alignment of the packed form (it spills into the multiply loop there).
+template <int NIT, int CX>
+struct Acc<float, NIT, CX, false> {
   float c[NIT][8][PV][CX];
   __device__ __forceinline__ void zero() {
 #pragma unroll
@@ -885,10 +1029,12 @@ struct Acc<float, NIT, CX> {
     }
   }
   // Dense operator: one B row feeds the NIT row groups of the warp.
+  template <bool STREAM>
   __device__ __forceinline__ void mac_dense(const OpSmem<float> &A, const ChunkDesc &cd, int NS, int slot0, const char *stage, int NE,
-                                            int wc, int lane, const char *ablocks) {
+                                            int wc, int lane, int a_off) {
     const char *bp0 = stage + (uint32_t)(wc * 32 * CX + lane * CX) * 4u;
-    const char *ap0 = ablocks + (uint32_t)slot0 * 32u;
+    const char *ap0 = STREAM ? stage + a_off + (uint32_t)slot0 * 32u
+                             : reinterpret_cast<const char *>(A.vals) + (uint32_t)(cd.base * NS + slot0) * 32u;
     const uint32_t rs = (uint32_t)NE * 4u, vs = (uint32_t)cd.step * rs, as = (uint32_t)NS * 32u;
 #pragma unroll 2
     for (int k = 0; k < cd.nrows; ++k) {

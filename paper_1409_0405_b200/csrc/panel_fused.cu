@@ -288,7 +288,8 @@ struct alignas(64) GradArgs {
 template <typename T, int NIT, int CX>
 __global__ void __launch_bounds__(32 * panel_maxw<T>(NIT, CX, true)) k_fused_grad(const __grid_constant__ GradArgs<T> a) {
   extern __shared__ __align__(1024) char panel_smem[];
-  panel_mainloop<T, NIT, CX>(a.op, a.prod, a.epi, a.npanels, 1, panel_smem);
+  // FP32: the scalar accumulator form (panel.cuh: the packed pairs do not fit this kernel's register budget)
+  panel_mainloop<T, NIT, CX, TmaProducer<T>, GradEpilogue<T>, false>(a.op, a.prod, a.epi, a.npanels, 1, panel_smem);
 }
 
 }  // namespace

@@ -14,10 +14,10 @@ struct alignas(64) PlainArgs {
   int nbatch;
 };
 
-template <typename T, int NIT, int CX>
+template <typename T, int NIT, int CX, bool STREAM>
 __global__ void __launch_bounds__(32 * panel_maxw<T>(NIT, CX)) k_panel_gemm(const __grid_constant__ PlainArgs<T> a) {
   extern __shared__ __align__(1024) char panel_smem[];
-  panel_mainloop<T, NIT, CX>(a.op, a.prod, a.epi, a.npanels, a.nbatch, panel_smem);
+  panel_mainloop<T, NIT, CX, TmaProducer<T>, PlainEpilogue<T>, true, STREAM>(a.op, a.prod, a.epi, a.npanels, a.nbatch, panel_smem);
 }
 
 }  // namespace
@@ -50,7 +50,8 @@ void panel_gemm_run(const PanelOp<T> &op, long long N, T c1, const T *B, long lo
   a.nbatch = nbatch;
 #define FR_CASE(NIT_, CX_)                                                                        \
   if (op.NIT == NIT_ && op.CX == CX_) {                                                           \
-    panel_launch(k_panel_gemm<T, NIT_, CX_>, a, op, a.npanels * a.nbatch, s);                     \
+    if (op.streamed()) panel_launch(k_panel_gemm<T, NIT_, CX_, true>, a, op, a.npanels * a.nbatch, s); \
+    else panel_launch(k_panel_gemm<T, NIT_, CX_, false>, a, op, a.npanels * a.nbatch, s);          \
     return;                                                                                       \
   }
   if constexpr (sizeof(T) == 8) {

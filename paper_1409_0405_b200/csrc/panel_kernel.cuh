@@ -124,7 +124,9 @@ struct PlainEpilogue {
 
 // ---- the persistent main loop.  Grid = any number of CTAs; CTA b, group g owns panels b*NG+g, b*NG+g + grid*NG, ...
 // `prod` must refer to the kernel's __grid_constant__ parameter.
-template <typename T, int NIT, int CX, class Prod, class Epi>
+// STREAM: the operator's packed blocks travel through the ring (PanelOp::stream; plain products only -- a compile-time switch so that
+// the kernels of resident operators carry none of it).
+template <typename T, int NIT, int CX, class Prod, class Epi, bool PACKED = true, bool STREAM = false>
 __device__ __forceinline__ void panel_mainloop(const PanelOp<T> &op, const Prod &prod, const Epi &epi, long long npanels_per_batch,
                                                int nbatch, char *smem_raw) {
   const int WC = op.WC, NS = op.NS, NE = op.NE, NG = op.NG;
@@ -168,7 +170,7 @@ __device__ __forceinline__ void panel_mainloop(const PanelOp<T> &op, const Prod 
       // the operator image: five bulk copies counted on one barrier
       mbar_expect_tx(bar_img, (uint32_t)op.smem_op);
       uint32_t d = s0;
-      if (op.bytes_vals) bulk_load(d, op.vals, (uint32_t)op.bytes_vals, bar_img);   // a streamed operator keeps no blocks here
+      if (!STREAM) bulk_load(d, op.vals, (uint32_t)op.bytes_vals, bar_img);   // a streamed operator keeps no blocks here
       d += (uint32_t)op.bytes_vals;
       bulk_load(d, op.idx, (uint32_t)op.bytes_idx, bar_img);
       d += (uint32_t)op.bytes_idx;
@@ -189,11 +191,11 @@ __device__ __forceinline__ void panel_mainloop(const PanelOp<T> &op, const Prod 
         mbar_wait(gbar + stage * 16 + 8, phase ^ 1u);    // stage is empty
         const uint32_t full = gbar + stage * 16;
         // streamed operator: the chunk's packed blocks follow its rows of B into the stage (one bulk copy, L2-resident source)
-        const uint32_t abytes = op.stream ? (uint32_t)cd.nblk * ablk : 0u;
+        const uint32_t abytes = STREAM ? (uint32_t)cd.nblk * ablk : 0u;
         mbar_expect_tx(full, (uint32_t)(PV * NE * (int)sizeof(T)) * (uint32_t)cd.step + abytes);
         prod.issue(cd, batch, pl, gring + stage * stage_bytes, full, NE);
-        if (abytes)
-          bulk_load(gring + stage * stage_bytes + (uint32_t)op.a_off, reinterpret_cast<const char *>(op.vals) + (size_t)cd.base * ablk, abytes, full);
+        if (STREAM)
+          bulk_load(gring + stage * stage_bytes + (uint32_t)op.a_off(), reinterpret_cast<const char *>(op.vals) + (size_t)cd.base * ablk, abytes, full);
         if (++stage == nstage) {
           stage = 0;
           phase ^= 1u;
@@ -222,7 +224,7 @@ __device__ __forceinline__ void panel_mainloop(const PanelOp<T> &op, const Prod 
     if (grp == 1) asm volatile("bar.sync 3, %0;" ::"r"(2 * nwc * 32) : "memory");
     else if (stagger_q < 0) asm volatile("bar.arrive 3, %0;" ::"r"(2 * nwc * 32) : "memory");
   }
-  Acc<T, NIT, CX> acc;
+  Acc<T, NIT, CX, PACKED> acc;
   acc.zero();
   int stage = 0, cc = 0;
   uint32_t phase = 0;
@@ -236,12 +238,7 @@ __device__ __forceinline__ void panel_mainloop(const PanelOp<T> &op, const Prod 
 #endif
     {
       if (op.sparse) acc.mac_chunk(A, cc, A.chunks[cc], NS, wr * NIT, st, NE, wc, lane);
-      else {
-        const ChunkDesc &cd = A.chunks[cc];
-        const char *ablocks = op.stream ? st + op.a_off
-                                        : reinterpret_cast<const char *>(A.vals) + (uint32_t)(cd.base * NS) * (sizeof(T) == 8 ? 256u : 32u);
-        acc.mac_dense(A, cd, NS, wr * NIT, st, NE, wc, lane, ablocks);
-      }
+      else acc.template mac_dense<STREAM>(A, A.chunks[cc], NS, wr * NIT, st, NE, wc, lane, STREAM ? op.a_off() : 0);
     }
     __syncwarp();
     if (lane == 0) mbar_arrive(gbar + stage * 16 + 8);
