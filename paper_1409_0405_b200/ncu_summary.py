@@ -2,6 +2,7 @@
 `roofline.traffic`).
 
   python -m paper_1409_0405_b200.ncu_summary REPORT.ncu-rep --bench BENCH.json --prec f64 [--csv OUT.csv] [--append]
+  python -m paper_1409_0405_b200.ncu_summary --launches LAUNCHES.csv      (markdown table of an ncu launch list)
 
 REPORT.ncu-rep: `ncu --set full` capture of the first launches of bench.py's timed region (one right-hand side = every kernel from
 S1 to the last fused divergence kernel; the command is recorded in the .md next to the CSV).  BENCH.json: the line
@@ -36,7 +37,33 @@ def to_ms(value, unit):
     return v * {"ns": 1e-6, "us": 1e-3, "ms": 1.0, "s": 1e3}.get(unit, 1.0)
 
 
+def launch_table(path):
+    """Markdown table of an `ncu --metrics gpu__time_duration.sum --csv` launch list: launches, total and mean time, share per kernel."""
+    lines = [l for l in open(path) if l.startswith('"')]
+    rows = list(csv.reader(io.StringIO("".join(lines))))
+    col = {h: i for i, h in enumerate(rows[0])}
+    agg = {}
+    for r in rows[1:]:
+        if r[col["Metric Name"]] != "gpu__time_duration.sum":
+            continue
+        name = re.sub(r"\(.*", "", r[col["Kernel Name"]]).split("::")[-1].replace("void ", "")
+        key = "`%s` x%s" % (name, r[col["Block Size"]].strip("()").split(",")[0])
+        ms = to_ms(r[col["Metric Value"]], r[col["Metric Unit"]])
+        a = agg.setdefault(key, [0, 0.0])
+        a[0] += 1
+        a[1] += ms
+    tot = sum(a[1] for a in agg.values())
+    out = ["| kernel x threads per CTA | launches | total ms | share | mean ms |", "|---|---|---|---|---|"]
+    for k, (n, ms) in sorted(agg.items(), key=lambda kv: -kv[1][1]):
+        out.append("| %s | %d | %.3f | %.1f %% | %.3f |" % (k, n, ms, 100 * ms / tot, ms / n))
+    out.append("| total | %d | %.3f | | |" % (sum(a[0] for a in agg.values()), tot))
+    return "\n".join(out)
+
+
 def main():
+    if len(sys.argv) == 3 and sys.argv[1] == "--launches":
+        print(launch_table(sys.argv[2]))
+        return
     ap = argparse.ArgumentParser()
     ap.add_argument("report")
     ap.add_argument("--bench", required=True)
