@@ -1,6 +1,7 @@
 """Per-kernel roofline table of one right-hand side as markdown (what `profiles/r02_a_kernels.md` holds).
 
   python -m paper_1409_0405_b200.kernel_table BENCH.json [--traffic TRAFFIC.csv] [--prev PREV_BENCH.json] > table.md
+  python -m paper_1409_0405_b200.kernel_table --gemm BENCH.json          (the `gemm` object of the line as a table)
 
 BENCH.json: the line `python bench.py --kernels` printed (per-kernel CUDA-event times, algorithmic bytes and flops of
 `fr_profile_stage_kernels`, the peaks measured in the same run, the plans `fr_setup` chose).  TRAFFIC.csv: the DRAM bytes and pipe
@@ -22,7 +23,50 @@ def load(path):
     raise SystemExit("no bench line in %s" % path)
 
 
+def gemm_table(d):
+    """The `gemm` object of a bench line (operator product alone, eight shapes x two precisions) as a markdown table."""
+    out = ["| shape | M x K | N | FP64 ms | GB/s | TF | bound | frac | library ms | FP32 ms | GB/s | TF | bound | frac | library ms |",
+           "|" + "---|" * 15]
+    rows = {}
+    for g in d["gemm"]:
+        rows.setdefault((g["shape"], g["M"], g["K"]), {})[g["dtype"]] = g
+    for (shape, M, K), r in rows.items():
+        cells = [shape, "%d x %d" % (M, K), "%d" % r["f64"]["N"]]
+        for prec in ("f64", "f32"):
+            g = r[prec]
+            cells += ["%.3f" % g["ms"], "%.0f" % g["gbs"], "%.1f" % g["tflops"], g["bound"], "%.2f" % g["frac"], "%.3f" % g["library_gemm_ms"]]
+        out.append("| " + " | ".join(cells) + " |")
+    return "\n".join(out)
+
+
+def single_table(d):
+    """A line that carries one precision only (bench.py --workload config5): headline, per-kernel table, plan."""
+    prec = d["dtype"]
+    ks = d["kernels_" + prec]
+    hbm = d["roofline"]["hbm"]["peak"]
+    peak = d["peaks"]["fp64_tensor_tflops" if prec == "f64" else "fp32_ffma_tflops"]
+    tot = sum(k["ms"] for k in ks)
+    out = ["Workload: %s; %d DOF; %s; dt = %g." % (d["config"]["workload"], d["config"]["dof"], prec.upper(), d["config"]["dt"]), "",
+           "* **%.3f GDOF-RHS/s** (%.1f ms per RK45 step, %d kernel launches in the timed region of %d steps). SM clock %.0f of %.0f MHz, reasons %s."
+           % (d["value"], d["ms_per_step"], d["gpu_launches"], d["steps"], d["clocks"]["sm_mhz"], d["clocks"]["sm_max_mhz"], d["clocks"]["reasons"]),
+           "* end to end through `fr_rk_step_host` (%.2f GB of pinned host state in, one step, %.2f GB out): %.3f GDOF-RHS/s."
+           % (d["e2e"]["h2d_bytes_per_step"] / 1e9, d["e2e"]["d2h_bytes_per_step"] / 1e9, d["e2e"]["value"]),
+           "* one right-hand side as an RK stage runs it (`fr_profile_stage_kernels`, CUDA events, mean of 3): operator products incl. fused point-wise "
+           "work %.1f ms, stand-alone point-wise (S6) %.1f ms, interface kernels %.1f ms; total %.1f ms."
+           % (d["kernel_groups"]["operator_products_incl_fused_pointwise_ms"], d["kernel_groups"]["pointwise_flux_ms"],
+              d["kernel_groups"]["interface_ms"], d["kernel_groups"]["total_ms"]), "",
+           "| kernel | ms | share | algorithmic GB/s | of %.0f GB/s | TFLOP/s | of %.1f |" % (hbm, peak), "|---|---|---|---|---|---|---|"]
+    for k in ks:
+        gbs, tf = k["alg_bytes"] / k["ms"] / 1e6, k["flops"] / k["ms"] / 1e9
+        out.append("| %s | %.2f | %.1f %% | %.0f | %.0f %% | %.1f | %.0f %% |" % (k["name"], k["ms"], 100 * k["ms"] / tot, gbs, 100 * gbs / hbm, tf, 100 * tf / peak))
+    out += ["", "Plan chosen by `fr_setup` (`fr_plan_describe`):", "", "```"] + list(d["plan"]) + ["```", ""]
+    return "\n".join(out)
+
+
 def main():
+    if len(sys.argv) == 3 and sys.argv[1] == "--gemm":
+        print(gemm_table(load(sys.argv[2])))
+        return
     ap = argparse.ArgumentParser()
     ap.add_argument("bench")
     ap.add_argument("--traffic", default=None)
@@ -35,6 +79,9 @@ def main():
         for r in csv.reader(open(args.traffic)):
             if len(r) >= 8:
                 traffic[(r[0], r[1])] = dict(dram=float(r[2]), pipe64=float(r[6]), pipe32=float(r[7]))
+    if "kernels_f64" not in d or "fp32" not in d:
+        sys.stdout.write(single_table(d))
+        return
     hbm = d["roofline"]["hbm"]["peak"]
     pk = d["peaks"]
     peak = {"f64": pk["fp64_tensor_tflops"], "f32": pk["fp32_ffma_tflops"]}
