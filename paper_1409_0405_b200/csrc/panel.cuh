@@ -333,7 +333,10 @@ bool panel_op_build(PanelOp<T> &p, int M, int K, const double *A, const std::vec
       ++si;
     }
   };
-  make_chunks(PANEL_KCMAX);
+  // Long stacked operands (the fused divergence operator of prisms at p >= 4: K = 330) take chunks of at most 32 rows: their packed image
+  // leaves the ring only two 40-row stages per warp group, and a third stage is worth more than the per-chunk overhead it costs
+  // (pri S8-S10 FP64 0.82 -> 0.72 ms; every shorter operand is slower with lower chunks).  A function of the operator alone.
+  make_chunks((srcs.size() == 2 && K >= 300) ? 32 : PANEL_KCMAX);
   int nchunks = (int)chunks.size();
   if (nchunks > PANEL_MAXCHUNKS) return false;
 
