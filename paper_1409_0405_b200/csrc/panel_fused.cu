@@ -56,6 +56,7 @@ struct VecIO<float, 1> {
 // K = -R/|J| (S9), then the stage update out1 = in1 + c1 K, out2 = in2 + c2 K (S10) or plain out1 = K
 template <typename T>
 struct RkEpilogue {
+  static constexpr bool kProducerPrefetch = false;
   const T *rcpdjac;
   long long ld, neles;
   int curved, NE;
@@ -190,12 +191,27 @@ __global__ void __launch_bounds__(32 * panel_maxw<T>(NIT, CX)) k_fused_div(const
 
 // ------------------------------------------------------------------------------------------------ fused_grad
 // epilogue S4: physical gradient from the three reference components held by one thread
-template <typename T>
-struct GradEpilogue {
+// PF: per-point metric terms (curved / non-affine types) prefetched into L2 by the producer warp; a compile-time variant, so that
+// the kernels of affine types stay as they are
+struct EpiNoMaps {};
+struct EpiMetricMaps {
+  CUtensorMap tm_s, tm_j;   // smats [9][nupts][ld], rcpdjac [1][nupts][ld], boxes of one panel
+};
+template <typename T, bool PF>
+struct GradEpilogue : std::conditional_t<PF, EpiMetricMaps, EpiNoMaps> {
   const T *smats, *rcpdjac;
   T *grad;                  // [3][Nu][5][ld]  physical gradients G (read again by S5 and S6)
   long long ld, neles;
   int nupts, curved, NE;
+  // PF: the panel's metric terms through the maps, one instruction per array and panel, so that the epilogue's loads are L2 hits
+  // without costing the consumer warps anything
+  static constexpr bool kProducerPrefetch = PF;
+  __device__ __forceinline__ void producer_prefetch(long long pl) const {
+    if constexpr (PF) {
+      tma_prefetch_3d(&this->tm_s, (int)(pl * NE), 0, 0);
+      tma_prefetch_3d(&this->tm_j, (int)(pl * NE), 0, 0);
+    }
+  }
   template <typename ACC>
   __device__ __forceinline__ void prefetch(ACC &acc, const int *rowmap, int slot0, long long, long long pl, int wc, int lane) const {
     const long long e0 = pl * NE;
@@ -277,19 +293,19 @@ struct GradEpilogue {
   }
 };
 
-template <typename T>
+template <typename T, bool PF>
 struct alignas(64) GradArgs {
   TmaProducer<T> prod;
   PanelOp<T> op;
-  GradEpilogue<T> epi;
+  GradEpilogue<T, PF> epi;
   long long npanels;
 };
 
-template <typename T, int NIT, int CX>
-__global__ void __launch_bounds__(32 * panel_maxw<T>(NIT, CX, true)) k_fused_grad(const __grid_constant__ GradArgs<T> a) {
+template <typename T, int NIT, int CX, bool PF>
+__global__ void __launch_bounds__(32 * panel_maxw<T>(NIT, CX, true)) k_fused_grad(const __grid_constant__ GradArgs<T, PF> a) {
   extern __shared__ __align__(1024) char panel_smem[];
   // FP32: the scalar accumulator form (panel.cuh: the packed pairs do not fit this kernel's register budget)
-  panel_mainloop<T, NIT, CX, TmaProducer<T>, GradEpilogue<T>, false>(a.op, a.prod, a.epi, a.npanels, 1, panel_smem);
+  panel_mainloop<T, NIT, CX, TmaProducer<T>, GradEpilogue<T, PF>, false>(a.op, a.prod, a.epi, a.npanels, 1, panel_smem);
 }
 
 }  // namespace
@@ -379,21 +395,36 @@ bool fused_grad_build(PanelOp<T> &op, int nu, int nf, const double *M460, const 
   return panel_op_build(op, M, K, A.data(), srcs, opt, 150 * 1024);
 }
 
-template <typename T>
-int launch_fused_grad(const PanelOp<T> &op, const EleView<T> &ev, const T *u, const T *c, T *grad, cudaStream_t s) {
-  GradArgs<T> a;
+namespace {
+template <typename T, bool PF>
+int launch_fused_grad_pf(const PanelOp<T> &op, const EleView<T> &ev, const T *u, const T *c, T *grad, cudaStream_t s) {
+  GradArgs<T, PF> a;
   a.op = op;
-  // The epilogue's metric terms are pulled into L2 while the panel's first chunk is multiplied; with per-point terms in FP64
-  // (20 lines per thread) the prefetch costs more than the latency it hides (pri S3+S4 0.94 -> 1.04 ms).
-  a.op.pf_epi = (ev.affine || sizeof(T) == 4) ? 1 : 0;
+  // Affine types and FP32: the consumers pull the epilogue's metric terms into L2 while the panel's first chunk is multiplied; with
+  // per-point terms in FP64 (20 lines per thread) that costs more than the latency it hides (pri S3+S4 0.94 -> 1.04 ms).  PF: the
+  // producer warp prefetches them instead, and the consumers issue nothing.
+  a.op.pf_epi = PF ? 0 : ((ev.affine || sizeof(T) == 4) ? 1 : 0);
   a.prod.tm[0] = tmap_state(u, (long long)ev.nupts, ev.ld, op.NE, op.src_step[0]);
   a.prod.tm[1] = tmap_state(c, (long long)ev.nfpts, ev.ld, op.NE, op.src_step[1]);
   a.prod.plain = 0;
-  a.epi = GradEpilogue<T>{ev.smats, ev.rcpdjac, grad, ev.ld, ev.neles, ev.nupts, ev.affine ? 0 : 1, op.NE};
+  a.epi.smats = ev.smats;
+  a.epi.rcpdjac = ev.rcpdjac;
+  a.epi.grad = grad;
+  a.epi.ld = ev.ld;
+  a.epi.neles = ev.neles;
+  a.epi.nupts = ev.nupts;
+  a.epi.curved = ev.affine ? 0 : 1;
+  a.epi.NE = op.NE;
+  if constexpr (PF) {
+    bool ok1 = false, ok2 = false;
+    a.epi.tm_s = tmap_epi(ev.smats, 9, (long long)ev.nupts, ev.ld, op.NE, ok1);
+    a.epi.tm_j = tmap_epi(ev.rcpdjac, 1, (long long)ev.nupts, ev.ld, op.NE, ok2);
+    FR_REQUIRE(ok1 && ok2, "launch_fused_grad: metric maps");
+  }
   a.npanels = ev.ld / op.NE;
 #define FR_CASE(NIT_, CX_)                                                          \
   if (op.NIT == NIT_ && op.CX == CX_) {                                             \
-    panel_launch(k_fused_grad<T, NIT_, CX_>, a, op, a.npanels, s);                  \
+    panel_launch(k_fused_grad<T, NIT_, CX_, PF>, a, op, a.npanels, s);              \
     return 1;                                                                       \
   }
   if constexpr (sizeof(T) == 8) {
@@ -403,6 +434,14 @@ int launch_fused_grad(const PanelOp<T> &op, const EleView<T> &ev, const T *u, co
   }
 #undef FR_CASE
   throw Error{FR_ESTATE, "launch_fused_grad: no kernel for this accumulator shape"};
+}
+}  // namespace
+
+template <typename T>
+int launch_fused_grad(const PanelOp<T> &op, const EleView<T> &ev, const T *u, const T *c, T *grad, cudaStream_t s) {
+  // per-point metric terms within the box limits of a tensor map (256 rows): producer-side prefetch
+  if (!ev.affine && ev.nupts <= 256) return launch_fused_grad_pf<T, true>(op, ev, u, c, grad, s);
+  return launch_fused_grad_pf<T, false>(op, ev, u, c, grad, s);
 }
 
 #define FR_INST(T)                                                                                                          \

@@ -50,6 +50,7 @@ struct alignas(64) TmaProducer {
 // stores the accumulators as they are: no FP64 instruction in the epilogue, which would queue behind the other warps' DMMAs.
 template <typename T>
 struct PlainEpilogue {
+  static constexpr bool kProducerPrefetch = false;
   T *C;
   long long ldc, bstride;
   ColMap cm;
@@ -196,6 +197,10 @@ __device__ __forceinline__ void panel_mainloop(const PanelOp<T> &op, const Prod 
         prod.issue(cd, batch, pl, gring + stage * stage_bytes, full, NE);
         if (STREAM)
           bulk_load(gring + stage * stage_bytes + (uint32_t)op.a_off(), reinterpret_cast<const char *>(op.vals) + (size_t)cd.base * ablk, abytes, full);
+        // with the panel's last chunk on its way, pull what its epilogue will read into L2 (epilogues that have tensor maps for it)
+        if constexpr (Epi::kProducerPrefetch) {
+          if (c == nchunks - 1) epi.producer_prefetch(pl);
+        }
         if (++stage == nstage) {
           stage = 0;
           phase ^= 1u;

@@ -11,6 +11,7 @@
 // PAPER.md:37 eq. 1 (fr_gemm, S1, S5) with one copy per 16-column (FP64) / NE-column (FP32) block, ragged N and K
 // zero-filled by the copy itself.
 #pragma once
+#include <cstring>
 #include <cuda.h>
 
 #include "common.cuh"
@@ -83,7 +84,31 @@ inline CUtensorMap tmap_plain(const T *p, long long K, long long N, long long ld
   return tm;
 }
 
+// What a fused epilogue reads per panel, for prefetching into L2 by the producer warp (cp.async.bulk.prefetch.tensor: one instruction
+// for the whole box, no shared memory): an array [nplanes][rows][ld] (nplanes * rows metric terms or stage-register rows of NE
+// elements each).  Boxes are limited to 256 per dimension: ok = false beyond that (the caller then skips the prefetch).
+template <typename T>
+inline CUtensorMap tmap_epi(const T *p, int nplanes, long long rows, long long ld, int NE, bool &ok) {
+  CUtensorMap tm;
+  memset(&tm, 0, sizeof tm);
+  ok = rows >= 1 && rows <= 256 && nplanes >= 1 && nplanes <= 256;
+  if (!ok) return tm;
+  const cuuint32_t es[3] = {1, 1, 1};
+  const cuuint64_t dims[3] = {(cuuint64_t)ld, (cuuint64_t)rows, (cuuint64_t)nplanes};
+  const cuuint64_t strides[2] = {(cuuint64_t)ld * sizeof(T), (cuuint64_t)rows * ld * sizeof(T)};
+  const cuuint32_t box[3] = {(cuuint32_t)NE, (cuuint32_t)rows, (cuuint32_t)nplanes};
+  tmap_check(tmap_encode_fn()(&tm, tmap_dtype<T>(), 3, (void *)p, dims, strides, box, es, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                              CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE),
+             "an epilogue operand");
+  return tm;
+}
+
 #ifdef __CUDACC__
+
+// the box at (c0, c1, c2) into L2; nothing to wait for
+__device__ __forceinline__ void tma_prefetch_3d(const CUtensorMap *tm, int c0, int c1, int c2) {
+  asm volatile("cp.async.bulk.prefetch.tensor.3d.L2.global.tile [%0, {%1, %2, %3}];" ::"l"(tm), "r"(c0), "r"(c1), "r"(c2) : "memory");
+}
 
 __device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
 
