@@ -214,10 +214,10 @@ struct PackOptions {
 
 // Rows per chunk of a source with `rows` rows: the multiple of 8 (<= PANEL_KCMAX) with the fewest chunks, counting a fixed
 // per-chunk overhead worth six rows.  A function of `rows` alone (see the determinism note at the top).
-inline int panel_chunk_step(int rows) {
+inline int panel_chunk_step(int rows, int cap = PANEL_KCMAX) {
   int best = 8;
   long bestc = 1l << 60;
-  for (int step = 8; step <= PANEL_KCMAX; step += 8) {
+  for (int step = 8; step <= cap; step += 8) {
     const long nch = (rows + step - 1) / step;
     const long c = nch * (step + 6);
     if (c <= bestc) {
@@ -323,7 +323,7 @@ bool panel_op_build(PanelOp<T> &p, int M, int K, const double *A, const std::vec
     chunk_k0.clear();
     int k0 = 0, si = 0;
     for (auto &s : srcs) {
-      const int step = std::min(panel_chunk_step(s.rows), step_cap);
+      const int step = std::min(panel_chunk_step(s.rows, std::max(step_cap, PANEL_KCMAX)), step_cap);
       src_step[si] = step;
       for (int r = 0; r < s.rows; r += step) {
         chunks.push_back(ChunkDesc{si, r, std::min(step, s.rows - r), step, 0, 0, 0, 0});
@@ -335,8 +335,9 @@ bool panel_op_build(PanelOp<T> &p, int M, int K, const double *A, const std::vec
   };
   // Long stacked operands (the fused divergence operator of prisms at p >= 4: K = 330) take chunks of at most 32 rows: their packed image
   // leaves the ring only two 40-row stages per warp group, and a third stage is worth more than the per-chunk overhead it costs
-  // (pri S8-S10 FP64 0.82 -> 0.72 ms; every shorter operand is slower with lower chunks).  A function of the operator alone.
-  make_chunks((srcs.size() == 2 && K >= 300) ? 32 : PANEL_KCMAX);
+  // (pri S8-S10 FP64 0.82 -> 0.72 ms; every shorter operand is slower with lower chunks; in FP32 the image is half the size and the
+  // rule does not apply).  A function of the operator alone.
+  make_chunks((f64 && srcs.size() == 2 && K >= 300) ? 32 : PANEL_KCMAX);
   int nchunks = (int)chunks.size();
   if (nchunks > PANEL_MAXCHUNKS) return false;
 
@@ -406,12 +407,31 @@ bool panel_op_build(PanelOp<T> &p, int M, int K, const double *A, const std::vec
       lists = sl;
     }
   }
+  // k-list operators take chunks of up to 128 rows (one chunk per operand of configs 1-3): a group's k-list is cut into blocks of four per
+  // chunk, so every chunk boundary leaves a partly filled block -- fewer chunks, fewer multiplies (pri S3+S4 0.95 -> 0.82 ms FP64, 0.59 ->
+  // 0.53 FP32; tet S3+S4 1.29 -> 1.26; dense operators are slower with chunks above 40 rows, their block count does not depend on it).
+  // Still a function of the operator alone: if no geometry fits shared memory with the high chunks, all candidates use the default ones.
+  const int default_cap = (f64 && srcs.size() == 2 && K >= 300) ? 32 : PANEL_KCMAX;
+  bool high_chunks = sparse && !opt.stream && default_cap == PANEL_KCMAX;
+  if (high_chunks) {
+    make_chunks(128);
+    nchunks = (int)chunks.size();
+    lists = make_lists(order);
+  }
   const int G = (int)order.size() / 8;
 
   // ---- geometry: candidate k = the k-th geometry of the list that fits shared memory
   const std::vector<PanelGeom> geoms = list_geoms<T>(G, opt.min_ne, opt.max_ne, opt.triple, !sparse);
   if (opt.cand < 0) return false;
   int nfit = 0;
+  for (int attempt = 0; attempt < 2; ++attempt) {
+  if (attempt == 1) {
+    if (!high_chunks || nfit > 0) break;   // the candidate does not exist, or there is nothing else to try
+    high_chunks = false;
+    make_chunks(default_cap);
+    nchunks = (int)chunks.size();
+    lists = make_lists(order);
+  }
   for (const PanelGeom &geo : geoms) {
     size_t smem_total = smem_total_in;
     if (geo.occ == 2) smem_total = smem_total / 2 - 1024;
@@ -633,6 +653,7 @@ bool panel_op_build(PanelOp<T> &p, int M, int K, const double *A, const std::vec
     up(p.rowmap, rowmap);
     up(p.chunks, chunks);
     return true;
+  }
   }
   return false;
 }
