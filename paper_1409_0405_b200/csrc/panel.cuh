@@ -407,12 +407,12 @@ bool panel_op_build(PanelOp<T> &p, int M, int K, const double *A, const std::vec
       lists = sl;
     }
   }
-  // k-list operators take chunks of up to 128 rows (one chunk per operand of configs 1-3): a group's k-list is cut into blocks of four per
-  // chunk, so every chunk boundary leaves a partly filled block -- fewer chunks, fewer multiplies (pri S3+S4 0.95 -> 0.82 ms FP64, 0.59 ->
-  // 0.53 FP32; tet S3+S4 1.29 -> 1.26; dense operators are slower with chunks above 40 rows, their block count does not depend on it).
-  // Still a function of the operator alone: if no geometry fits shared memory with the high chunks, all candidates use the default ones.
+  // k-list operators take chunks of up to 128 rows (one chunk per operand of configs 1-3).  FP64: a group's k-list is cut into blocks of four
+  // per chunk, so every chunk boundary leaves a partly filled block -- fewer chunks, fewer multiplies (pri S3+S4 0.95 -> 0.82 ms, tet S3+S4
+  // 1.29 -> 1.26; dense operators are slower with chunks above 40 rows, their block count does not depend on it).  Still a function of the
+  // operator alone: if no geometry fits shared memory with the high chunks, all candidates use the default ones.  FP32: see the geometry loop.
   const int default_cap = (f64 && srcs.size() == 2 && K >= 300) ? 32 : PANEL_KCMAX;
-  bool high_chunks = sparse && !opt.stream && default_cap == PANEL_KCMAX;
+  bool high_chunks = f64 && sparse && !opt.stream && default_cap == PANEL_KCMAX;
   if (high_chunks) {
     make_chunks(128);
     nchunks = (int)chunks.size();
@@ -581,7 +581,18 @@ bool panel_op_build(PanelOp<T> &p, int M, int K, const double *A, const std::vec
       return true;
     };
     bool fits = false;
-    if (!opt.stream) {
+    if (!f64 && sparse && !opt.stream) {
+      // FP32 k-lists hold single rows, in increasing order whatever the chunking: the chunk height may follow the geometry without
+      // changing a bit of the result.  The highest chunks (fewest chunk boundaries: pri S3+S4 0.59 -> 0.53 ms) that leave this
+      // geometry's panel width a ring of two stages.
+      for (int cap : {128, 96, 64, PANEL_KCMAX}) {
+        make_chunks(cap);
+        nchunks = (int)chunks.size();
+        lists = make_lists(order);
+        fits = pack();
+        if (fits) break;
+      }
+    } else if (!opt.stream) {
       fits = pack();
     } else {
       // the highest chunks that leave a ring of four stages; failing that, the deepest ring any chunk height gives
