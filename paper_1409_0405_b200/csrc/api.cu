@@ -426,7 +426,11 @@ struct Ctx : CtxBase {
       std::string tag = std::string(tname[t]);
       if (e.pM0.pop)
         tune(*e.pM0.pop, [&](PanelOp<T> &op, int k) { return panel_gemm_build(op, nf, nu, d.M0, k); },
-             [&](const PanelOp<T> &op) { panel_gemm_run(op, n5, T(1), (const T *)e.X.p, n5, 0, T(0), ufp, n5, 0, 1, stream); },
+             [&](const PanelOp<T> &op) {
+               // both uses of M0: S1, and (Navier-Stokes) S5 on the three gradient components, which is three quarters of its time
+               panel_gemm_run(op, n5, T(1), (const T *)e.X.p, n5, 0, T(0), ufp, n5, 0, 1, stream);
+               if (ns) panel_gemm_run(op, n5, T(1), (const T *)e.grad.p, n5, (long long)nu * n5, T(0), gf.p + tt.gbase[t], n5, tt.gcomp[t], 3, stream);
+             },
              (tag + ":M0").c_str());
       StageArgs<T> plain{nullptr, nullptr, nullptr, e.R.p, nullptr};
       for (auto &q : e.pDiv)

@@ -183,10 +183,10 @@ struct alignas(64) DivArgs {
   long long npanels;
 };
 
-template <typename T, int NIT, int CX>
+template <typename T, int NIT, int CX, bool DYN>
 __global__ void __launch_bounds__(32 * panel_maxw<T>(NIT, CX)) k_fused_div(const __grid_constant__ DivArgs<T> a) {
   extern __shared__ __align__(1024) char panel_smem[];
-  panel_mainloop<T, NIT, CX>(a.op, a.prod, a.epi, a.npanels, 1, panel_smem);
+  panel_mainloop<T, NIT, CX, TmaProducer<T>, RkEpilogue<T>, true, false, DYN>(a.op, a.prod, a.epi, a.npanels, 1, panel_smem);
 }
 
 // ------------------------------------------------------------------------------------------------ fused_grad
@@ -301,11 +301,11 @@ struct alignas(64) GradArgs {
   long long npanels;
 };
 
-template <typename T, int NIT, int CX, bool PF>
+template <typename T, int NIT, int CX, bool PF, bool DYN>
 __global__ void __launch_bounds__(32 * panel_maxw<T>(NIT, CX, true)) k_fused_grad(const __grid_constant__ GradArgs<T, PF> a) {
   extern __shared__ __align__(1024) char panel_smem[];
   // FP32: the scalar accumulator form (panel.cuh: the packed pairs do not fit this kernel's register budget)
-  panel_mainloop<T, NIT, CX, TmaProducer<T>, GradEpilogue<T, PF>, false>(a.op, a.prod, a.epi, a.npanels, 1, panel_smem);
+  panel_mainloop<T, NIT, CX, TmaProducer<T>, GradEpilogue<T, PF>, false, false, DYN>(a.op, a.prod, a.epi, a.npanels, 1, panel_smem);
 }
 
 }  // namespace
@@ -348,7 +348,8 @@ int launch_fused_div(const PanelOp<T> &op, const EleView<T> &ev, const T *ftil, 
   a.npanels = ev.ld / op.NE;
 #define FR_CASE(NIT_, CX_)                                                          \
   if (op.NIT == NIT_ && op.CX == CX_) {                                             \
-    panel_launch(k_fused_div<T, NIT_, CX_>, a, op, a.npanels, s);                   \
+    if (panel_use_units(op)) panel_launch(k_fused_div<T, NIT_, CX_, true>, a, op, a.npanels, s); \
+    else panel_launch(k_fused_div<T, NIT_, CX_, false>, a, op, a.npanels, s);       \
     return 1;                                                                       \
   }
   if constexpr (sizeof(T) == 8) {
@@ -424,7 +425,8 @@ int launch_fused_grad_pf(const PanelOp<T> &op, const EleView<T> &ev, const T *u,
   a.npanels = ev.ld / op.NE;
 #define FR_CASE(NIT_, CX_)                                                          \
   if (op.NIT == NIT_ && op.CX == CX_) {                                             \
-    panel_launch(k_fused_grad<T, NIT_, CX_, PF>, a, op, a.npanels, s);              \
+    if (panel_use_units(op)) panel_launch(k_fused_grad<T, NIT_, CX_, PF, true>, a, op, a.npanels, s); \
+    else panel_launch(k_fused_grad<T, NIT_, CX_, PF, false>, a, op, a.npanels, s);  \
     return 1;                                                                       \
   }
   if constexpr (sizeof(T) == 8) {

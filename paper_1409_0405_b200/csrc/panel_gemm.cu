@@ -14,10 +14,10 @@ struct alignas(64) PlainArgs {
   int nbatch;
 };
 
-template <typename T, int NIT, int CX, bool STREAM>
+template <typename T, int NIT, int CX, bool STREAM, bool DYN>
 __global__ void __launch_bounds__(32 * panel_maxw<T>(NIT, CX)) k_panel_gemm(const __grid_constant__ PlainArgs<T> a) {
   extern __shared__ __align__(1024) char panel_smem[];
-  panel_mainloop<T, NIT, CX, TmaProducer<T>, PlainEpilogue<T>, true, STREAM>(a.op, a.prod, a.epi, a.npanels, a.nbatch, panel_smem);
+  panel_mainloop<T, NIT, CX, TmaProducer<T>, PlainEpilogue<T>, true, STREAM, DYN>(a.op, a.prod, a.epi, a.npanels, a.nbatch, panel_smem);
 }
 
 }  // namespace
@@ -48,10 +48,15 @@ void panel_gemm_run(const PanelOp<T> &op, long long N, T c1, const T *B, long lo
   a.epi = PlainEpilogue<T>{C, ldc, bsC, cm, c1, c2, (c1 == T(1) && c2 == T(0)) ? 1 : 0};
   a.npanels = (N + pw - 1) / pw;
   a.nbatch = nbatch;
+  const bool units = panel_use_units(op);
 #define FR_CASE(NIT_, CX_)                                                                        \
   if (op.NIT == NIT_ && op.CX == CX_) {                                                           \
-    if (op.streamed()) panel_launch(k_panel_gemm<T, NIT_, CX_, true>, a, op, a.npanels * a.nbatch, s); \
-    else panel_launch(k_panel_gemm<T, NIT_, CX_, false>, a, op, a.npanels * a.nbatch, s);          \
+    /* one warp group: the consumer warps take units from a counter (panel_kernel.cuh DYN) */     \
+    if (units) {                                                                   \
+      if (op.streamed()) panel_launch(k_panel_gemm<T, NIT_, CX_, true, true>, a, op, a.npanels * a.nbatch, s); \
+      else panel_launch(k_panel_gemm<T, NIT_, CX_, false, true>, a, op, a.npanels * a.nbatch, s); \
+    } else if (op.streamed()) panel_launch(k_panel_gemm<T, NIT_, CX_, true, false>, a, op, a.npanels * a.nbatch, s); \
+    else panel_launch(k_panel_gemm<T, NIT_, CX_, false, false>, a, op, a.npanels * a.nbatch, s);  \
     return;                                                                                       \
   }
   if constexpr (sizeof(T) == 8) {

@@ -127,7 +127,11 @@ struct PlainEpilogue {
 // `prod` must refer to the kernel's __grid_constant__ parameter.
 // STREAM: the operator's packed blocks travel through the ring (PanelOp::stream; plain products only -- a compile-time switch so that
 // the kernels of resident operators carry none of it).
-template <typename T, int NIT, int CX, class Prod, class Epi, bool PACKED = true, bool STREAM = false>
+// DYN (one warp group): the consumer warps take (panel, warp role) units from a shared counter instead of keeping a fixed role.  The
+// FP64 tensor pipe is per SM sub-partition, and ten consumer warps sit 3/3/2/2 on the four of them: with fixed roles the warps of the
+// crowded sub-partitions set the pace and the others wait at the ring; with units, a warp that runs faster simply takes more of them.
+// Results do not depend on which warp computes a unit.
+template <typename T, int NIT, int CX, class Prod, class Epi, bool PACKED = true, bool STREAM = false, bool DYN = false>
 __device__ __forceinline__ void panel_mainloop(const PanelOp<T> &op, const Prod &prod, const Epi &epi, long long npanels_per_batch,
                                                int nbatch, char *smem_raw) {
   const int WC = op.WC, NS = op.NS, NE = op.NE, NG = op.NG;
@@ -151,6 +155,7 @@ __device__ __forceinline__ void panel_mainloop(const PanelOp<T> &op, const Prod 
     }
     mbar_init(bar_img, 1);
     mbar_fence_init();
+    if (DYN) *reinterpret_cast<int *>(smem_raw + (bar_img + 16u - s0)) = 0;   // the unit counter
   }
   __syncthreads();
   OpSmem<T> A;
@@ -231,6 +236,34 @@ __device__ __forceinline__ void panel_mainloop(const PanelOp<T> &op, const Prod 
   }
   Acc<T, NIT, CX, PACKED> acc;
   acc.zero();
+  if constexpr (DYN) {
+    int *ctr = reinterpret_cast<int *>(smem_raw + (bar_img + 16u - s0));
+    const int nunits = mine * nwc;
+    for (;;) {
+      int U = 0;
+      if (lane == 0) U = atomicAdd(ctr, 1);
+      U = __shfl_sync(0xffffffffu, U, 0);
+      if (U >= nunits) break;
+      const int pi = U / nwc, role = U - pi * nwc;         // panel of this CTA's sequence, warp role in it
+      const int uwr = role / WC, uwc = role - uwr * WC;
+      const long long pabs = (long long)first + (long long)pi * stride;
+      const int ubatch = (int)(pabs / npb), upl = (int)(pabs - (long long)ubatch * npb);
+      for (int c = 0; c < nchunks; ++c) {
+        const int q = pi * nchunks + c;                    // the chunk's number in the ring: stage and phase follow from it
+        const int stg = q % nstage;
+        mbar_wait(gbar + stg * 16, (uint32_t)(q / nstage) & 1u);
+        const char *st = ringp + (size_t)stg * stage_bytes;
+        if (c == 0 && op.pf_epi) epi.prefetch(acc, A.rowmap, uwr * NIT, ubatch, upl, uwc, lane);
+        if (op.sparse) acc.mac_chunk(A, c, A.chunks[c], NS, uwr * NIT, st, NE, uwc, lane);
+        else acc.template mac_dense<STREAM>(A, A.chunks[c], NS, uwr * NIT, st, NE, uwc, lane, STREAM ? op.a_off() : 0);
+        __syncwarp();
+        if (lane == 0) mbar_arrive(gbar + stg * 16 + 8);
+      }
+      epi(acc, A.rowmap, uwr * NIT, ubatch, upl, uwc, lane);
+      acc.zero();
+    }
+    return;
+  }
   int stage = 0, cc = 0;
   uint32_t phase = 0;
   for (int q = 0; q < total; ++q) {
@@ -266,6 +299,13 @@ __device__ __forceinline__ void panel_mainloop(const PanelOp<T> &op, const Prod 
       }
     }
   }
+}
+
+// Units (DYN) pay an atomic and an index computation per unit: worth it where fixed roles leave the sub-partitions unevenly loaded,
+// i.e. where the consumer warps of the one group are not a multiple of four.  FRB_NO_DYN=1: fixed roles everywhere.
+template <typename T>
+inline bool panel_use_units(const PanelOp<T> &op) {
+  return op.NG == 1 && (op.WR * op.WC) % 4 != 0 && getenv("FRB_NO_DYN") == nullptr;
 }
 
 // Dispatch over the compile-time accumulator shapes.  FP64: NIT*CX <= 8; FP32: NIT*CX <= 4.
