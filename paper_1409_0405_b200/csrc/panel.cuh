@@ -7,14 +7,15 @@
 // B200 design:
 //   * the operator is packed once at fr_setup into 8-row groups (dense operators: every k of a chunk, in k-blocks shared by
 //     all groups; sparse operators: per group a compact list of the k that are non-zero in it) and stays resident in shared
-//     memory for the life of the persistent CTA;
+//     memory for the life of the persistent CTA (plain products whose image exceeds shared memory stream the packed blocks
+//     through the ring instead: PanelOp::streamed);
 //   * B chunks are moved by the TMA unit (cp.async.bulk.tensor from tensor maps over the state matrices, tma.cuh): a producer
 //     warp per warp group issues the copies into a ring of stages, each stage guarded by a full and an empty mbarrier; the
 //     consumer warps never issue a copy and never meet at a CTA-wide barrier;
 //   * FP64 multiplies on the FP64 tensor pipe, mma.sync.m8n8k4.f64 (DMMA), reading its B fragments from the 128-byte-swizzled
 //     stage; the four rows of a k-block are chosen at set-up so that these loads are bank-conflict free;
-//     FP32 multiplies with FFMA on register tiles of 8 rows x 5 variables x (1|2) elements (no TF32: the 2e-5 parity
-//     bound excludes it, and tcgen05 has no FP32/FP64 kind);
+//     FP32 multiplies on register tiles of 8 rows x 5 variables x (1|2) elements with packed fma.rn.f32x2 (two IEEE FP32 FMAs per
+//     instruction; the gradient kernels keep scalar FFMA) -- no TF32: the 2e-5 parity bound excludes it, and tcgen05 has no FP32/FP64 kind;
 //   * the chunking of K and the composition of every k-block depend on the operator alone, never on the launch geometry, so
 //     every geometry the autotuner may pick gives bit-identical results;
 //   * epilogues (what happens to the accumulators) are policies, which is how the gradient transform, the -1/|J| scaling and

@@ -6,7 +6,8 @@
 //   consumers: wait on the full barrier, multiply the chunk into their register accumulators, release the stage (one arrive
 //     per warp on the empty barrier), and after the panel's last chunk run the epilogue on their own rows and columns.
 // No warp ever waits for another consumer warp: a warp in its (latency-bound) epilogue leaves the tensor pipe to the warps that
-// are already multiplying the next panel, as far ahead as the ring is deep.
+// are already multiplying the next panel, as far ahead as the ring is deep.  In plans with one warp group whose consumer warps are
+// not a multiple of four, the warps do not even keep a fixed (row, column) role: they take (panel, role) units from a counter (DYN).
 #pragma once
 #include "panel.cuh"
 #include "tma.cuh"
